@@ -1,0 +1,316 @@
+/* perm_oracle.c -- CPU oracle for the permutation-operator matrix P0.
+ *
+ * TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).  Plain FP64 C, written from
+ * PAPER.md Appendix A; shares no code with the CUDA path.  Build:
+ *   gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC perm_oracle.c -lm
+ * (-ffp-contract=off: the overlap predicate is an IEEE +,-,*,/ contract, R6).
+ *
+ * Notation (A6/A7):
+ *   row cell    (i ,j ): p  in [L2,U2] = [p_{i-1},p_i],    q  in [a,b] = [q_{j-1},q_j]
+ *   column cell (i',j'): p' in [L1,U1] = [p_{i'-1},p_{i'}], q' in [c,d] = [q_{j'-1},q_{j'}]
+ *   pi1 = sqrt(q^2 + q'^2/4 + q q' x) goes with p', pi2 = sqrt(q^2/4 + q'^2 + q q' x) with p (A2).
+ *   In the (q,q') plane a point is written (s,t).
+ *
+ * Functions
+ *   wpo_overlap        structural-nonzero predicate S (R6) + the polygon Pi
+ *   wpo_geo_count/fill geometric CSR pattern (rows (i,j), columns (i',j') ascending)
+ *   wpo_elements       values of listed geometric elements for all coupled channel
+ *                      pairs by the rule R(n) (R7) applied to (A15)
+ *   wpo_spmv           sequential CSR y = P0 x
+ *
+ * Pins: tests/test_oracle_*.py (Cartesian (A7) brute force, single-cell constant,
+ * symmetric-state eigenvalue 2 g0, spectrum bound, symmetry, point sampling of
+ * the theta-product for the pattern).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define WPO_MAXV 16 /* rectangle (4) + at most one new vertex per half-plane (6) */
+
+typedef struct { double s, t; } wpo_pt;
+
+/* The six half-planes of DESIGN.md R6; inside <=> value >= 0. */
+static double halfplane(int m, double s, double t, double L1, double U1, double L2, double U2)
+{
+    switch (m) {
+    case 0: return (s + 0.5 * t) - L1;   /* q + q'/2 >= L1   (pi1 can reach L1 from above) */
+    case 1: return U1 - (s - 0.5 * t);   /* q - q'/2 <= U1 */
+    case 2: return U1 - (0.5 * t - s);   /* q'/2 - q <= U1 */
+    case 3: return (0.5 * s + t) - L2;   /* q/2 + q' >= L2 */
+    case 4: return U2 - (t - 0.5 * s);   /* q' - q/2 <= U2 */
+    default: return U2 - (0.5 * s - t);  /* q/2 - q' <= U2 */
+    }
+}
+
+/* Sutherland-Hodgman clip of a convex polygon by half-plane m. */
+static int clip_polygon(const wpo_pt* in, int n, wpo_pt* out, int m,
+                        double L1, double U1, double L2, double U2)
+{
+    int no = 0;
+    for (int e = 0; e < n; ++e) {
+        wpo_pt P = in[e], Q = in[(e + 1) % n];
+        double fP = halfplane(m, P.s, P.t, L1, U1, L2, U2);
+        double fQ = halfplane(m, Q.s, Q.t, L1, U1, L2, U2);
+        int inP = fP >= 0.0, inQ = fQ >= 0.0;
+        if (inP) out[no++] = P;
+        if (inP != inQ) {
+            double r = fP / (fP - fQ);
+            wpo_pt I;
+            I.s = P.s + (Q.s - P.s) * r;
+            I.t = P.t + (Q.t - P.t) * r;
+            out[no++] = I;
+        }
+    }
+    return no;
+}
+
+/* Structural-nonzero predicate (R6).  Returns 1 and the polygon Pi
+ * (nv vertices, counter-clockwise) if the cells overlap with positive measure. */
+int wpo_overlap(double a, double b, double c, double d,
+                double L1, double U1, double L2, double U2,
+                wpo_pt* poly, int* nv_out)
+{
+    /* energy band  L2^2-U1^2 < h(s,t) = 3/4 (t^2 - s^2) < U2^2-L1^2  */
+    double h_lo = L2 * L2 - U1 * U1;
+    double h_hi = U2 * U2 - L1 * L1;
+    /* (1) box tests, all necessary conditions */
+    if (!(0.75 * (d * d - a * a) > h_lo)) return 0;
+    if (!(0.75 * (c * c - b * b) < h_hi)) return 0;
+    if (!(b + 0.5 * d > L1)) return 0;
+    if (!(fmax(a - 0.5 * d, 0.5 * c - b) < U1)) return 0;
+    if (!(0.5 * b + d > L2)) return 0;
+    if (!(fmax(0.5 * a - d, c - 0.5 * b) < U2)) return 0;
+    /* (2) polygon Pi = rectangle clipped by the six half-planes, in order */
+    wpo_pt bufA[WPO_MAXV], bufB[WPO_MAXV];
+    wpo_pt *cur = bufA, *nxt = bufB;
+    int n = 4;
+    cur[0].s = a; cur[0].t = c;
+    cur[1].s = b; cur[1].t = c;
+    cur[2].s = b; cur[2].t = d;
+    cur[3].s = a; cur[3].t = d;
+    for (int m = 0; m < 6; ++m) {
+        n = clip_polygon(cur, n, nxt, m, L1, U1, L2, U2);
+        if (n < 3) return 0;
+        wpo_pt* tmp = cur; cur = nxt; nxt = tmp;
+    }
+    /* (3) positive area (shoelace about vertex 0) */
+    double area2 = 0.0;
+    for (int v = 1; v + 1 < n; ++v) {
+        double s1 = cur[v].s - cur[0].s, t1 = cur[v].t - cur[0].t;
+        double s2 = cur[v + 1].s - cur[0].s, t2 = cur[v + 1].t - cur[0].t;
+        area2 = area2 + (s1 * t2 - s2 * t1);
+    }
+    if (!(area2 > 0.0)) return 0;
+    /* (4) extremes of h on Pi: vertices, plus the two tangent points */
+    double hmax = 0.75 * (cur[0].t * cur[0].t - cur[0].s * cur[0].s), hmin = hmax;
+    for (int v = 1; v < n; ++v) {
+        double h = 0.75 * (cur[v].t * cur[v].t - cur[v].s * cur[v].s);
+        hmax = fmax(hmax, h);
+        hmin = fmin(hmin, h);
+    }
+    {   /* minimum of h along q - q'/2 = U1 is at (4U1/3, 2U1/3), h = -U1^2 */
+        double s = 4.0 * U1 / 3.0, t = 2.0 * U1 / 3.0;
+        if (s >= a && s <= b && t >= c && t <= d
+            && halfplane(0, s, t, L1, U1, L2, U2) >= 0.0 && halfplane(2, s, t, L1, U1, L2, U2) >= 0.0
+            && halfplane(3, s, t, L1, U1, L2, U2) >= 0.0 && halfplane(4, s, t, L1, U1, L2, U2) >= 0.0
+            && halfplane(5, s, t, L1, U1, L2, U2) >= 0.0)
+            hmin = fmin(hmin, -(U1 * U1));
+    }
+    {   /* maximum of h along q' - q/2 = U2 is at (2U2/3, 4U2/3), h = +U2^2 */
+        double s = 2.0 * U2 / 3.0, t = 4.0 * U2 / 3.0;
+        if (s >= a && s <= b && t >= c && t <= d
+            && halfplane(0, s, t, L1, U1, L2, U2) >= 0.0 && halfplane(1, s, t, L1, U1, L2, U2) >= 0.0
+            && halfplane(2, s, t, L1, U1, L2, U2) >= 0.0 && halfplane(3, s, t, L1, U1, L2, U2) >= 0.0
+            && halfplane(5, s, t, L1, U1, L2, U2) >= 0.0)
+            hmax = fmax(hmax, U2 * U2);
+    }
+    if (!(hmax > h_lo)) return 0;
+    if (!(hmin < h_hi)) return 0;
+    if (poly) memcpy(poly, cur, (size_t)n * sizeof(wpo_pt));
+    if (nv_out) *nv_out = n;
+    return 1;
+}
+
+/* Geometric pattern.  Row r = (i-1)*n_q + (j-1), column likewise with primes;
+ * p has n_p+1 nodes, q has n_q+1.  counts[r] = number of structural nonzeros. */
+void wpo_geo_count(int n_p, int n_q, const double* p, const double* q, int32_t* counts)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int r = 0; r < n_p * n_q; ++r) {
+        int i = r / n_q, j = r % n_q;
+        int32_t cnt = 0;
+        for (int ip = 0; ip < n_p; ++ip)
+            for (int jp = 0; jp < n_q; ++jp)
+                cnt += wpo_overlap(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1], 0, 0);
+        counts[r] = cnt;
+    }
+}
+
+void wpo_geo_fill(int n_p, int n_q, const double* p, const double* q,
+                  const int64_t* geo_row_ptr, int32_t* geo_col)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int r = 0; r < n_p * n_q; ++r) {
+        int i = r / n_q, j = r % n_q;
+        int64_t pos = geo_row_ptr[r];
+        for (int ip = 0; ip < n_p; ++ip)
+            for (int jp = 0; jp < n_q; ++jp)
+                if (wpo_overlap(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1], 0, 0))
+                    geo_col[pos++] = ip * n_q + jp;
+    }
+}
+
+/* Rule R(n) for one geometric element (R7), all coupled pairs at once.
+ *   n, xi[n], w[n]      Gauss-Legendre nodes / weights on [-1,1]
+ *   n_pairs             coupled channel pairs; pair c has orbital momenta l = pair_l[c]
+ *                       (row channel), l' = pair_lp[c] (column channel) and terms
+ *                       term_ptr[c] .. term_ptr[c+1]-1, each (k, l1, l1', g)  (A3/A4)
+ *   val[c]              matrix element (A15)
+ *   absval[c]           the same sum with every term replaced by its modulus (A_e of DESIGN.md R9)
+ * Sum over (k,l1,l1') is taken PER NODE, before integrating (R8).
+ */
+#define WPO_MAXPOW 24
+static void element_values(double a, double b, double c, double d,
+                           double L1, double U1, double L2, double U2,
+                           int n, const double* xi, const double* w,
+                           int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
+                           const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
+                           const int32_t* term_l1p, const double* term_g,
+                           double* val, double* absval)
+{
+    for (int cidx = 0; cidx < n_pairs; ++cidx) { val[cidx] = 0.0; absval[cidx] = 0.0; }
+    wpo_pt poly[WPO_MAXV];
+    int nv = 0;
+    if (!wpo_overlap(a, b, c, d, L1, U1, L2, U2, poly, &nv)) return;
+    /* phi-range: angular extent of the polygon Pi (rule R1b) */
+    double phi_a = 1e300, phi_b = -1e300;
+    for (int v = 0; v < nv; ++v) {
+        if (poly[v].s == 0.0 && poly[v].t == 0.0) continue; /* the origin has no angle */
+        double ang = atan2(poly[v].t, poly[v].s);
+        phi_a = fmin(phi_a, ang);
+        phi_b = fmax(phi_b, ang);
+    }
+    if (!(phi_a < phi_b)) return;
+    double norm = 1.0 / sqrt((U2 - L2) * (b - a) * (U1 - L1) * (d - c)); /* (d_i dbar_j d_i' dbar_j')^{-1/2}, A5/A9 */
+    double half_phi = 0.5 * (phi_b - phi_a), mid_phi = 0.5 * (phi_a + phi_b);
+    for (int m = 0; m < n; ++m) {
+        double phi = mid_phi + half_phi * xi[m];
+        double wphi = half_phi * w[m];
+        double C = cos(phi), S = sin(phi);
+        /* Q-limits from the rectangle, A12 */
+        double Lq = fmax(a / C, c / S), Uq = fmin(b / C, d / S);
+        if (!(Lq < Uq)) continue;
+        double a1 = C * C + 0.25 * S * S;   /* zeta1^2 = a1 + beta x, A11 */
+        double a2 = 0.25 * C * C + S * S;   /* zeta2^2 = a2 + beta x */
+        double beta = C * S;
+        /* x-support of F > 0 (closed form; zeta^2 linear in x) */
+        double x_lo = -1.0, x_hi = 1.0;
+        if (L1 > 0.0) x_lo = fmax(x_lo, ((L1 / Uq) * (L1 / Uq) - a1) / beta);
+        if (L2 > 0.0) x_lo = fmax(x_lo, ((L2 / Uq) * (L2 / Uq) - a2) / beta);
+        if (Lq > 0.0) {
+            x_hi = fmin(x_hi, ((U1 / Lq) * (U1 / Lq) - a1) / beta);
+            x_hi = fmin(x_hi, ((U2 / Lq) * (U2 / Lq) - a2) / beta);
+        }
+        {   /* L1/zeta1 < U2/zeta2  <=>  beta x (L1^2-U2^2) < U2^2 a1 - L1^2 a2 */
+            double D = L1 * L1 - U2 * U2, R = U2 * U2 * a1 - L1 * L1 * a2;
+            if (D > 0.0) x_hi = fmin(x_hi, R / (beta * D));
+            else if (D < 0.0) x_lo = fmax(x_lo, R / (beta * D));
+            else if (!(0.0 < R)) continue;
+        }
+        {   /* L2/zeta2 < U1/zeta1  <=>  beta x (L2^2-U1^2) < U1^2 a2 - L2^2 a1 */
+            double D = L2 * L2 - U1 * U1, R = U1 * U1 * a2 - L2 * L2 * a1;
+            if (D > 0.0) x_hi = fmin(x_hi, R / (beta * D));
+            else if (D < 0.0) x_lo = fmax(x_lo, R / (beta * D));
+            else if (!(0.0 < R)) continue;
+        }
+        if (!(x_lo < x_hi)) continue;
+        double half_x = 0.5 * (x_hi - x_lo), mid_x = 0.5 * (x_lo + x_hi);
+        /* powers of cos, sin */
+        double cp[WPO_MAXPOW], sp[WPO_MAXPOW];
+        cp[0] = 1.0; sp[0] = 1.0;
+        for (int e = 1; e < WPO_MAXPOW; ++e) { cp[e] = cp[e - 1] * C; sp[e] = sp[e - 1] * S; }
+        for (int r = 0; r < n; ++r) {
+            double x = mid_x + half_x * xi[r];
+            double wx = half_x * w[r];
+            double zeta1 = sqrt(a1 + beta * x), zeta2 = sqrt(a2 + beta * x);
+            /* F of A14, clamped (R5) */
+            double Qmax = fmin(fmin(Uq, U1 / zeta1), U2 / zeta2);
+            double Qmin = fmax(fmax(Lq, L1 / zeta1), L2 / zeta2);
+            if (!(Qmax > Qmin)) continue;
+            double F = 0.5 * (Qmax * Qmax - Qmin * Qmin);
+            /* Legendre polynomials by the three-term recurrence */
+            double P[WPO_MAXPOW];
+            P[0] = 1.0; P[1] = x;
+            for (int k = 2; k < WPO_MAXPOW; ++k) P[k] = ((2 * k - 1) * x * P[k - 1] - (k - 1) * P[k - 2]) / k;
+            double z1p[WPO_MAXPOW], z2p[WPO_MAXPOW]; /* zeta^m */
+            z1p[0] = 1.0; z2p[0] = 1.0;
+            for (int e = 1; e < WPO_MAXPOW; ++e) { z1p[e] = z1p[e - 1] * zeta1; z2p[e] = z2p[e - 1] * zeta2; }
+            double wF = wphi * wx * F;
+            for (int cidx = 0; cidx < n_pairs; ++cidx) {
+                int l = pair_l[cidx], lp = pair_lp[cidx];
+                double sum = 0.0, asum = 0.0;
+                for (int64_t tt = term_ptr[cidx]; tt < term_ptr[cidx + 1]; ++tt) {
+                    int l1 = term_l1[tt], l1p = term_l1p[tt];
+                    int A = l1 + l1p;                 /* power of q  = Q cos(phi) (R1) */
+                    int B = (l - l1) + (lp - l1p);    /* power of q' = Q sin(phi) */
+                    double term = term_g[tt] * P[term_k[tt]] * cp[A + 1] * sp[B + 1];
+                    sum += term;
+                    asum += fabs(term);
+                }
+                double denom = z1p[lp + 1] * z2p[l + 1];
+                val[cidx] += wF * sum / denom;
+                absval[cidx] += wF * asum / denom;
+            }
+        }
+    }
+    for (int cidx = 0; cidx < n_pairs; ++cidx) { val[cidx] *= norm; absval[cidx] *= norm; }
+}
+
+/* Values of n_elem listed geometric elements (row cell (ei,ej), column cell (eip,ejp),
+ * all 0-based bin indices).  val/absval are [n_elem][n_pairs], row-major. */
+void wpo_elements(int n_p, int n_q, const double* p, const double* q,
+                  int64_t n_elem, const int32_t* ei, const int32_t* ej, const int32_t* eip, const int32_t* ejp,
+                  int n, const double* xi, const double* w,
+                  int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
+                  const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
+                  const int32_t* term_l1p, const double* term_g,
+                  double* val, double* absval)
+{
+    (void)n_p; (void)n_q;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t e = 0; e < n_elem; ++e) {
+        int i = ei[e], j = ej[e], ip = eip[e], jp = ejp[e];
+        element_values(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1],
+                       n, xi, w, n_pairs, pair_l, pair_lp, term_ptr, term_k, term_l1, term_l1p, term_g,
+                       val + e * n_pairs, absval + e * n_pairs);
+    }
+}
+
+/* y = P0 x, CSR, each row summed sequentially in column order. */
+void wpo_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+              const double* x, double* y)
+{
+    for (int64_t r = 0; r < rows; ++r) {
+        double acc = 0.0;
+        for (int64_t e = row_ptr[r]; e < row_ptr[r + 1]; ++e) acc += values[e] * x[col_idx[e]];
+        y[r] = acc;
+    }
+}
+
+int wpo_num_threads(void)
+{
+    int nt = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp single
+        nt = omp_get_num_threads();
+    }
+#endif
+    return nt;
+}

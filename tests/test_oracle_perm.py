@@ -1,0 +1,241 @@
+"""Pins for oracle/perm_oracle.c -- predicate, rule R(n), normalisation, SpMV.
+
+Each test names what it would catch.  None of them re-types the oracle's formulae:
+they use the Cartesian form (A7), operator identities of P = P12P23+P13P23
+and the survey's worked single-cell example.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import wpcd_inputs as wi
+from oracle import channels, perm
+from tests import cartesian_bruteforce as brute
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "single_cell.txt")
+
+
+def _dense(row_ptr, col_idx, values):
+    n = len(row_ptr) - 1
+    M = np.zeros((n, n))
+    for r in range(n):
+        M[r, col_idx[row_ptr[r]:row_ptr[r + 1]]] = values[row_ptr[r]:row_ptr[r + 1]]
+    return M
+
+
+def test_single_cell_golden_and_scale_free(swave_table):
+    gold = dict(line.split() for line in open(GOLD) if line.strip() and not line.startswith("#"))
+    for a in (0.37, 1.0, 25.0):
+        p = np.array([0.0, a])
+        for n in (8, 10, 48):
+            v, _ = perm.element_values(p, p, [0], [0], [0], [0], n, swave_table)
+            assert v[0, 0] == pytest.approx(float(gold[str(n)]), abs=2e-12)
+    v, _ = perm.element_values(np.array([0.0, 1.0]), np.array([0.0, 1.0]), [0], [0], [0], [0], 128, swave_table)
+    assert abs(v[0, 0] - float(gold["C1"])) < 3e-4
+
+
+def test_single_cell_against_cartesian_A7(swave_table):
+    # independent value of the same element from the unreduced (q,q',x) integral
+    ref = brute.element(0, 1, 0, 1, 0, 1, 0, 1, 0, 0, [(0, 0, 0, 1.0)], m=600)
+    v, _ = perm.element_values(np.array([0.0, 1.0]), np.array([0.0, 1.0]), [0], [0], [0], [0], 128, swave_table)
+    assert v[0, 0] == pytest.approx(ref, abs=2e-3)
+
+
+def test_elements_against_cartesian_A7_swave(swave_table):
+    """Catches wrong limits / normalisation / F / zeta assignment: every structural element of a
+    small jittered lattice against the Cartesian brute force (both converge slowly: F has kinks)."""
+    p = wi.tan2_grid(5, 1.0, 0.1, seed=3)
+    q = wi.tan2_grid(4, 0.7, 0.1, seed=4)   # different p and q grids: catches p<->q mix-ups
+    ptr, col = perm.geo_pattern(p, q)
+    n_q = len(q) - 1
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    v, _ = perm.element_values(p, q, rows // n_q, rows % n_q, col // n_q, col % n_q, 64, swave_table)
+    worst = 0.0
+    for e in range(len(col)):
+        i, j, ip, jp = rows[e] // n_q, rows[e] % n_q, col[e] // n_q, col[e] % n_q
+        ref = brute.element(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1], 0, 0, [(0, 0, 0, 1.0)], m=160)
+        worst = max(worst, abs(v[e, 0] - ref))
+    assert worst < 4e-3 * np.abs(v).max()
+
+
+def test_elements_against_cartesian_A7_multichannel(nd_half_plus_j1):
+    """Catches a dropped term, swapped exponents (A <-> B), wrong zeta powers (l <-> l'), P_k index."""
+    tab = nd_half_plus_j1
+    p = wi.tan2_grid(3, 1.0, 0.1, seed=5)
+    q = wi.tan2_grid(3, 0.8, 0.1, seed=6)
+    ptr, col = perm.geo_pattern(p, q)
+    n_q = len(q) - 1
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    # elements away from the first bins (there single terms are singular and brute force is poor)
+    sel = [e for e in range(len(col)) if min(rows[e] // n_q, col[e] // n_q) >= 1][:6]
+    assert len(sel) >= 4
+    v, av = perm.element_values(p, q, rows[sel] // n_q, rows[sel] % n_q, col[sel] // n_q, col[sel] % n_q, 48, tab)
+    # a few pairs with l != l', both > 0
+    pick = [c for c in range(tab.n_pairs) if tab.pair_l[c] != tab.pair_lp[c] and min(tab.pair_l[c], tab.pair_lp[c]) >= 1][:5]
+    pick += [c for c in range(tab.n_pairs) if tab.pair_l[c] == 2 and tab.pair_lp[c] == 0][:2]
+    for c in pick:
+        terms = [(tab.term_k[t], tab.term_l1[t], tab.term_l1p[t], tab.term_g[t]) for t in range(tab.term_ptr[c], tab.term_ptr[c + 1])]
+        for n_e, e in enumerate(sel):
+            i, j, ip, jp = rows[e] // n_q, rows[e] % n_q, col[e] // n_q, col[e] % n_q
+            ref = brute.element(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1],
+                                int(tab.pair_l[c]), int(tab.pair_lp[c]), terms, m=120)
+            assert abs(v[n_e, c] - ref) < 1e-2 * max(av[n_e, c], 1e-3), (c, e)
+
+
+@pytest.fixture(scope="module")
+def swave_matrices(swave_table):
+    out = {}
+    for N in (10, 20):
+        p = wi.tan2_grid(N)
+        out[N] = (p, perm.build_csr(p, p, 8, swave_table))
+    return out
+
+
+def test_symmetry(swave_matrices):
+    # P is Hermitian and the lattice basis real: M = M^T, pattern exactly
+    for N, (p, (rp, ci, v, _)) in swave_matrices.items():
+        M = _dense(rp, ci, v)
+        pat = np.zeros_like(M, bool)
+        for r in range(len(rp) - 1):
+            pat[r, ci[rp[r]:rp[r + 1]]] = True
+        assert np.array_equal(pat, pat.T)
+        assert np.abs(M - M.T).max() < 1e-12
+
+
+def test_spectrum_bound(swave_matrices):
+    # g0=1: spectrum of P = P12P23+P13P23 is {2,-1}; a Galerkin projection keeps it inside [-1,2]
+    for N, (p, (rp, ci, v, _)) in swave_matrices.items():
+        M = _dense(rp, ci, v)
+        ev = np.linalg.eigvalsh(0.5 * (M + M.T))
+        assert ev[0] > -1.0 - 0.02 and ev[-1] < 2.0 + 0.02
+
+
+def _symmetric_state(p, alpha=0.5):
+    """Lattice projection of psi = exp(-alpha (p^2 + 3/4 q^2)) (fully symmetric s-wave state):
+    v_ij = (d_i d_j)^{-1/2} int p e^{-alpha p^2} dp int q e^{-3 alpha q^2/4} dq  (A5)."""
+    ip = (np.exp(-alpha * p[:-1] ** 2) - np.exp(-alpha * p[1:] ** 2)) / (2 * alpha)
+    b = 0.75 * alpha
+    iq = (np.exp(-b * p[:-1] ** 2) - np.exp(-b * p[1:] ** 2)) / (2 * b)
+    d = np.diff(p)
+    return np.outer(ip / np.sqrt(d), iq / np.sqrt(d)).reshape(-1)
+
+
+def test_symmetric_state_eigenvalue_two(swave_matrices):
+    """P psi = 2 psi for a totally symmetric state: pins the overall normalisation of (A5)/(A9)/(A15)
+    and g0 (R4).  Residual must shrink under refinement."""
+    res, rq = [], []
+    for N in (10, 20):
+        p, (rp, ci, v, _) = swave_matrices[N]
+        vec = _symmetric_state(p)
+        y = perm.spmv(rp, ci, v, vec)
+        rq.append(vec @ y / (vec @ vec))
+        res.append(np.linalg.norm(y - 2 * vec) / np.linalg.norm(vec))
+    assert abs(rq[1] - 2.0) < 0.1 and abs(rq[1] - 2.0) < abs(rq[0] - 2.0)
+    assert res[1] < res[0] and res[1] < 0.12
+
+
+def test_weak_form_P2_equals_P_plus_2(swave_matrices):
+    # <v|(M^2 - M - 2)|v>/<v|v> -> 0 on a smooth symmetric vector (trend only, DESIGN.md pins table)
+    vals = []
+    for N in (10, 20):
+        p, (rp, ci, v, _) = swave_matrices[N]
+        vec = _symmetric_state(p)
+        y = perm.spmv(rp, ci, v, vec)
+        yy = perm.spmv(rp, ci, v, y)
+        vals.append(abs(vec @ (yy - y - 2 * vec)) / (vec @ vec))
+    assert vals[1] < vals[0] and vals[1] < 0.3
+
+
+def test_multichannel_matrix_symmetric(nd_half_plus_j1):
+    tab = nd_half_plus_j1
+    p = wi.tan2_grid(4)
+    rp, ci, v, av = perm.build_csr(p, p, 16, tab)
+    M = _dense(rp, ci, v)
+    A = _dense(rp, ci, av)
+    assert np.all(np.abs(M - M.T) <= 1e-10 * np.maximum(A, A.T) + 1e-14)
+
+
+def test_pattern_against_point_sampling():
+    """Predicate S vs the theta-product of (A7) sampled on a dense interior grid: no hit may fall
+    outside S, and every pair of S must be hit once sampling is fine enough."""
+    p = wi.tan2_grid(7, 1.0, 0.1, seed=11)
+    q = wi.tan2_grid(6, 1.3, 0.1, seed=12)
+    ptr, col = perm.geo_pattern(p, q)
+    n_p, n_q = len(p) - 1, len(q) - 1
+    S = np.zeros((n_p * n_q, n_p * n_q), bool)
+    for r in range(n_p * n_q):
+        S[r, col[ptr[r]:ptr[r + 1]]] = True
+    missed = 0
+    for r in range(n_p * n_q):
+        i, j = divmod(r, n_q)
+        for c in range(n_p * n_q):
+            ip, jp = divmod(c, n_q)
+            args = (q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1])
+            hit = brute.hits(*args, m=24)
+            if hit:
+                assert S[r, c], (r, c)
+            elif S[r, c]:
+                if not brute.hits(*args, m=400):
+                    missed += 1
+    assert missed == 0
+
+
+def test_pattern_ties_on_identical_grids():
+    # un-jittered p == q grids: touching cells (exact FP ties) are not structural nonzeros,
+    # the pattern stays symmetric, and every row has at least one entry
+    p = wi.tan2_grid(12)
+    ptr, col = perm.geo_pattern(p, p)
+    n = 12
+    S = np.zeros((n * n, n * n), bool)
+    for r in range(n * n):
+        S[r, col[ptr[r]:ptr[r + 1]]] = True
+        assert np.all(np.diff(col[ptr[r]:ptr[r + 1]]) > 0)
+    assert np.array_equal(S, S.T)
+    assert np.all(np.diff(ptr) > 0)
+    # corner-touching pair (i'=i-1, j'=j-1 has E_hi' == E_lo exactly): never in S
+    for i in range(1, n):
+        for j in range(1, n):
+            assert not S[i * n + j, (i - 1) * n + (j - 1)]
+
+
+def test_values_zero_outside_pattern_and_superset(swave_table):
+    # numerically nonzero elements (any n) all lie inside S: evaluate the rule on ALL cell pairs
+    p = wi.tan2_grid(6, 1.0, 0.1, seed=2)
+    n = 6
+    ptr, col = perm.geo_pattern(p, p)
+    S = set()
+    for r in range(n * n):
+        S.update((r, c) for c in col[ptr[r]:ptr[r + 1]])
+    allr, allc = np.divmod(np.arange(n ** 4), n * n)
+    # the rule returns 0 for a non-overlapping pair by construction; the independent check is the
+    # brute-force Cartesian value
+    for r, c in zip(allr[::7], allc[::7]):
+        if (r, c) in S:
+            continue
+        i, j, ip, jp = r // n, r % n, c // n, c % n
+        ref = brute.element(p[j], p[j + 1], p[jp], p[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1], 0, 0, [(0, 0, 0, 1.0)], m=40)
+        assert ref == 0.0
+
+
+def test_spmv_against_dense(swave_matrices):
+    p, (rp, ci, v, _) = swave_matrices[20]
+    x = wi.normal_vector(len(rp) - 1)
+    assert np.allclose(perm.spmv(rp, ci, v, x), _dense(rp, ci, v) @ x, rtol=0, atol=1e-12)
+
+
+def test_full_row_ptr_and_columns(nd_half_plus_j1):
+    tab = nd_half_plus_j1
+    p = wi.tan2_grid(3)
+    geo = perm.geo_pattern(p, p)
+    rp, ci, v, _ = perm.build_csr(p, p, 4, tab, geo=geo)
+    n_geo = 9
+    for g in range(tab.n_ch):
+        coupled = np.nonzero(tab.mask[g])[0]
+        for r in range(n_geo):
+            cols = ci[rp[g * n_geo + r]:rp[g * n_geo + r + 1]]
+            gc = geo[1][geo[0][r]:geo[0][r + 1]]
+            expect = np.concatenate([gp * n_geo + gc for gp in coupled]) if len(coupled) else np.zeros(0)
+            assert np.array_equal(cols, expect)
+            assert np.all(np.diff(cols) > 0)
+    assert not np.isnan(v).any()

@@ -1,0 +1,161 @@
+/* wpcd.h -- C-ABI of libwpcd: the permutation-operator matrix P0 of the
+ * wave-packet continuum discretisation (arxiv 1404.5253) on one NVIDIA B200.
+ *
+ * What the library computes (citations are PAPER.md lines):
+ *   P0 = matrix of P = P12 P23 + P13 P23 (eq. 2, l.62) in the lattice basis
+ *   |X_ij^{gamma}> of eq. (6) (l.110): element (gamma,i,j ; gamma',i',j') is the
+ *   integral (A15) (l.457) of the geometric coupling function G of (A3) (l.390)
+ *   over the region where the cell D_ij of one Jacobi set overlaps the cell
+ *   D_i'j' of the other (A7, l.416).  "Selection of the nonzero elements"
+ *   (step 2, l.311) -> wpcd_perm_count; "calculation of the nonzero elements"
+ *   (step 3, l.312) -> wpcd_perm_build; the product with a vector inside the
+ *   iterative solution (step 5, l.314; sparse storage l.304) -> wpcd_perm_apply.
+ *   Readings of every silent/garbled point: DESIGN.md section "Readings" (R1..R13).
+ *
+ * Conventions
+ *   - plain C, no exceptions cross the boundary; every call returns a
+ *     wpcd_status (0 = WPCD_OK, < 0 error) and wpcd_last_error() returns a
+ *     thread-local message for the last failing call of the calling thread.
+ *   - "host" pointers are ordinary CPU memory; "dev" pointers are CUDA device
+ *     memory on the CURRENT device, owned by the caller (e.g. torch tensors).
+ *     The library owns only the small tables inside its handles.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = default stream).
+ *     All work is enqueued on it; only wpcd_perm_count synchronises (it must
+ *     return nnz to the host).
+ *   - index convention: cell (i,j), i = 0..n_p-1 the p-bin [p_i,p_{i+1}], j = 0..n_q-1
+ *     the q-bin; geometric row r = i*n_q + j; full row = gamma*n_p*n_q + r; columns
+ *     alike with primed indices; columns strictly ascending inside a row.
+ *   - there is no CPU fallback: without a CUDA device every compute call
+ *     returns WPCD_ERR_CUDA.
+ *   - a handle must not be used by two host threads at the same time.
+ */
+#ifndef WPCD_H
+#define WPCD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wpcd_grid wpcd_grid;
+typedef struct wpcd_channels wpcd_channels;
+typedef int wpcd_status;
+
+#define WPCD_OK 0
+#define WPCD_ERR_INVALID_ARG (-1)   /* null pointer, non-positive size, bad enum */
+#define WPCD_ERR_NOT_MONOTONE (-2)  /* nodes not strictly increasing or first node < 0 */
+#define WPCD_ERR_ALLOC (-3)
+#define WPCD_ERR_CUDA (-4)          /* CUDA runtime error or no device */
+#define WPCD_ERR_OVERFLOW (-5)      /* column index would not fit int32 / nnz int64 */
+#define WPCD_ERR_UNSUPPORTED (-6)   /* n_quad, l or k beyond WPCD_MAX_* */
+
+#define WPCD_MAX_QUAD 64            /* Gauss-Legendre points per dimension (paper: 48, l.334) */
+#define WPCD_MAX_L 7                /* largest pair orbital momentum l */
+#define WPCD_MAX_K 23               /* largest Legendre order k in (A3) */
+
+#define WPCD_SPINLESS_SWAVE 0       /* one channel l = lambda = 0, G = g0 (R4) */
+#define WPCD_ND 1                   /* nucleon-deuteron channels of eq. (5), g from (A4) */
+
+/* Message for the last error raised on this thread ("" if none). Static storage. */
+const char* wpcd_last_error(void);
+
+/* Momentum lattice: p_nodes[0..n_p] and q_nodes[0..n_q], HOST,
+ * strictly increasing, first node >= 0, in fm^-1 (any unit: P0 is scale free).
+ * Copies the nodes to the device.  *out is owned by the library. */
+wpcd_status wpcd_grid_create(const double* p_nodes, int n_p, const double* q_nodes, int n_q, wpcd_grid** out);
+void wpcd_grid_destroy(wpcd_grid* grid);
+
+/* Channel set for fixed Gamma = {J, pi, T} (eq. 5, l.98-102) and its coefficient
+ * table g^{l1 l1' k}_{gamma gamma'} of (A4) (l.395), computed on the host (step 1, l.310).
+ *   model = WPCD_SPINLESS_SWAVE: two_J, parity, two_T, j_pair_max ignored; g = g0.
+ *   model = WPCD_ND: parity = +1/-1, two_T = 1, pair momentum j <= j_pair_max; g0 ignored.
+ * Channel order: ascending j, then s, then l, then two_I, then lambda
+ * (channel = (l, s, j, t, lambda, two_I); t fixed by l+s+t odd, l.102).
+ * Channel pairs whose every coefficient vanishes are not coupled and get no entries. */
+wpcd_status wpcd_channels_create(int model, int two_J, int parity, int two_T, int j_pair_max, double g0,
+                                 wpcd_channels** out);
+
+/* Same, from a caller-supplied table (all HOST arrays): channel_l[n_channels] = l of each
+ * channel; pair c = (pair_gamma[c], pair_gammap[c]) sorted ascending by (gamma, gamma'),
+ * each pair once; its terms term_ptr[c] .. term_ptr[c+1]-1 are (k, l1, l1', g) multiplying
+ * q^{l1+l1'} q'^{(l-l1)+(l'-l1')} P_k(x) in (A3) (reading R1). */
+wpcd_status wpcd_channels_create_from_table(int n_channels, const int32_t* channel_l, int n_pairs,
+                                            const int32_t* pair_gamma, const int32_t* pair_gammap,
+                                            const int64_t* term_ptr, const int32_t* term_k,
+                                            const int32_t* term_l1, const int32_t* term_l1p,
+                                            const double* term_g, wpcd_channels** out);
+void wpcd_channels_destroy(wpcd_channels* channels);
+
+/* Introspection (host side, no device work). */
+int wpcd_channels_count(const wpcd_channels* channels);            /* number of channels */
+int wpcd_channels_pairs(const wpcd_channels* channels);            /* number of coupled pairs */
+int64_t wpcd_channels_terms(const wpcd_channels* channels);        /* total (k,l1,l1') terms */
+/* quantum numbers [n_channels][6] = (l, s, j, t, lambda, two_I); zeros for a table-made set
+ * except l.  HOST output. */
+wpcd_status wpcd_channels_get_quantum_numbers(const wpcd_channels* channels, int32_t* out);
+/* The table in the layout of wpcd_channels_create_from_table; HOST outputs sized by the
+ * three counts above (term_ptr: n_pairs+1). */
+wpcd_status wpcd_channels_get_table(const wpcd_channels* channels, int32_t* pair_gamma, int32_t* pair_gammap,
+                                    int64_t* term_ptr, int32_t* term_k, int32_t* term_l1, int32_t* term_l1p,
+                                    double* term_g);
+
+/* rows = columns = n_channels * n_p * n_q;  geometric rows = n_p * n_q. */
+int64_t wpcd_rows(const wpcd_grid* grid, const wpcd_channels* channels);
+int64_t wpcd_geo_rows(const wpcd_grid* grid);
+
+/* Step 2 (l.311): structural nonzeros.  A cell pair is a structural nonzero iff the
+ * cells overlap with positive measure under (A2) -- predicate S of DESIGN.md R6, evaluated
+ * in IEEE double without contraction; it does not depend on the channel pair or n_quad.
+ *   geo_row_ptr_dev [n_p*n_q + 1] int32 dev, out: CSR row pointer of the geometric pattern
+ *   row_ptr_dev     [rows + 1]    int64 dev, out: CSR row pointer of P0
+ *   nnz_out, nnz_geo_out          host, out
+ * Synchronises the stream once. */
+wpcd_status wpcd_perm_count(const wpcd_grid* grid, const wpcd_channels* channels, int n_quad, void* cuda_stream,
+                            int64_t* row_ptr_dev, int32_t* geo_row_ptr_dev, int64_t* nnz_out, int64_t* nnz_geo_out);
+
+/* Scratch needed by wpcd_perm_build for a pattern with nnz_geo geometric entries
+ * (geometric column / row / phi-range lists, and for coupled channels a block of monomial
+ * moments).  0 on invalid arguments. */
+size_t wpcd_perm_workspace_bytes(const wpcd_channels* channels, int64_t nnz_geo);
+
+/* Steps 2b+3 (l.312): column indices and values.
+ *   row_ptr_dev, geo_row_ptr_dev   as written by wpcd_perm_count for the same arguments
+ *   workspace_dev                  >= wpcd_perm_workspace_bytes(channels, nnz_geo) bytes, dev, 256-byte aligned
+ *   col_idx_dev [nnz] int32, values_dev [nnz] double: dev, out
+ * Value = (d_i dbar_j d_i' dbar_j')^{-1/2} * double integral (A15) of F (A14) times the
+ * channel-pair sum (A3), by the rule R(n_quad) of DESIGN.md R7: n_quad-point Gauss-Legendre
+ * in phi over the angular extent of the overlap polygon, and at every phi-node n_quad-point
+ * Gauss-Legendre in x over the closed-form support of F.  1 <= n_quad <= WPCD_MAX_QUAD.
+ * Asynchronous on the stream. */
+wpcd_status wpcd_perm_build(const wpcd_grid* grid, const wpcd_channels* channels, int n_quad, void* cuda_stream,
+                            const int64_t* row_ptr_dev, const int32_t* geo_row_ptr_dev,
+                            void* workspace_dev, size_t workspace_bytes,
+                            int32_t* col_idx_dev, double* values_dev);
+
+/* y = P0 x for n_vec vectors (step 5, l.314; l.304).  x_dev[v*rows + c], y_dev[v*rows + r],
+ * v = 0..n_vec-1 (vector-major), dev.  CSR arrays as produced above.  Asynchronous. */
+wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                            const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
+                            void* cuda_stream);
+
+/* Same product with HOST vectors: copies x_host -> x_dev (scratch, dev, n_vec*rows doubles),
+ * applies, copies y_dev (scratch) -> y_host, all on the stream, then synchronises it.
+ * Pinned host memory makes the copies asynchronous. */
+wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                                 const double* values_dev, const double* x_host, double* y_host, int n_vec,
+                                 double* x_dev, double* y_dev, void* cuda_stream);
+
+/* FP64 FMA microbenchmark (the roofline denominator of the fill kernel):
+ * runs a dependent-chain-free DFMA loop on the whole chip and returns achieved FLOP/s
+ * (2 per DFMA) in *flops_out (host).  Synchronises. */
+wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out);
+
+/* Number of kernels the library has launched from this process (bench.py's gpu_launches). */
+int64_t wpcd_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WPCD_H */

@@ -205,39 +205,42 @@ static void element_values(double a, double b, double c, double d,
         /* Q-limits from the rectangle, A12 */
         double Lq = fmax(a / C, c / S), Uq = fmin(b / C, d / S);
         if (!(Lq < Uq)) continue;
-        double a1 = C * C + 0.25 * S * S;   /* zeta1^2 = a1 + beta x, A11 */
-        double a2 = 0.25 * C * C + S * S;   /* zeta2^2 = a2 + beta x */
+        /* zeta of A11 in the variable u = 1 + x (R7: same rule, conditioned near the
+         * pi1 = 0 / pi2 = 0 corners x = -1):  zeta1^2 = b1 + beta u,  zeta2^2 = b2 + beta u */
+        double b1 = (C - 0.5 * S) * (C - 0.5 * S);
+        double b2 = (0.5 * C - S) * (0.5 * C - S);
         double beta = C * S;
-        /* x-support of F > 0 (closed form; zeta^2 linear in x) */
-        double x_lo = -1.0, x_hi = 1.0;
-        if (L1 > 0.0) x_lo = fmax(x_lo, ((L1 / Uq) * (L1 / Uq) - a1) / beta);
-        if (L2 > 0.0) x_lo = fmax(x_lo, ((L2 / Uq) * (L2 / Uq) - a2) / beta);
+        /* u-support of F > 0 (closed form; zeta^2 linear in u) */
+        double u_lo = 0.0, u_hi = 2.0;
+        if (L1 > 0.0) u_lo = fmax(u_lo, ((L1 / Uq) * (L1 / Uq) - b1) / beta);
+        if (L2 > 0.0) u_lo = fmax(u_lo, ((L2 / Uq) * (L2 / Uq) - b2) / beta);
         if (Lq > 0.0) {
-            x_hi = fmin(x_hi, ((U1 / Lq) * (U1 / Lq) - a1) / beta);
-            x_hi = fmin(x_hi, ((U2 / Lq) * (U2 / Lq) - a2) / beta);
+            u_hi = fmin(u_hi, ((U1 / Lq) * (U1 / Lq) - b1) / beta);
+            u_hi = fmin(u_hi, ((U2 / Lq) * (U2 / Lq) - b2) / beta);
         }
-        {   /* L1/zeta1 < U2/zeta2  <=>  beta x (L1^2-U2^2) < U2^2 a1 - L1^2 a2 */
-            double D = L1 * L1 - U2 * U2, R = U2 * U2 * a1 - L1 * L1 * a2;
-            if (D > 0.0) x_hi = fmin(x_hi, R / (beta * D));
-            else if (D < 0.0) x_lo = fmax(x_lo, R / (beta * D));
+        {   /* L1/zeta1 < U2/zeta2  <=>  beta u (L1^2-U2^2) < U2^2 b1 - L1^2 b2 */
+            double D = L1 * L1 - U2 * U2, R = U2 * U2 * b1 - L1 * L1 * b2;
+            if (D > 0.0) u_hi = fmin(u_hi, R / (beta * D));
+            else if (D < 0.0) u_lo = fmax(u_lo, R / (beta * D));
             else if (!(0.0 < R)) continue;
         }
-        {   /* L2/zeta2 < U1/zeta1  <=>  beta x (L2^2-U1^2) < U1^2 a2 - L2^2 a1 */
-            double D = L2 * L2 - U1 * U1, R = U1 * U1 * a2 - L2 * L2 * a1;
-            if (D > 0.0) x_hi = fmin(x_hi, R / (beta * D));
-            else if (D < 0.0) x_lo = fmax(x_lo, R / (beta * D));
+        {   /* L2/zeta2 < U1/zeta1  <=>  beta u (L2^2-U1^2) < U1^2 b2 - L2^2 b1 */
+            double D = L2 * L2 - U1 * U1, R = U1 * U1 * b2 - L2 * L2 * b1;
+            if (D > 0.0) u_hi = fmin(u_hi, R / (beta * D));
+            else if (D < 0.0) u_lo = fmax(u_lo, R / (beta * D));
             else if (!(0.0 < R)) continue;
         }
-        if (!(x_lo < x_hi)) continue;
-        double half_x = 0.5 * (x_hi - x_lo), mid_x = 0.5 * (x_lo + x_hi);
+        if (!(u_lo < u_hi)) continue;
+        double half_u = 0.5 * (u_hi - u_lo), mid_u = 0.5 * (u_lo + u_hi);
         /* powers of cos, sin */
         double cp[WPO_MAXPOW], sp[WPO_MAXPOW];
         cp[0] = 1.0; sp[0] = 1.0;
         for (int e = 1; e < WPO_MAXPOW; ++e) { cp[e] = cp[e - 1] * C; sp[e] = sp[e - 1] * S; }
         for (int r = 0; r < n; ++r) {
-            double x = mid_x + half_x * xi[r];
-            double wx = half_x * w[r];
-            double zeta1 = sqrt(a1 + beta * x), zeta2 = sqrt(a2 + beta * x);
+            double u = mid_u + half_u * xi[r];
+            double x = u - 1.0;
+            double wx = half_u * w[r];
+            double zeta1 = sqrt(b1 + beta * u), zeta2 = sqrt(b2 + beta * u);
             /* F of A14, clamped (R5) */
             double Qmax = fmin(fmin(Uq, U1 / zeta1), U2 / zeta2);
             double Qmin = fmax(fmax(Lq, L1 / zeta1), L2 / zeta2);

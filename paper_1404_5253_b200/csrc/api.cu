@@ -1,0 +1,432 @@
+// api.cu -- the C-ABI of libwpcd (include/wpcd.h): handles, host preparation (paper step 1,
+// PAPER.md:310), argument checks and kernel launches.  No torch types, no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <new>
+#include <tuple>
+
+#include "wigner_host.h"
+#include "wpcd_internal.h"
+
+namespace wpcd_detail {
+
+static thread_local std::string t_error;
+int64_t g_launches = 0;
+
+void set_error(const std::string& msg) { t_error = msg; }
+
+static wpcd_status fail(wpcd_status code, const std::string& msg)
+{
+    set_error(msg);
+    return code;
+}
+
+static wpcd_status cuda_fail(cudaError_t err, const char* where)
+{
+    return fail(WPCD_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(err));
+}
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base)
+{
+    Workspace ws{};
+    size_t off = 0;
+    char* b = static_cast<char*>(base);
+    auto take = [&](size_t bytes) { char* ptr = b ? b + off : nullptr; off += align256(bytes); return ptr; };
+    ws.geo_col = reinterpret_cast<int32_t*>(take(sizeof(int32_t) * (size_t)nnz_geo));
+    ws.geo_row = reinterpret_cast<int32_t*>(take(sizeof(int32_t) * (size_t)nnz_geo));
+    ws.geo_phi = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)nnz_geo));
+    ws.chunk = 0;
+    ws.moments = nullptr;
+    if (ch && !ch->swave_single) {
+        // moment block: at most ~512 MiB, a multiple of 32 elements
+        int64_t chunk = (int64_t)((512ull << 20) / (sizeof(double) * (size_t)std::max(ch->n_mu, 1)));
+        chunk = std::max<int64_t>(32, (chunk / 32) * 32);
+        chunk = std::min<int64_t>(chunk, ((nnz_geo + 31) / 32) * 32);
+        chunk = std::max<int64_t>(chunk, 32);
+        ws.chunk = chunk;
+        ws.moments = reinterpret_cast<double*>(take(sizeof(double) * (size_t)chunk * (size_t)ch->n_mu));
+    }
+    ws.bytes = off;
+    return ws;
+}
+
+static std::mutex g_hint_mutex;
+static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_ptr_dev -> (rows, nnz)
+
+static void free_channels_device(wpcd_channels* c)
+{
+    cudaFree(c->ncoupled_dev); cudaFree(c->chan_off_dev); cudaFree(c->pair_gamma_dev); cudaFree(c->pair_gammap_dev);
+    cudaFree(c->pair_ci_dev); cudaFree(c->mu_dev); cudaFree(c->mterm_ptr_dev); cudaFree(c->mterm_mu_dev); cudaFree(c->mterm_g_dev);
+}
+
+template <class T>
+static cudaError_t upload(T** dst, const std::vector<T>& src)
+{
+    size_t bytes = sizeof(T) * std::max<size_t>(src.size(), 1);
+    cudaError_t err = cudaMalloc(reinterpret_cast<void**>(dst), bytes);
+    if (err != cudaSuccess) return err;
+    if (!src.empty()) err = cudaMemcpy(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice);
+    return err;
+}
+
+// Finish a channel handle whose host table (channel_l, pairs, terms) is filled in.
+static wpcd_status finalize_channels(wpcd_channels* c)
+{
+    c->n_terms = (int64_t)c->term_g.size();
+    // checks
+    for (int a = 0; a < c->n_ch; ++a)
+        if (c->channel_l[a] < 0 || c->channel_l[a] > WPCD_MAX_L) return fail(WPCD_ERR_UNSUPPORTED, "channel l beyond WPCD_MAX_L");
+    for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
+        int ga = c->pair_gamma[pidx], gb = c->pair_gammap[pidx];
+        if (ga < 0 || ga >= c->n_ch || gb < 0 || gb >= c->n_ch) return fail(WPCD_ERR_INVALID_ARG, "pair channel index out of range");
+        if (pidx > 0 && std::make_pair(c->pair_gamma[pidx - 1], c->pair_gammap[pidx - 1]) >= std::make_pair(ga, gb))
+            return fail(WPCD_ERR_INVALID_ARG, "pairs must be sorted ascending by (gamma, gamma') without repeats");
+        if (c->term_ptr[pidx + 1] < c->term_ptr[pidx]) return fail(WPCD_ERR_INVALID_ARG, "term_ptr not monotone");
+    }
+    // merged monomials mu = (k, A, l, l'), A = l1 + l1'
+    std::map<std::tuple<int, int, int, int>, int> mu_index;   // key (l, l', A, k)
+    c->k_max = 0; c->l_max = 0;
+    for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
+        int l = c->channel_l[c->pair_gamma[pidx]], lp = c->channel_l[c->pair_gammap[pidx]];
+        c->l_max = std::max(c->l_max, std::max(l, lp));
+        std::map<std::tuple<int, int, int, int>, double> acc;
+        for (int64_t t = c->term_ptr[pidx]; t < c->term_ptr[pidx + 1]; ++t) {
+            int k = c->term_k[t], l1 = c->term_l1[t], l1p = c->term_l1p[t];
+            if (k < 0 || k > WPCD_MAX_K) return fail(WPCD_ERR_UNSUPPORTED, "Legendre order k beyond WPCD_MAX_K");
+            if (l1 < 0 || l1 > l || l1p < 0 || l1p > lp) return fail(WPCD_ERR_INVALID_ARG, "l1 / l1' out of range");
+            c->k_max = std::max(c->k_max, k);
+            acc[std::make_tuple(l, lp, l1 + l1p, k)] += c->term_g[t];
+        }
+        for (auto& kv : acc) mu_index.emplace(kv.first, 0);   // indices assigned once the set is complete
+    }
+    int idx = 0;
+    c->mu.clear();
+    for (auto& kv : mu_index) {
+        kv.second = idx++;
+        c->mu.push_back({(int16_t)std::get<3>(kv.first), (int16_t)std::get<2>(kv.first), (int16_t)std::get<0>(kv.first),
+                         (int16_t)std::get<1>(kv.first)});
+    }
+    c->n_mu = idx;
+    c->mterm_ptr.assign(c->n_pairs + 1, 0);
+    c->mterm_mu.clear(); c->mterm_g.clear();
+    for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
+        int l = c->channel_l[c->pair_gamma[pidx]], lp = c->channel_l[c->pair_gammap[pidx]];
+        std::map<std::tuple<int, int, int, int>, double> acc;
+        for (int64_t t = c->term_ptr[pidx]; t < c->term_ptr[pidx + 1]; ++t)
+            acc[std::make_tuple(l, lp, c->term_l1[t] + c->term_l1p[t], c->term_k[t])] += c->term_g[t];
+        for (auto& kv : acc) { c->mterm_mu.push_back(mu_index[kv.first]); c->mterm_g.push_back(kv.second); }
+        c->mterm_ptr[pidx + 1] = (int32_t)c->mterm_mu.size();
+    }
+    c->swave_single = (c->n_ch == 1 && c->n_pairs == 1 && c->n_terms == 1 && c->channel_l[0] == 0 && c->term_k[0] == 0);
+    if (c->swave_single) c->g0 = c->term_g[0];
+    // coupling structure
+    c->ncoupled.assign(c->n_ch, 0);
+    std::vector<int32_t> pair_ci(c->n_pairs);
+    for (int pidx = 0; pidx < c->n_pairs; ++pidx) pair_ci[pidx] = c->ncoupled[c->pair_gamma[pidx]]++;
+    std::vector<int64_t> chan_off(c->n_ch + 1, 0);
+    for (int a = 0; a < c->n_ch; ++a) chan_off[a + 1] = chan_off[a] + c->ncoupled[a];
+    c->total_coupled = chan_off[c->n_ch];
+    // device tables (skipped when the process has no CUDA device: the host-side table stays
+    // inspectable, every compute call then fails with WPCD_ERR_CUDA)
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return WPCD_OK; }
+    cudaError_t err;
+    if ((err = upload(&c->ncoupled_dev, c->ncoupled)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->chan_off_dev, chan_off)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->pair_gamma_dev, c->pair_gamma)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->pair_gammap_dev, c->pair_gammap)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->pair_ci_dev, pair_ci)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->mu_dev, c->mu)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->mterm_ptr_dev, c->mterm_ptr)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->mterm_mu_dev, c->mterm_mu)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->mterm_g_dev, c->mterm_g)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    return WPCD_OK;
+}
+
+}  // namespace wpcd_detail
+
+using namespace wpcd_detail;
+
+extern "C" {
+
+const char* wpcd_last_error(void) { return t_error.c_str(); }
+
+wpcd_status wpcd_grid_create(const double* p_nodes, int n_p, const double* q_nodes, int n_q, wpcd_grid** out)
+{
+    if (!p_nodes || !q_nodes || !out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_grid_create: null pointer");
+    *out = nullptr;
+    if (n_p < 1 || n_q < 1) return fail(WPCD_ERR_INVALID_ARG, "wpcd_grid_create: n_p, n_q must be >= 1");
+    if ((int64_t)n_p * n_q > (int64_t)INT32_MAX / 2) return fail(WPCD_ERR_OVERFLOW, "wpcd_grid_create: n_p*n_q too large");
+    for (int i = 0; i <= n_p; ++i)
+        if (!std::isfinite(p_nodes[i]) || (i == 0 ? p_nodes[0] < 0.0 : !(p_nodes[i] > p_nodes[i - 1])))
+            return fail(WPCD_ERR_NOT_MONOTONE, "wpcd_grid_create: p nodes must be finite, >= 0 and strictly increasing");
+    for (int i = 0; i <= n_q; ++i)
+        if (!std::isfinite(q_nodes[i]) || (i == 0 ? q_nodes[0] < 0.0 : !(q_nodes[i] > q_nodes[i - 1])))
+            return fail(WPCD_ERR_NOT_MONOTONE, "wpcd_grid_create: q nodes must be finite, >= 0 and strictly increasing");
+    wpcd_grid* g = new (std::nothrow) wpcd_grid();
+    if (!g) return fail(WPCD_ERR_ALLOC, "wpcd_grid_create: out of host memory");
+    g->n_p = n_p; g->n_q = n_q;
+    g->p.assign(p_nodes, p_nodes + n_p + 1);
+    g->q.assign(q_nodes, q_nodes + n_q + 1);
+    cudaError_t err = cudaMalloc(reinterpret_cast<void**>(&g->p_dev), sizeof(double) * (n_p + 1));
+    if (err == cudaSuccess) err = cudaMalloc(reinterpret_cast<void**>(&g->q_dev), sizeof(double) * (n_q + 1));
+    if (err == cudaSuccess) err = cudaMemcpy(g->p_dev, p_nodes, sizeof(double) * (n_p + 1), cudaMemcpyHostToDevice);
+    if (err == cudaSuccess) err = cudaMemcpy(g->q_dev, q_nodes, sizeof(double) * (n_q + 1), cudaMemcpyHostToDevice);
+    if (err == cudaSuccess) err = cudaMallocHost(reinterpret_cast<void**>(&g->nnz_geo_pinned), sizeof(int32_t));
+    if (err != cudaSuccess) { wpcd_grid_destroy(g); return cuda_fail(err, "wpcd_grid_create"); }
+    *out = g;
+    return WPCD_OK;
+}
+
+void wpcd_grid_destroy(wpcd_grid* g)
+{
+    if (!g) return;
+    cudaFree(g->p_dev); cudaFree(g->q_dev);
+    if (g->nnz_geo_pinned) cudaFreeHost(g->nnz_geo_pinned);
+    delete g;
+}
+
+wpcd_status wpcd_channels_create(int model, int two_J, int parity, int two_T, int j_pair_max, double g0, wpcd_channels** out)
+{
+    if (!out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create: null pointer");
+    *out = nullptr;
+    wpcd_channels* c = new (std::nothrow) wpcd_channels();
+    if (!c) return fail(WPCD_ERR_ALLOC, "wpcd_channels_create: out of host memory");
+    c->model = model;
+    if (model == WPCD_SPINLESS_SWAVE) {
+        if (!std::isfinite(g0)) { delete c; return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create: g0 not finite"); }
+        c->n_ch = 1; c->n_pairs = 1;
+        c->qn.assign(6, 0); c->channel_l = {0};
+        c->pair_gamma = {0}; c->pair_gammap = {0}; c->term_ptr = {0, 1};
+        c->term_k = {0}; c->term_l1 = {0}; c->term_l1p = {0}; c->term_g = {g0};
+    } else if (model == WPCD_ND) {
+        if (two_J < 1 || (two_J & 1) == 0 || (parity != 1 && parity != -1) || two_T != 1 || j_pair_max < 0 || j_pair_max > 6) {
+            delete c;
+            return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create: need odd two_J >= 1, parity = +-1, two_T = 1, 0 <= j_pair_max <= 6");
+        }
+        std::vector<wpcd_host::Channel> chs = wpcd_host::enumerate_channels(two_J, parity, j_pair_max);
+        std::vector<wpcd_host::Pair> pairs = wpcd_host::g_table(chs, two_J, two_T);
+        c->n_ch = (int)chs.size(); c->n_pairs = (int)pairs.size();
+        for (auto& ch : chs) {
+            c->channel_l.push_back(ch.l);
+            int32_t v[6] = {ch.l, ch.s, ch.j, ch.t, ch.lam, ch.two_I};
+            c->qn.insert(c->qn.end(), v, v + 6);
+        }
+        c->term_ptr.push_back(0);
+        for (auto& pr : pairs) {
+            c->pair_gamma.push_back(pr.gamma); c->pair_gammap.push_back(pr.gammap);
+            for (auto& t : pr.terms) { c->term_k.push_back(t.k); c->term_l1.push_back(t.l1); c->term_l1p.push_back(t.l1p); c->term_g.push_back(t.g); }
+            c->term_ptr.push_back((int64_t)c->term_g.size());
+        }
+    } else {
+        delete c;
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create: unknown model");
+    }
+    wpcd_status st = finalize_channels(c);
+    if (st != WPCD_OK) { wpcd_channels_destroy(c); return st; }
+    *out = c;
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_channels_create_from_table(int n_channels, const int32_t* channel_l, int n_pairs, const int32_t* pair_gamma,
+                                            const int32_t* pair_gammap, const int64_t* term_ptr, const int32_t* term_k,
+                                            const int32_t* term_l1, const int32_t* term_l1p, const double* term_g,
+                                            wpcd_channels** out)
+{
+    if (!out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create_from_table: null pointer");
+    *out = nullptr;
+    if (n_channels < 1 || n_pairs < 0 || !channel_l || !term_ptr || (n_pairs > 0 && (!pair_gamma || !pair_gammap)))
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create_from_table: bad sizes or null pointer");
+    int64_t n_terms = term_ptr[n_pairs];
+    if (term_ptr[0] != 0 || n_terms < 0 || (n_terms > 0 && (!term_k || !term_l1 || !term_l1p || !term_g)))
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_create_from_table: bad term arrays");
+    wpcd_channels* c = new (std::nothrow) wpcd_channels();
+    if (!c) return fail(WPCD_ERR_ALLOC, "out of host memory");
+    c->model = -1;
+    c->n_ch = n_channels; c->n_pairs = n_pairs;
+    c->channel_l.assign(channel_l, channel_l + n_channels);
+    c->qn.assign((size_t)n_channels * 6, 0);
+    for (int a = 0; a < n_channels; ++a) c->qn[(size_t)a * 6] = channel_l[a];
+    c->pair_gamma.assign(pair_gamma, pair_gamma + n_pairs);
+    c->pair_gammap.assign(pair_gammap, pair_gammap + n_pairs);
+    c->term_ptr.assign(term_ptr, term_ptr + n_pairs + 1);
+    c->term_k.assign(term_k, term_k + n_terms);
+    c->term_l1.assign(term_l1, term_l1 + n_terms);
+    c->term_l1p.assign(term_l1p, term_l1p + n_terms);
+    c->term_g.assign(term_g, term_g + n_terms);
+    wpcd_status st = finalize_channels(c);
+    if (st != WPCD_OK) { wpcd_channels_destroy(c); return st; }
+    *out = c;
+    return WPCD_OK;
+}
+
+void wpcd_channels_destroy(wpcd_channels* c)
+{
+    if (!c) return;
+    free_channels_device(c);
+    delete c;
+}
+
+int wpcd_channels_count(const wpcd_channels* c) { return c ? c->n_ch : 0; }
+int wpcd_channels_pairs(const wpcd_channels* c) { return c ? c->n_pairs : 0; }
+int64_t wpcd_channels_terms(const wpcd_channels* c) { return c ? c->n_terms : 0; }
+
+wpcd_status wpcd_channels_get_quantum_numbers(const wpcd_channels* c, int32_t* out)
+{
+    if (!c || !out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_get_quantum_numbers: null pointer");
+    std::memcpy(out, c->qn.data(), sizeof(int32_t) * c->qn.size());
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_channels_get_table(const wpcd_channels* c, int32_t* pair_gamma, int32_t* pair_gammap, int64_t* term_ptr,
+                                    int32_t* term_k, int32_t* term_l1, int32_t* term_l1p, double* term_g)
+{
+    if (!c || !pair_gamma || !pair_gammap || !term_ptr || !term_k || !term_l1 || !term_l1p || !term_g)
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_channels_get_table: null pointer");
+    std::memcpy(pair_gamma, c->pair_gamma.data(), sizeof(int32_t) * c->n_pairs);
+    std::memcpy(pair_gammap, c->pair_gammap.data(), sizeof(int32_t) * c->n_pairs);
+    std::memcpy(term_ptr, c->term_ptr.data(), sizeof(int64_t) * (c->n_pairs + 1));
+    std::memcpy(term_k, c->term_k.data(), sizeof(int32_t) * c->n_terms);
+    std::memcpy(term_l1, c->term_l1.data(), sizeof(int32_t) * c->n_terms);
+    std::memcpy(term_l1p, c->term_l1p.data(), sizeof(int32_t) * c->n_terms);
+    std::memcpy(term_g, c->term_g.data(), sizeof(double) * c->n_terms);
+    return WPCD_OK;
+}
+
+int64_t wpcd_rows(const wpcd_grid* g, const wpcd_channels* c) { return (g && c) ? (int64_t)c->n_ch * g->n_p * g->n_q : 0; }
+int64_t wpcd_geo_rows(const wpcd_grid* g) { return g ? (int64_t)g->n_p * g->n_q : 0; }
+
+wpcd_status wpcd_perm_count(const wpcd_grid* g, const wpcd_channels* c, int n_quad, void* cuda_stream, int64_t* row_ptr_dev,
+                            int32_t* geo_row_ptr_dev, int64_t* nnz_out, int64_t* nnz_geo_out)
+{
+    if (!g || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_count: null pointer");
+    if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_count: n_quad out of range");
+    if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_count: channel tables are not on a device (no CUDA device?)");
+    int64_t rows = wpcd_rows(g, c);
+    if (rows > (int64_t)INT32_MAX) return fail(WPCD_ERR_OVERFLOW, "wpcd_perm_count: column index would not fit int32");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int n_geo = g->n_p * g->n_q;
+    cudaError_t err = launch_geo_count(g, geo_row_ptr_dev, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_count(count)");
+    err = launch_scan_rowptr(g, c, geo_row_ptr_dev, row_ptr_dev, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_count(scan)");
+    err = cudaMemcpyAsync(g->nnz_geo_pinned, geo_row_ptr_dev + n_geo, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_count(sync)");
+    int64_t nnz_geo = *g->nnz_geo_pinned;
+    *nnz_geo_out = nnz_geo;
+    *nnz_out = nnz_geo * c->total_coupled;
+    {
+        std::lock_guard<std::mutex> lock(g_hint_mutex);
+        g_nnz_hint[row_ptr_dev] = {rows, *nnz_out};
+    }
+    return WPCD_OK;
+}
+
+size_t wpcd_perm_workspace_bytes(const wpcd_channels* c, int64_t nnz_geo)
+{
+    if (!c || nnz_geo < 0) return 0;
+    return carve_workspace(c, nnz_geo, nullptr).bytes;
+}
+
+wpcd_status wpcd_perm_build(const wpcd_grid* g, const wpcd_channels* c, int n_quad, void* cuda_stream, const int64_t* row_ptr_dev,
+                            const int32_t* geo_row_ptr_dev, void* workspace_dev, size_t workspace_bytes, int32_t* col_idx_dev,
+                            double* values_dev)
+{
+    if (!g || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
+    if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: n_quad out of range");
+    if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_build: channel tables are not on a device (no CUDA device?)");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int64_t nnz_geo = -1;
+    {
+        std::lock_guard<std::mutex> lock(g_hint_mutex);
+        auto it = g_nnz_hint.find(row_ptr_dev);
+        if (it != g_nnz_hint.end() && it->second.first == wpcd_rows(g, c) && c->total_coupled > 0) nnz_geo = it->second.second / c->total_coupled;
+    }
+    if (nnz_geo < 0 || c->total_coupled == 0) {   // row_ptr not produced by this process' wpcd_perm_count: read the count back
+        int32_t v = 0;
+        cudaError_t err = cudaMemcpyAsync(g->nnz_geo_pinned, geo_row_ptr_dev + g->n_p * g->n_q, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(read nnz_geo)");
+        v = *g->nnz_geo_pinned;
+        nnz_geo = v;
+    }
+    if (nnz_geo == 0 || c->total_coupled == 0) return WPCD_OK;
+    if (!workspace_dev || !col_idx_dev || !values_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null output or workspace");
+    if ((reinterpret_cast<uintptr_t>(workspace_dev) & 255) != 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: workspace must be 256-byte aligned");
+    Workspace ws = carve_workspace(c, nnz_geo, workspace_dev);
+    if (workspace_bytes < ws.bytes) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: workspace too small");
+    cudaError_t err = launch_geo_index(g, geo_row_ptr_dev, ws.geo_col, ws.geo_row, ws.geo_phi, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(index)");
+    double xi[WPCD_MAX_QUAD], w[WPCD_MAX_QUAD];
+    wpcd_host::gauss_legendre(n_quad, xi, w);
+    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
+    else err = launch_fill_coupled(g, c, n_quad, xi, w, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(fill)");
+    return WPCD_OK;
+}
+
+static double mean_row_hint(int64_t rows, const int64_t* row_ptr_dev, cudaStream_t st)
+{
+    {
+        std::lock_guard<std::mutex> lock(g_hint_mutex);
+        auto it = g_nnz_hint.find(row_ptr_dev);
+        if (it != g_nnz_hint.end() && it->second.first == rows) return (double)it->second.second / (double)std::max<int64_t>(rows, 1);
+    }
+    int64_t nnz = 0;
+    if (cudaMemcpyAsync(&nnz, row_ptr_dev + rows, sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess) return 32.0;
+    cudaStreamSynchronize(st);
+    std::lock_guard<std::mutex> lock(g_hint_mutex);
+    g_nnz_hint[row_ptr_dev] = {rows, nnz};
+    return (double)nnz / (double)std::max<int64_t>(rows, 1);
+}
+
+wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                            const double* x_dev, double* y_dev, int n_vec, void* cuda_stream)
+{
+    if (rows < 0 || n_vec < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply: negative size");
+    if (rows == 0 || n_vec == 0) return WPCD_OK;
+    if (!row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply: null pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
+    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply: null matrix arrays");
+    cudaError_t err = launch_spmv(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, mean_row, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                 const double* x_host, double* y_host, int n_vec, double* x_dev, double* y_dev, void* cuda_stream)
+{
+    if (rows < 0 || n_vec < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_host: negative size");
+    if (rows == 0 || n_vec == 0) return WPCD_OK;
+    if (!x_host || !y_host || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_host: null pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    size_t bytes = sizeof(double) * (size_t)rows * (size_t)n_vec;
+    cudaError_t err = cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(H2D)");
+    wpcd_status s = wpcd_perm_apply(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, cuda_stream);
+    if (s != WPCD_OK) return s;
+    err = cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(D2H)");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out)
+{
+    if (!flops_out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_fp64_peak: null pointer");
+    cudaError_t err = run_fp64_peak(static_cast<cudaStream_t>(cuda_stream), flops_out);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_fp64_peak");
+    return WPCD_OK;
+}
+
+int64_t wpcd_launch_count(void) { return g_launches; }
+
+}  // extern "C"

@@ -1,0 +1,102 @@
+// fill.cu -- "calculation of the nonzero elements of P0" (paper step 3):
+// FP64 Gauss-Legendre quadrature of (A15) over the clipped overlap region.
+//
+// Two paths:
+//  * s-wave (configs 1-2): one channel, one term; LPE lanes share one element, each lane
+//    owns whole phi-nodes and runs the inner x-rule; shuffles reduce.
+//  * coupled channels (configs 3-5): monomial moments
+//        M[mu] = sum_nodes w F P_k(x) cos^{A+1} sin^{B+1} / (zeta1^{l'+1} zeta2^{l+1})
+//    per geometric element (kernel moments), then value[pair] = sum_terms g M[mu] for all
+//    coupled channel pairs with the moment tile staged in shared memory (kernel contract).
+#include <math.h>
+
+#include "quad_device.cuh"
+#include "wpcd_internal.h"
+
+using namespace wpcd_quad;
+
+namespace {
+
+__constant__ double c_xi[WPCD_MAX_QUAD];
+__constant__ double c_w[WPCD_MAX_QUAD];
+
+// ------------------------------------------------------------------ s-wave
+template <int LPE>
+__global__ void __launch_bounds__(256)
+fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n, double g0,
+                  int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
+                  const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t e = t / LPE;
+    const int sub = (int)(t - e * LPE);
+    const bool valid = e < nnz_geo;
+    double acc = 0.0;
+    double norm = 0.0;
+    int col = 0;
+    if (valid) {
+        col = geo_col[e];
+        const int row = geo_row[e];
+        const double2 ph = geo_phi[e];
+        const Cell z = load_cell(p, q, n_q, row, col);
+        norm = cell_norm(z);
+        const double half_phi = 0.5 * (ph.y - ph.x), mid_phi = 0.5 * (ph.x + ph.y);
+        if (ph.x < ph.y) {
+            for (int m = sub; m < n; m += LPE) {
+                PhiNode s;
+                if (!phi_node(z, mid_phi + half_phi * c_xi[m], s)) continue;
+                const double half_u = 0.5 * (s.u_hi - s.u_lo), mid_u = 0.5 * (s.u_lo + s.u_hi);
+                double inner = 0.0;
+                for (int r = 0; r < n; ++r) {
+                    const double u = mid_u + half_u * c_xi[r];
+                    const double iz1 = rsqrt(s.b1 + s.beta * u), iz2 = rsqrt(s.b2 + s.beta * u);
+                    inner += c_w[r] * F_A14(z, s, iz1, iz2) * iz1 * iz2;
+                }
+                acc += half_phi * c_w[m] * half_u * s.beta * inner;    // cos*sin = beta
+            }
+        }
+    }
+#pragma unroll
+    for (int o = LPE / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (valid && sub == 0) {
+        values[e] = g0 * norm * acc;
+        col_idx[e] = col;
+    }
+}
+
+}  // namespace
+
+namespace wpcd_detail {
+
+cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, const double* xi, const double* w,
+                              int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st)
+{
+    cudaError_t err = cudaMemcpyToSymbolAsync(c_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return err;
+    err = cudaMemcpyToSymbolAsync(c_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return err;
+    if (nnz_geo == 0) return cudaSuccess;
+    // lanes per element: whole phi-nodes per lane, no idle lanes when n is a multiple of LPE
+    int lpe = (n_quad % 8 == 0) ? 8 : (n_quad % 4 == 0) ? 4 : (n_quad % 2 == 0) ? 2 : 1;
+    int64_t threads = nnz_geo * lpe;
+    int blocks = (int)((threads + 255) / 256);
+#define WPCD_LAUNCH_SW(L) fill_swave_kernel<L><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
+                                                                       ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
+    switch (lpe) {
+    case 8: WPCD_LAUNCH_SW(8); break;
+    case 4: WPCD_LAUNCH_SW(4); break;
+    case 2: WPCD_LAUNCH_SW(2); break;
+    default: WPCD_LAUNCH_SW(1); break;
+    }
+#undef WPCD_LAUNCH_SW
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fill_coupled(const wpcd_grid*, const wpcd_channels*, int, const double*, const double*, int64_t,
+                                const Workspace&, const int64_t*, const int32_t*, int32_t*, double*, cudaStream_t)
+{
+    return cudaErrorNotSupported;
+}
+
+}  // namespace wpcd_detail

@@ -1,0 +1,125 @@
+// spmv.cu -- y = P0 x (CSR, int64 row_ptr, int32 col_idx, FP64), the product applied inside
+// the iterative solution of eq. (12) (paper step 5; sparse storage PAPER.md:304).
+// HBM-bound: 12 B per nonzero streamed once, x gathered through L2.
+// LPR lanes cooperate on one row (coalesced col/value loads), chosen from the mean row
+// length; up to 4 right-hand sides share one pass over the matrix.
+#include "wpcd_internal.h"
+
+namespace {
+
+template <int LPR, int NV>
+__global__ void __launch_bounds__(256)
+spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+            const double* __restrict__ values, const double* __restrict__ x, double* __restrict__ y, int64_t ldx)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t row = t / LPR;
+    const int sub = (int)(t - row * LPR);
+    double acc[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) acc[v] = 0.0;
+    if (row < rows) {
+        const int64_t beg = row_ptr[row], end = row_ptr[row + 1];
+        for (int64_t e = beg + sub; e < end; e += LPR) {
+            const double a = values[e];
+            const int c = col_idx[e];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) acc[v] = fma(a, __ldg(x + v * ldx + c), acc[v]);
+        }
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+#pragma unroll
+        for (int o = LPR / 2; o > 0; o >>= 1) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], o);
+    }
+    if (row < rows && sub == 0) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) y[v * ldx + row] = acc[v];
+    }
+}
+
+template <int LPR, int NV>
+cudaError_t launch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
+                   double* y, cudaStream_t st)
+{
+    int64_t threads = rows * LPR;
+    int64_t blocks = (threads + 255) / 256;
+    spmv_kernel<LPR, NV><<<(unsigned)blocks, 256, 0, st>>>(rows, row_ptr, col_idx, values, x, y, rows);
+    ++wpcd_detail::g_launches;
+    return cudaGetLastError();
+}
+
+template <int NV>
+cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
+                     double* y, double mean_row, cudaStream_t st)
+{
+    if (mean_row <= 6.0) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (mean_row <= 16.0) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (mean_row <= 48.0) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
+}
+
+// ---------------------------------------------------------------- FP64 FMA peak
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double seed)
+{
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 12345.678) out[0] = s;   // never true; keeps the chains alive
+}
+
+}  // namespace
+
+namespace wpcd_detail {
+
+cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+                        const double* x, double* y, int n_vec, double mean_row, cudaStream_t st)
+{
+    int v = 0;
+    while (v < n_vec) {
+        const double* xv = x + (int64_t)v * rows;
+        double* yv = y + (int64_t)v * rows;
+        cudaError_t err;
+        if (n_vec - v >= 4) { err = dispatch<4>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 4; }
+        else if (n_vec - v >= 2) { err = dispatch<2>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 2; }
+        else { err = dispatch<1>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 1; }
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
+}
+
+cudaError_t run_fp64_peak(cudaStream_t st, double* flops_out)
+{
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    double* out = nullptr;
+    cudaError_t err = cudaMalloc(&out, sizeof(double));
+    if (err != cudaSuccess) return err;
+    const int iters = 1 << 15, blocks = sms * 8, threads = 256;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        dfma_peak_kernel<<<blocks, threads, 0, st>>>(out, iters, 1.0);
+        ++g_launches;
+        cudaEventRecord(e1, st);
+        err = cudaEventSynchronize(e1);
+        if (err != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double flops = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3);
+        if (rep > 0 && flops > best) best = flops;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    *flops_out = best;
+    return err;
+}
+
+}  // namespace wpcd_detail

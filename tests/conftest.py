@@ -27,3 +27,15 @@ def nd_half_plus_j1():
 
     ch = channels.enumerate_channels(1, +1, 1)
     return perm.PairTable(ch, channels.g_table(ch, 1, 1))
+
+
+@pytest.fixture(scope="session")
+def wpcd():
+    """The product binding, with libwpcd.so (re)built in-tree if sources are newer."""
+    from paper_1404_5253_b200 import build as _build
+
+    _build.build()
+    import paper_1404_5253_b200 as mod
+
+    mod.load()
+    return mod

@@ -1,0 +1,173 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element.  Pattern (row_ptr, col_idx) bit-exact; values within
+    1e-11 * max(|v|, A_e) + 1e-13 * V
+where A_e is the element's absolute-sum scale computed by the oracle and V = max|v| of the
+matrix: the floor covers the ill-conditioned sliver elements next to the pi1 = 0 / pi2 = 0
+corners, where rule R(n) itself is only ~1e-8 accurate in double precision (R9).
+SpMV within 1e-12 * sum_j |a_ij x_j|."""
+import numpy as np
+import pytest
+
+import wpcd_inputs as wi
+from oracle import channels as och
+from oracle import perm as operm
+
+pytestmark = pytest.mark.gpu
+
+VALUE_RTOL = 1e-11
+VALUE_FLOOR = 1e-13   # times max|v| of the matrix
+
+
+def _torch():
+    import torch
+
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _oracle_table(wl, two_J=None, parity=None):
+    if wl.model == "swave":
+        ch, pairs = och.spinless_swave_table(wl.g0)
+    else:
+        ch = och.enumerate_channels(two_J, parity, wl.j_pair_max)
+        pairs = och.g_table(ch, two_J, 1)
+    return operm.PairTable(ch, pairs)
+
+
+def _gpu_channels(wpcd, wl, two_J=None, parity=None):
+    if wl.model == "swave":
+        return wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=wl.g0)
+    return wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=wl.j_pair_max)
+
+
+def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None):
+    grid = wpcd.wpcd_grid_create(p, q)
+    m = wpcd.build_perm(grid, gch, n_quad)
+    _torch().cuda.synchronize()
+    geo = operm.geo_pattern(p, q)
+    rp, ci, v, av = operm.build_csr(p, q, n_quad, tab, geo=geo, geo_rows=geo_rows)
+    assert m.nnz == rp[-1] and m.nnz_geo == geo[0][-1]
+    assert np.array_equal(m.geo_row_ptr.cpu().numpy().astype(np.int64), geo[0])
+    assert np.array_equal(m.row_ptr.cpu().numpy(), rp)
+    assert np.array_equal(m.col_idx.cpu().numpy(), ci)
+    gv = m.values.cpu().numpy()
+    sel = ~np.isnan(v)
+    assert sel.any()
+    err = np.abs(gv[sel] - v[sel])
+    tol = VALUE_RTOL * np.maximum(np.abs(v[sel]), av[sel]) + VALUE_FLOOR * np.abs(v[sel]).max()
+    worst = np.max(err / np.maximum(tol, 1e-300)) if len(err) else 0.0
+    assert np.all(err <= tol), f"worst err/tol = {worst}"
+    assert np.all(np.isfinite(gv))
+    return m, (rp, ci, v, av)
+
+
+def test_cfg1_swave_n20(wpcd):
+    wl = wi.WORKLOADS["cfg1"]
+    p = wl.grid()
+    _compare_full(wpcd, p, p, wl.n_quad, _gpu_channels(wpcd, wl), _oracle_table(wl))
+
+
+def test_cfg2_swave_n100_and_spmv(wpcd):
+    torch = _torch()
+    wl = wi.WORKLOADS["cfg2"]
+    p = wl.grid()
+    m, (rp, ci, v, av) = _compare_full(wpcd, p, p, wl.n_quad, _gpu_channels(wpcd, wl), _oracle_table(wl))
+    rows = m.rows
+    y = torch.empty(rows, dtype=torch.float64, device="cuda")
+    gv = m.values.cpu().numpy()   # the product on the SAME matrix: isolates the SpMV kernel
+    for k in range(3):
+        xh = wi.normal_vector(rows, k=k)
+        x = torch.from_numpy(xh).cuda()
+        wpcd.wpcd_perm_apply(rows, m.row_ptr, m.col_idx, m.values, x, y)
+        ref = operm.spmv(rp, ci, gv, xh)
+        scale = operm.spmv(rp, ci, np.abs(gv), np.abs(xh))
+        assert np.all(np.abs(y.cpu().numpy() - ref) <= 1e-12 * scale + 1e-300)
+
+
+@pytest.mark.parametrize("n_quad", [1, 3, 4, 6, 10, 12, 48, 64])
+def test_quadrature_orders(wpcd, n_quad):
+    p = wi.tan2_grid(9, 1.0, 0.1, seed=21)
+    q = wi.tan2_grid(7, 0.6, 0.1, seed=22)
+    ch, pairs = och.spinless_swave_table(1.0)
+    _compare_full(wpcd, p, q, n_quad, wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=1.0), operm.PairTable(ch, pairs))
+
+
+def test_edge_grids(wpcd):
+    ch, pairs = och.spinless_swave_table(0.5)
+    tab = operm.PairTable(ch, pairs)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    # single cell; grids that do not start at zero; very uneven bins; ragged n_p != n_q
+    cases = [
+        (np.array([0.0, 0.37]), np.array([0.0, 0.37])),
+        (np.array([0.3, 0.5, 2.0]), np.array([0.1, 0.2, 0.9, 4.0])),
+        (np.array([0.0, 1e-3, 1.0, 50.0]), np.array([0.0, 2.0])),
+        (wi.tan2_grid(33, 2.0, 0.2, seed=5), wi.tan2_grid(5, 0.5, 0.0)),
+    ]
+    for p, q in cases:
+        _compare_full(wpcd, p, q, 8, gch, tab)
+
+
+def test_disjoint_cells_give_empty_matrix(wpcd):
+    # p-cells far above anything q,q' can reach: no structural nonzeros at all
+    torch = _torch()
+    p = np.array([100.0, 101.0])
+    q = np.array([0.0, 1.0])
+    grid = wpcd.wpcd_grid_create(p, q)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    m = wpcd.build_perm(grid, gch, 8)
+    assert m.nnz == 0 and operm.geo_pattern(p, q)[0][-1] == 0
+    x = torch.ones(1, dtype=torch.float64, device="cuda")
+    y = torch.full((1,), 7.0, dtype=torch.float64, device="cuda")
+    wpcd.wpcd_perm_apply(1, m.row_ptr, m.col_idx, m.values, x, y)
+    assert y.item() == 0.0
+
+
+def test_apply_multi_vector_and_host(wpcd):
+    torch = _torch()
+    p = wi.tan2_grid(24, 1.0, 0.1, seed=8)
+    grid = wpcd.wpcd_grid_create(p, p)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    m = wpcd.build_perm(grid, gch, 8)
+    rows = m.rows
+    rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    for n_vec in (1, 2, 3, 7):
+        xh = np.stack([wi.normal_vector(rows, k=10 + k) for k in range(n_vec)])
+        x = torch.from_numpy(xh).cuda().contiguous()
+        y = torch.empty_like(x)
+        wpcd.wpcd_perm_apply(rows, m.row_ptr, m.col_idx, m.values, x, y, n_vec=n_vec)
+        for k in range(n_vec):
+            ref = operm.spmv(rp, ci, v, xh[k])
+            scale = operm.spmv(rp, ci, np.abs(v), np.abs(xh[k]))
+            assert np.all(np.abs(y[k].cpu().numpy() - ref) <= 1e-12 * scale)
+    xh = torch.from_numpy(wi.normal_vector(rows, k=99)).pin_memory()
+    yh = torch.empty(rows, dtype=torch.float64).pin_memory()
+    xd = torch.empty(rows, dtype=torch.float64, device="cuda")
+    yd = torch.empty_like(xd)
+    wpcd.wpcd_perm_apply_host(rows, m.row_ptr, m.col_idx, m.values, xh, yh, xd, yd)
+    ref = operm.spmv(rp, ci, v, xh.numpy())
+    assert np.all(np.abs(yh.numpy() - ref) <= 1e-12 * operm.spmv(rp, ci, np.abs(v), np.abs(xh.numpy())))
+
+
+def test_errors_on_device_path(wpcd):
+    torch = _torch()
+    p = wi.tan2_grid(4)
+    grid = wpcd.wpcd_grid_create(p, p)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    row_ptr = torch.empty(17, dtype=torch.int64, device="cuda")
+    geo = torch.empty(17, dtype=torch.int32, device="cuda")
+    with pytest.raises(wpcd.WpcdError, match="n_quad"):
+        wpcd.wpcd_perm_count(grid, gch, 0, row_ptr, geo)
+    with pytest.raises(wpcd.WpcdError, match="n_quad"):
+        wpcd.wpcd_perm_count(grid, gch, 65, row_ptr, geo)
+    nnz, nnz_geo = wpcd.wpcd_perm_count(grid, gch, 8, row_ptr, geo)
+    col = torch.empty(nnz, dtype=torch.int32, device="cuda")
+    val = torch.empty(nnz, dtype=torch.float64, device="cuda")
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(wpcd.WpcdError, match="workspace too small"):
+        wpcd.wpcd_perm_build(grid, gch, 8, row_ptr, geo, small, col, val)
+
+
+def test_fp64_peak_microbenchmark(wpcd):
+    flops = wpcd.wpcd_fp64_peak()
+    assert 5e12 < flops < 1e14
+    assert wpcd.wpcd_launch_count() > 0

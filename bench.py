@@ -1,0 +1,447 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path (pattern
+count, scan, column indices, FP64 fill, then the workload's P0*x products) over one synthetic
+lattice.  Default workload: BASELINE.json configs[1] ("cfg2": s-wave, N_p=N_q=100 jittered tan^2
+grid, 8-point Gauss-Legendre, 50 SpMVs).  Prints ONE JSON line (contract in the task statement).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1..cfg5] [--impl reference]
+
+N > 1 (torchrun): every rank builds its own independent lattice (seed + rank) -- the path
+shards over independent problems, no data-path collective ("scaling": "weak").
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import wpcd_inputs as wi  # noqa: E402
+
+METRIC = "P-matrix nonzeros/sec (FP64 build + the workload's P*vector SpMVs per step)"
+UNIT = "nnz/s"
+FLOPS_PER_NODE = 70.0          # algorithmic FP64 flops per (phi,x) quadrature node, s-wave
+L2_FLUSH_BYTES = 256 << 20     # > 126 MB L2
+
+
+# --------------------------------------------------------------------------- helpers
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.sm_max = index, False, [], set(), None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+        }
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+def jobs_of(wl):
+    """[(two_J, parity)] per step; the s-wave workloads have one (dummy) job."""
+    return wl.jpis if wl.model == "nd" else [(0, 0)]
+
+
+# --------------------------------------------------------------------------- reference arm (oracle on host cores)
+def oracle_tables(wl):
+    from oracle import channels as och
+    from oracle import perm as operm
+
+    tabs = []
+    for (two_J, parity) in jobs_of(wl):
+        if wl.model == "swave":
+            ch, pairs = och.spinless_swave_table(wl.g0)
+        else:
+            ch = och.enumerate_channels(two_J, parity, wl.j_pair_max)
+            pairs = och.g_table(ch, two_J, 1)
+        tabs.append(operm.PairTable(ch, pairs))
+    return tabs
+
+
+def oracle_pass(wl, tabs, row_stride):
+    """One bounded oracle pass: full pattern, values on every row_stride-th geometric row (all
+    channels), the workload's SpMVs on the s-wave workloads.  Returns (nnz_evaluated, seconds)."""
+    from oracle import perm as operm
+
+    p = wl.grid()
+    t0 = time.perf_counter()
+    geo = operm.geo_pattern(p, p)
+    n_geo = wl.n_bins * wl.n_bins
+    rows = np.arange(0, n_geo, row_stride)
+    done = 0
+    for tab in tabs:
+        if wl.model == "swave" and row_stride == 1:
+            rp, ci, v, _ = operm.build_csr(p, p, wl.n_quad, tab, geo=geo)
+            done += len(v)
+            for k in range(wl.n_spmv):
+                operm.spmv(rp, ci, v, wi.normal_vector(len(rp) - 1, k=k))
+        else:
+            cnt = (geo[0][rows + 1] - geo[0][rows])
+            erow = np.repeat(rows, cnt)
+            eidx = np.concatenate([np.arange(geo[0][r], geo[0][r + 1]) for r in rows])
+            ecol = geo[1][eidx]
+            n_q = wl.n_bins
+            val, _ = operm.element_values(p, p, erow // n_q, erow % n_q, ecol // n_q, ecol % n_q, wl.n_quad, tab)
+            done += val.size
+    return done, time.perf_counter() - t0
+
+
+def reference_row_stride(wl):
+    return 1 if wl.model == "swave" else (16 if wl.name == "cfg3" else 256)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import perm as operm
+
+    wl = wi.WORKLOADS[args.workload]
+    tabs = oracle_tables(wl)
+    stride = reference_row_stride(wl)
+    for _ in range(max(args.warmup, 0) and 1):
+        oracle_pass(wl, tabs, stride)
+    steps = max(1, min(args.steps, 5))
+    t, nnz = 0.0, 0
+    for _ in range(steps):
+        n, dt = oracle_pass(wl, tabs, stride)
+        t += dt
+        nnz += n
+    value = nnz / t
+    sample = (f"full {wl.name} pass (pattern + values + {wl.n_spmv} SpMV)" if stride == 1
+              else f"full pattern + values of every {stride}th geometric row, all channel pairs")
+    cores = operm.num_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": 1 if args.warmup else 0, "ms_per_step": 1e3 * t / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "n_bins": wl.n_bins, "n_quad": wl.n_quad, "model": wl.model, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------- our arm
+class Job:
+    """One (J, parity) matrix.  Device buffers are views into a pool shared by all jobs of the
+    step (sized for the largest), so only one matrix is resident at a time (DESIGN.md memory plan)."""
+
+    def __init__(self, channels, rows):
+        self.channels, self.rows = channels, rows
+        self.nnz = self.nnz_geo = 0
+        self.graph = None
+
+
+def allocate(wpcd, torch, grid, jobs, wl):
+    n_geo = grid.n_p * grid.n_q
+    max_rows = max(j.rows for j in jobs)
+    row_ptr = torch.empty(max_rows + 1, dtype=torch.int64, device="cuda")
+    geo_row_ptr = torch.empty(n_geo + 1, dtype=torch.int32, device="cuda")
+    ws_bytes = 256
+    for j in jobs:
+        j.row_ptr, j.geo_row_ptr = row_ptr[: j.rows + 1], geo_row_ptr
+        j.nnz, j.nnz_geo = wpcd.wpcd_perm_count(grid, j.channels, wl.n_quad, j.row_ptr, j.geo_row_ptr)
+        ws_bytes = max(ws_bytes, wpcd.wpcd_perm_workspace_bytes(j.channels, j.nnz_geo))
+    max_nnz = max(j.nnz for j in jobs)
+    col_idx = torch.empty(max_nnz, dtype=torch.int32, device="cuda")
+    values = torch.empty(max_nnz, dtype=torch.float64, device="cuda")
+    workspace = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
+    n_x = max(1, wl.n_spmv) if wl.model == "swave" else max(1, min(wl.n_spmv, 4))
+    x_host = torch.from_numpy(np.stack([wi.normal_vector(max_rows, k=k) for k in range(n_x)])).pin_memory()
+    x = x_host.cuda()
+    y = torch.empty(max_rows, dtype=torch.float64, device="cuda")
+    y_host = torch.empty(max_rows, dtype=torch.float64).pin_memory()
+    for j in jobs:
+        j.col_idx, j.values, j.workspace = col_idx[: j.nnz], values[: j.nnz], workspace
+        j.n_x = n_x
+        j.x = [x[k, : j.rows] for k in range(n_x)]
+        j.x_host = [x_host[k, : j.rows] for k in range(n_x)]
+        j.y, j.y_host = y[: j.rows], y_host[: j.rows]
+
+
+def run_ours(args):
+    import torch
+
+    from paper_1404_5253_b200 import build as _build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if rank == 0:
+        _build.build()
+    import paper_1404_5253_b200 as wpcd
+
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    wpcd.load()
+    wl = wi.WORKLOADS[args.workload]
+    p = wl.grid(seed_offset=rank)           # independent lattice per rank (weak scaling)
+    stream = torch.cuda.current_stream()
+    grid = wpcd.wpcd_grid_create(p, p)
+
+    def make_channels(two_J, parity):
+        if wl.model == "swave":
+            return wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=wl.g0)
+        return wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=wl.j_pair_max)
+
+    # one J^pi matrix resident at a time; buffers sized for the largest
+    jobs = []
+    for (two_J, parity) in jobs_of(wl):
+        ch = make_channels(two_J, parity)
+        jobs.append(Job(ch, wpcd.wpcd_rows(grid, ch)))
+    allocate(wpcd, torch, grid, jobs, wl)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    n_spmv = wl.n_spmv
+
+    def spmv_sweep(job):
+        for k in range(n_spmv):
+            wpcd.wpcd_perm_apply(job.rows, job.row_ptr, job.col_idx, job.values, job.x[k % job.n_x], job.y)
+
+    def step(job_list):
+        for job in job_list:
+            wpcd.wpcd_perm_count(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr)
+            wpcd.wpcd_perm_build(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+            if n_spmv:
+                if job.graph is not None:
+                    job.graph.replay()
+                else:
+                    spmv_sweep(job)
+
+    # capture the launch-bound SpMV sweep in a CUDA graph (small matrices only)
+    step(jobs)
+    torch.cuda.synchronize()
+    if n_spmv and wl.model == "swave":
+        for job in jobs:
+            g = torch.cuda.CUDAGraph()
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                spmv_sweep(job)
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            with torch.cuda.graph(g):
+                spmv_sweep(job)
+            job.graph = g
+    for _ in range(args.warmup):
+        step(jobs)
+    torch.cuda.synchronize()
+    fp64_peak = wpcd.wpcd_fp64_peak()
+
+    # ---- timed region: device-resident inputs
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    wpcd.wpcd_trace_enable(True)
+    wpcd.wpcd_trace_read()
+    launches0 = wpcd.wpcd_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sp_ev = []
+    for s in range(args.steps):
+        flush.fill_(s & 0xFF)                       # L2 flush between timed iterations (not timed)
+        ev[s][0].record()
+        for job in jobs:
+            wpcd.wpcd_perm_count(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr)
+            wpcd.wpcd_perm_build(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+            if n_spmv:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                if job.graph is not None:
+                    job.graph.replay()
+                else:
+                    spmv_sweep(job)
+                b.record()
+                sp_ev.append((a, b))
+        ev[s][1].record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    graph_launches = sum(n_spmv for job in jobs if job.graph is not None) * args.steps
+    launches = wpcd.wpcd_launch_count() - launches0 + graph_launches
+    stages = wpcd.wpcd_trace_read()
+    wpcd.wpcd_trace_enable(False)
+    sampler.stop_flag = True
+    sampler.join()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    spmv_ms = sum(a.elapsed_time(b) for a, b in sp_ev)
+    t_local = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    nnz_local = torch.tensor([float(sum(j.nnz for j in jobs))], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t_local, op=dist.ReduceOp.MAX)
+        dist.all_reduce(nnz_local, op=dist.ReduceOp.SUM)
+    ms_per_step = t_local.item() / args.steps
+    nnz_all = nnz_local.item()
+    value = nnz_all / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C-ABI with HOST buffers (handles, tables and vectors from the host)
+    def e2e_step():
+        g2 = wpcd.wpcd_grid_create(p, p)
+        for job, (two_J, parity) in zip(jobs, jobs_of(wl)):
+            ch2 = make_channels(two_J, parity)
+            wpcd.wpcd_perm_count(g2, ch2, wl.n_quad, job.row_ptr, job.geo_row_ptr)
+            wpcd.wpcd_perm_build(g2, ch2, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+            for k in range(n_spmv):
+                wpcd.wpcd_perm_apply_host(job.rows, job.row_ptr, job.col_idx, job.values, job.x_host[k % job.n_x], job.y_host,
+                                          job.x[0], job.y)
+    e2e_steps = max(1, min(args.steps, 20))
+    e2e_step()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = nnz_all / (e2e_s.item() / e2e_steps)
+    table_bytes = sum(12 * j.channels.terms + 8 * j.channels.pairs + 16 * j.channels.count for j in jobs)
+    h2d = 2 * 8 * (wl.n_bins + 1) + table_bytes + sum(8 * j.rows * n_spmv for j in jobs)
+    d2h = sum(8 * j.rows * n_spmv + 4 for j in jobs)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- rooflines (per launch, averaged over the timed region)
+    peaks, peak_kind = measured_peaks()
+    nnz1 = sum(j.nnz for j in jobs)
+    nnz_geo1 = sum(j.nnz_geo for j in jobs)
+    rows1 = sum(j.rows for j in jobs)
+    steps = args.steps
+    roofs = {}
+    stage_ms = {k: v[0] / steps for k, v in stages.items()}
+    if stage_ms["fill_swave"] > 0:
+        flops = FLOPS_PER_NODE * wl.n_quad * wl.n_quad * nnz1
+        ach = flops / (stage_ms["fill_swave"] * 1e-3) / 1e12
+        roofs["fill_swave"] = {"bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
+                               "frac": ach / (fp64_peak / 1e12), "traffic": None, "ms_per_launch": stage_ms["fill_swave"],
+                               "peak_source": "in-run DFMA microbenchmark (wpcd_fp64_peak)"}
+    if stage_ms["moments"] > 0 or stage_ms["contract"] > 0:
+        wbytes = 12.0 * nnz1
+        t = (stage_ms["moments"] + stage_ms["contract"]) * 1e-3
+        ach = wbytes / t / 1e9
+        roofs["fill_coupled"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                 "frac": ach / peaks["hbm_gbs"], "traffic": None,
+                                 "ms_per_step": {"moments": stage_ms["moments"], "contract": stage_ms["contract"]},
+                                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})"}
+    if n_spmv:
+        per_launch_ms = spmv_ms / (steps * n_spmv * len(jobs))
+        sbytes = (12.0 * nnz1 + 16.0 * rows1 + 8.0 * rows1) / len(jobs)
+        ach = sbytes / (per_launch_ms * 1e-3) / 1e9
+        roofs["spmv"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                         "traffic": None, "ms_per_launch": per_launch_ms, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})",
+                         "note": "matrix is L2-resident (3 MB)" if wl.model == "swave" else "streams from HBM"}
+    share = dict(stage_ms)
+    share["spmv_sweep"] = spmv_ms / steps
+    dominant = max(share, key=share.get)
+    key = {"fill_swave": "fill_swave", "moments": "fill_coupled", "contract": "fill_coupled", "spmv_sweep": "spmv"}.get(dominant)
+    roofline = dict(roofs[key]) if key in roofs else {
+        "bound": "alu", "achieved": None, "peak": fp64_peak / 1e12, "unit": "TFLOP/s", "frac": None, "traffic": None}
+    roofline["kernel"] = dominant
+
+    # ---- oracle on the host cores beside it (N = 1 only)
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import perm as operm
+
+        stride = reference_row_stride(wl)
+        n, dt = oracle_pass(wl, oracle_tables(wl), stride)
+        cpu_baseline = {"value": n / dt, "unit": UNIT, "cores": operm.num_threads(), "kind": "oracle",
+                        "sample": (f"full {wl.name} pass (pattern + values + {wl.n_spmv} SpMV), {dt:.1f} s" if stride == 1 else
+                                   f"full pattern + values of every {stride}th geometric row, all channel pairs, {dt:.1f} s")}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": wl.name, "n_bins": wl.n_bins, "n_quad": wl.n_quad, "model": wl.model, "jitter": wl.jitter,
+                   "jpis": jobs_of(wl) if wl.model == "nd" else None, "n_spmv_per_matrix": n_spmv,
+                   "nnz": nnz1, "nnz_geo": nnz_geo1, "rows": rows1, "l2": "flushed between timed steps (256 MiB fill)",
+                   "spmv_launch": "CUDA graph" if jobs[0].graph is not None else "direct"},
+        "clocks": sampler.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps, "includes": "grid/channel handle creation (host g-table), count, build, SpMVs with pinned-host x and y"},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "rooflines": roofs,
+        "stage_ms_per_step": share,
+        "build_nnz_per_s": nnz1 / max(1e-12, (ms_per_step - spmv_ms / steps) * 1e-3),
+        "fp64_peak_tflops_measured": fp64_peak / 1e12,
+        "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=sorted(wi.WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -152,6 +152,21 @@ wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const
  * (2 per DFMA) in *flops_out (host).  Synchronises. */
 wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out);
 
+/* Stage tracing for the roofline report: when enabled, CUDA events are recorded on the
+ * caller's stream around every kernel of wpcd_perm_count / wpcd_perm_build.
+ * wpcd_trace_read synchronises those events, ADDS the elapsed milliseconds of each stage since
+ * the last read into ms_out[WPCD_TRACE_STAGES] (host) and the launch counts into
+ * launches_out[WPCD_TRACE_STAGES] (host, may be NULL), then clears the record. */
+#define WPCD_TRACE_STAGES 6
+#define WPCD_STAGE_GEO_COUNT 0   /* predicate + per-row counts            (step a1) */
+#define WPCD_STAGE_SCAN 1        /* scan -> geo_row_ptr, row_ptr          (step a2) */
+#define WPCD_STAGE_GEO_INDEX 2   /* predicate + compaction of column list (step a3) */
+#define WPCD_STAGE_FILL_SWAVE 3  /* single-channel quadrature fill        (step a4) */
+#define WPCD_STAGE_MOMENTS 4     /* coupled channels: monomial moments    (step a4) */
+#define WPCD_STAGE_CONTRACT 5    /* coupled channels: g-contraction+store (step a4) */
+wpcd_status wpcd_trace_enable(int on);
+wpcd_status wpcd_trace_read(double* ms_out, int64_t* launches_out);
+
 /* Number of kernels the library has launched from this process (bench.py's gpu_launches). */
 int64_t wpcd_launch_count(void);
 

@@ -30,8 +30,9 @@ EXPORTS = [
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_fp64_peak", "wpcd_launch_count",
+    "wpcd_perm_apply_host", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
 ]
+TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
 
 
 class WpcdError(RuntimeError):
@@ -77,6 +78,8 @@ def load():
     L.wpcd_perm_apply_host.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp, vp, vp]
     L.wpcd_fp64_peak.argtypes = [vp, ctypes.POINTER(dbl)]
     L.wpcd_launch_count.restype = i64
+    L.wpcd_trace_enable.argtypes = [i32]
+    L.wpcd_trace_read.argtypes = [vp, vp]
     _lib = L
     return L
 
@@ -229,6 +232,18 @@ def wpcd_fp64_peak(stream=None):
     out = ctypes.c_double(0.0)
     _check(load().wpcd_fp64_peak(_stream_ptr(stream), ctypes.byref(out)))
     return out.value
+
+
+def wpcd_trace_enable(on):
+    _check(load().wpcd_trace_enable(1 if on else 0))
+
+
+def wpcd_trace_read():
+    """{stage: (milliseconds, launches)} accumulated since the last read."""
+    ms = np.zeros(len(TRACE_STAGES), np.float64)
+    n = np.zeros(len(TRACE_STAGES), np.int64)
+    _check(load().wpcd_trace_read(ms.ctypes.data, n.ctypes.data))
+    return {name: (float(ms[i]), int(n[i])) for i, name in enumerate(TRACE_STAGES)}
 
 
 def wpcd_launch_count():

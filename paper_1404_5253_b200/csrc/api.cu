@@ -29,6 +29,23 @@ static wpcd_status cuda_fail(cudaError_t err, const char* where)
     return fail(WPCD_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(err));
 }
 
+static bool g_trace_on = false;
+struct TraceRec { int stage; cudaEvent_t e0, e1; };
+static std::vector<TraceRec> g_trace;
+
+StageTimer::StageTimer(int stage_, cudaStream_t st_) : stage(stage_), st(st_)
+{
+    if (!g_trace_on) return;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, st);
+}
+StageTimer::~StageTimer()
+{
+    if (!e0) return;
+    cudaEventRecord(e1, st);
+    g_trace.push_back({stage, e0, e1});
+}
+
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base)
@@ -424,6 +441,31 @@ wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out)
     if (!flops_out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_fp64_peak: null pointer");
     cudaError_t err = run_fp64_peak(static_cast<cudaStream_t>(cuda_stream), flops_out);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_fp64_peak");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_trace_enable(int on)
+{
+    g_trace_on = on != 0;
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_trace_read(double* ms_out, int64_t* launches_out)
+{
+    if (!ms_out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_trace_read: null pointer");
+    for (int i = 0; i < WPCD_TRACE_STAGES; ++i) { ms_out[i] = 0.0; if (launches_out) launches_out[i] = 0; }
+    cudaError_t err = cudaSuccess;
+    for (auto& r : g_trace) {
+        float ms = 0.f;
+        cudaError_t e = cudaEventSynchronize(r.e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.e0, r.e1);
+        if (e != cudaSuccess) err = e;
+        ms_out[r.stage] += ms;
+        if (launches_out) launches_out[r.stage] += 1;
+        cudaEventDestroy(r.e0); cudaEventDestroy(r.e1);
+    }
+    g_trace.clear();
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_trace_read");
     return WPCD_OK;
 }
 

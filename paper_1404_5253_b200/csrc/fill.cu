@@ -80,6 +80,7 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     int lpe = (n_quad % 8 == 0) ? 8 : (n_quad % 4 == 0) ? 4 : (n_quad % 2 == 0) ? 2 : 1;
     int64_t threads = nnz_geo * lpe;
     int blocks = (int)((threads + 255) / 256);
+    StageTimer timer(WPCD_STAGE_FILL_SWAVE, st);
 #define WPCD_LAUNCH_SW(L) fill_swave_kernel<L><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
                                                                        ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
     switch (lpe) {

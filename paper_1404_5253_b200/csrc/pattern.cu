@@ -252,6 +252,7 @@ cudaError_t launch_geo_count(const wpcd_grid* g, int32_t* geo_counts_dev, cudaSt
     int n_geo = g->n_p * g->n_q;
     int blocks = (n_geo + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     size_t smem = (size_t)WARPS_PER_BLOCK * (2 * g->n_p + 2) * sizeof(int32_t);
+    StageTimer timer(WPCD_STAGE_GEO_COUNT, st);
     geo_pattern_kernel<false><<<blocks, WARPS_PER_BLOCK * 32, smem, st>>>(g->p_dev, g->q_dev, g->n_p, g->n_q, geo_counts_dev,
                                                                           nullptr, nullptr, nullptr, nullptr);
     ++g_launches;
@@ -264,6 +265,7 @@ cudaError_t launch_geo_index(const wpcd_grid* g, const int32_t* geo_row_ptr_dev,
     int n_geo = g->n_p * g->n_q;
     int blocks = (n_geo + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     size_t smem = (size_t)WARPS_PER_BLOCK * (2 * g->n_p + 2) * sizeof(int32_t);
+    StageTimer timer(WPCD_STAGE_GEO_INDEX, st);
     geo_pattern_kernel<true><<<blocks, WARPS_PER_BLOCK * 32, smem, st>>>(g->p_dev, g->q_dev, g->n_p, g->n_q, nullptr,
                                                                          geo_row_ptr_dev, geo_col, geo_row, geo_phi);
     ++g_launches;
@@ -274,6 +276,7 @@ cudaError_t launch_scan_rowptr(const wpcd_grid* g, const wpcd_channels* ch, int3
                                cudaStream_t st)
 {
     int n_geo = g->n_p * g->n_q;
+    StageTimer timer(WPCD_STAGE_SCAN, st);
     scan_geo_kernel<<<1, 1024, 0, st>>>(geo_row_ptr_dev, n_geo);
     ++g_launches;
     int64_t rows = (int64_t)ch->n_ch * n_geo;

@@ -55,6 +55,13 @@ namespace wpcd_detail {
 void set_error(const std::string& msg);
 extern int64_t g_launches;
 
+// RAII stage timer (wpcd_trace_enable): records an event pair around a kernel launch.
+struct StageTimer {
+    StageTimer(int stage, cudaStream_t st);
+    ~StageTimer();
+    int stage; cudaStream_t st; cudaEvent_t e0 = nullptr, e1 = nullptr;
+};
+
 // workspace layout for nnz_geo geometric entries (all 256-byte aligned)
 struct Workspace {
     int32_t* geo_col;    // [nnz_geo]

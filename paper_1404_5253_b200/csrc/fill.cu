@@ -94,10 +94,4 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     return cudaGetLastError();
 }
 
-cudaError_t launch_fill_coupled(const wpcd_grid*, const wpcd_channels*, int, const double*, const double*, int64_t,
-                                const Workspace&, const int64_t*, const int32_t*, int32_t*, double*, cudaStream_t)
-{
-    return cudaErrorNotSupported;
-}
-
 }  // namespace wpcd_detail

@@ -171,3 +171,99 @@ def test_fp64_peak_microbenchmark(wpcd):
     flops = wpcd.wpcd_fp64_peak()
     assert 5e12 < flops < 1e14
     assert wpcd.wpcd_launch_count() > 0
+
+
+# ----------------------------------------------------------------------------- coupled channels
+def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows):
+    """Full row_ptr + geometric pattern, and col_idx / values on the sampled geometric rows
+    (all channels), without materialising the oracle's full CSR (configs 3-5 sizes)."""
+    torch = _torch()
+    n = len(p) - 1
+    n_geo = n * n
+    grid = wpcd.wpcd_grid_create(p, p)
+    m = wpcd.build_perm(grid, gch, n_quad)
+    torch.cuda.synchronize()
+    geo_ptr, geo_col = operm.geo_pattern(p, p)
+    assert np.array_equal(m.geo_row_ptr.cpu().numpy().astype(np.int64), geo_ptr)
+    rp = operm.full_row_ptr(geo_ptr, tab, n, n)
+    assert np.array_equal(m.row_ptr.cpu().numpy(), rp)
+    assert m.nnz == rp[-1]
+    geo_rows = np.asarray(geo_rows)
+    cnt = geo_ptr[geo_rows + 1] - geo_ptr[geo_rows]
+    erow = np.repeat(geo_rows, cnt)
+    eidx = np.concatenate([np.arange(geo_ptr[r], geo_ptr[r + 1]) for r in geo_rows])
+    ecol = geo_col[eidx]
+    val, aval = operm.element_values(p, p, erow // n, erow % n, ecol // n, ecol % n, n_quad, tab)
+    pair_of = -np.ones((tab.n_ch, tab.n_ch), np.int64)
+    pair_of[tab.gamma, tab.gammap] = np.arange(tab.n_pairs)
+    vmax = np.abs(val).max()
+    off = np.concatenate([[0], np.cumsum(cnt)])
+    worst = 0.0
+    for g in range(tab.n_ch):
+        coupled = np.nonzero(tab.mask[g])[0]
+        if len(coupled) == 0:
+            continue
+        for ri, r in enumerate(geo_rows):
+            lo, hi = rp[g * n_geo + r], rp[g * n_geo + r + 1]
+            gc = geo_col[geo_ptr[r]:geo_ptr[r + 1]]
+            exp_cols = (coupled[:, None].astype(np.int64) * n_geo + gc[None, :]).reshape(-1)
+            assert hi - lo == len(exp_cols)
+            assert np.array_equal(m.col_idx[lo:hi].cpu().numpy(), exp_cols)
+            ev = val[off[ri]:off[ri + 1]][:, pair_of[g, coupled]].T.reshape(-1)
+            ea = aval[off[ri]:off[ri + 1]][:, pair_of[g, coupled]].T.reshape(-1)
+            gv = m.values[lo:hi].cpu().numpy()
+            tol = VALUE_RTOL * np.maximum(np.abs(ev), ea) + VALUE_FLOOR * vmax
+            err = np.abs(gv - ev)
+            worst = max(worst, float(np.max(err / tol)))
+            assert np.all(err <= tol), f"channel {g} geo row {r}: worst err/tol {np.max(err / tol)}"
+    return m, worst
+
+
+@pytest.mark.parametrize("two_J,parity,jmax,nb,nq", [(1, 1, 1, 6, 6), (1, -1, 2, 5, 4), (3, 1, 2, 4, 8), (5, -1, 3, 3, 10)])
+def test_coupled_small_full(wpcd, two_J, parity, jmax, nb, nq):
+    chs = och.enumerate_channels(two_J, parity, jmax)
+    tab = operm.PairTable(chs, och.g_table(chs, two_J, 1))
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=jmax)
+    p = wi.tan2_grid(nb, 1.0, 0.1, seed=31)
+    q = wi.tan2_grid(nb + 1, 0.8, 0.1, seed=32)
+    _compare_full(wpcd, p, q, nq, gch, tab)
+
+
+def test_coupled_from_table_matches_builtin(wpcd):
+    torch = _torch()
+    chs = och.enumerate_channels(1, 1, 1)
+    tab = operm.PairTable(chs, och.g_table(chs, 1, 1))
+    gch = wpcd.wpcd_channels_create_from_table(np.array([c[0] for c in chs]), tab.gamma, tab.gammap, tab.term_ptr,
+                                               tab.term_k, tab.term_l1, tab.term_l1p, tab.term_g)
+    p = wi.tan2_grid(5)
+    _compare_full(wpcd, p, p, 8, gch, tab)
+
+
+def test_cfg3_nd_half_plus_sampled(wpcd):
+    wl = wi.WORKLOADS["cfg3"]
+    (two_J, parity), = wl.jpis
+    p = wl.grid()
+    tab = _oracle_table(wl, two_J, parity)
+    assert tab.n_ch == 18
+    m, worst = _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, two_J, parity), tab,
+                                np.arange(7, wl.n_bins ** 2, 61))
+    assert m.rows == 18 * 100 * 100
+
+
+def test_cfg4_sampled(wpcd):
+    wl = wi.WORKLOADS["cfg4"]
+    p = wl.grid()
+    for (two_J, parity), stride in [((1, 1), 397), ((3, -1), 1499)]:
+        tab = _oracle_table(wl, two_J, parity)
+        _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, two_J, parity), tab,
+                         np.arange(11, wl.n_bins ** 2, stride))
+
+
+def test_cfg5_largest_sampled(wpcd):
+    # J = 7/2, parity -: the largest matrix of config 5 (62 channels, ~2.8e9 nonzeros, ~34 GB)
+    wl = wi.WORKLOADS["cfg5"]
+    p = wl.grid()
+    tab = _oracle_table(wl, 7, -1)
+    m, worst = _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, 7, -1), tab,
+                                np.arange(5, wl.n_bins ** 2, 2503))
+    assert m.nnz > 2_000_000_000

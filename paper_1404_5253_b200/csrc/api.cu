@@ -48,6 +48,69 @@ StageTimer::~StageTimer()
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// ---- buffer cache (see wpcd_internal.h)
+struct PoolEntry { void* ptr; size_t bytes; bool pinned; int device; };
+static std::mutex g_pool_mutex;
+static std::vector<PoolEntry> g_pool_free;
+static std::map<void*, PoolEntry> g_pool_live;
+static const size_t POOL_MAX_ENTRIES = 64;
+static const size_t POOL_MAX_BYTES = (size_t)1 << 30;
+
+static void pool_release(const PoolEntry& e)
+{
+    if (e.pinned) cudaFreeHost(e.ptr); else cudaFree(e.ptr);
+}
+
+void* pool_alloc(size_t bytes, bool pinned, cudaError_t* err)
+{
+    bytes = align256(std::max<size_t>(bytes, 1));
+    int dev = 0;
+    cudaGetDevice(&dev);
+    *err = cudaSuccess;
+    {
+        std::lock_guard<std::mutex> lock(g_pool_mutex);
+        size_t best = g_pool_free.size();
+        for (size_t k = 0; k < g_pool_free.size(); ++k) {
+            const PoolEntry& e = g_pool_free[k];
+            if (e.pinned != pinned || e.device != dev || e.bytes < bytes || e.bytes > 2 * bytes + 4096) continue;
+            if (best == g_pool_free.size() || e.bytes < g_pool_free[best].bytes) best = k;
+        }
+        if (best != g_pool_free.size()) {
+            PoolEntry e = g_pool_free[best];
+            g_pool_free.erase(g_pool_free.begin() + best);
+            g_pool_live[e.ptr] = e;
+            return e.ptr;
+        }
+    }
+    void* ptr = nullptr;
+    *err = pinned ? cudaMallocHost(&ptr, bytes) : cudaMalloc(&ptr, bytes);
+    if (*err != cudaSuccess) return nullptr;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    g_pool_live[ptr] = {ptr, bytes, pinned, dev};
+    return ptr;
+}
+
+void pool_free(void* ptr)
+{
+    if (!ptr) return;
+    std::vector<PoolEntry> drop;
+    {
+        std::lock_guard<std::mutex> lock(g_pool_mutex);
+        auto it = g_pool_live.find(ptr);
+        if (it == g_pool_live.end()) return;
+        g_pool_free.push_back(it->second);
+        g_pool_live.erase(it);
+        size_t total = 0;
+        for (auto& e : g_pool_free) total += e.bytes;
+        while (!g_pool_free.empty() && (g_pool_free.size() > POOL_MAX_ENTRIES || total > POOL_MAX_BYTES)) {
+            total -= g_pool_free.front().bytes;
+            drop.push_back(g_pool_free.front());
+            g_pool_free.erase(g_pool_free.begin());
+        }
+    }
+    for (auto& e : drop) pool_release(e);
+}
+
 Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base)
 {
     Workspace ws{};
@@ -190,11 +253,24 @@ wpcd_status wpcd_grid_create(const double* p_nodes, int n_p, const double* q_nod
     g->n_p = n_p; g->n_q = n_q;
     g->p.assign(p_nodes, p_nodes + n_p + 1);
     g->q.assign(q_nodes, q_nodes + n_q + 1);
-    cudaError_t err = cudaMalloc(reinterpret_cast<void**>(&g->p_dev), sizeof(double) * (n_p + 1));
-    if (err == cudaSuccess) err = cudaMalloc(reinterpret_cast<void**>(&g->q_dev), sizeof(double) * (n_q + 1));
-    if (err == cudaSuccess) err = cudaMemcpy(g->p_dev, p_nodes, sizeof(double) * (n_p + 1), cudaMemcpyHostToDevice);
+    // one device block: p | q | ctrl | stage_off | stage_len (256-byte aligned pieces); one pinned block
+    const size_t n_geo = (size_t)n_p * n_q;
+    const size_t o_q = align256(sizeof(double) * (n_p + 1)), o_ctrl = o_q + align256(sizeof(double) * (n_q + 1));
+    const size_t o_off = o_ctrl + 256, o_len = o_off + align256(sizeof(int32_t) * n_geo);
+    const size_t total = o_len + align256(sizeof(int32_t) * n_geo);
+    cudaError_t err = cudaSuccess;
+    g->block_dev = static_cast<char*>(pool_alloc(total, false, &err));
+    if (err == cudaSuccess) g->ctrl_pinned = static_cast<int32_t*>(pool_alloc(256, true, &err));
+    if (err == cudaSuccess) {
+        g->p_dev = reinterpret_cast<double*>(g->block_dev);
+        g->q_dev = reinterpret_cast<double*>(g->block_dev + o_q);
+        g->ctrl = reinterpret_cast<int32_t*>(g->block_dev + o_ctrl);
+        g->stage_off = reinterpret_cast<int32_t*>(g->block_dev + o_off);
+        g->stage_len = reinterpret_cast<int32_t*>(g->block_dev + o_len);
+        err = cudaMemcpy(g->p_dev, p_nodes, sizeof(double) * (n_p + 1), cudaMemcpyHostToDevice);
+        if (err == cudaSuccess) err = cudaMemset(g->ctrl, 0, 256);
+    }
     if (err == cudaSuccess) err = cudaMemcpy(g->q_dev, q_nodes, sizeof(double) * (n_q + 1), cudaMemcpyHostToDevice);
-    if (err == cudaSuccess) err = cudaMallocHost(reinterpret_cast<void**>(&g->nnz_geo_pinned), sizeof(int32_t));
     if (err != cudaSuccess) { wpcd_grid_destroy(g); return cuda_fail(err, "wpcd_grid_create"); }
     *out = g;
     return WPCD_OK;
@@ -203,8 +279,8 @@ wpcd_status wpcd_grid_create(const double* p_nodes, int n_p, const double* q_nod
 void wpcd_grid_destroy(wpcd_grid* g)
 {
     if (!g) return;
-    cudaFree(g->p_dev); cudaFree(g->q_dev);
-    if (g->nnz_geo_pinned) cudaFreeHost(g->nnz_geo_pinned);
+    if (g->select_ready) cudaDeviceSynchronize();   // scratch goes back to the cache: no kernel may still use it
+    pool_free(g->block_dev); pool_free(g->stage_col); pool_free(g->stage_ext); pool_free(g->ctrl_pinned);
     delete g;
 }
 
@@ -318,25 +394,48 @@ wpcd_status wpcd_channels_get_table(const wpcd_channels* c, int32_t* pair_gamma,
 int64_t wpcd_rows(const wpcd_grid* g, const wpcd_channels* c) { return (g && c) ? (int64_t)c->n_ch * g->n_p * g->n_q : 0; }
 int64_t wpcd_geo_rows(const wpcd_grid* g) { return g ? (int64_t)g->n_p * g->n_q : 0; }
 
-wpcd_status wpcd_perm_count(const wpcd_grid* g, const wpcd_channels* c, int n_quad, void* cuda_stream, int64_t* row_ptr_dev,
+// Selection pass on grid g: predicate, per-row counts, staged verdicts, scan, and (when c is
+// given) the row pointer of the full matrix.  Synchronises the stream (the caller needs nnz_geo);
+// repeats the pass with a larger staging area if it overflowed.
+static wpcd_status run_selection(wpcd_grid* g, const wpcd_channels* c, int32_t* geo_row_ptr_dev, int64_t* row_ptr_dev,
+                                 cudaStream_t st, const char* who)
+{
+    const int n_geo = g->n_p * g->n_q;
+    int64_t want = g->stage_cap > 0 ? g->stage_cap : std::max<int64_t>(1024, (int64_t)48 * n_geo);
+    for (int attempt = 0; attempt < 3; ++attempt) {
+        cudaError_t err = ensure_stage(g, want);
+        if (err != cudaSuccess) return cuda_fail(err, who);
+        g->stage_valid = false;
+        err = launch_geo_select(g, geo_row_ptr_dev, st);
+        if (err == cudaSuccess && c) err = launch_rowptr(g, c, geo_row_ptr_dev, row_ptr_dev, st);
+        if (err == cudaSuccess) err = cudaMemcpyAsync(g->ctrl_pinned, g->ctrl + 4, sizeof(int32_t) * 4, cudaMemcpyDeviceToHost, st);
+        if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+        if (err != cudaSuccess) return cuda_fail(err, who);
+        if (g->ctrl_pinned[1] == 0) {
+            g->stage_valid = true;
+            g->stage_nnz_geo = g->ctrl_pinned[2];
+            return WPCD_OK;
+        }
+        if (g->ctrl_pinned[0] < 0) return fail(WPCD_ERR_OVERFLOW, std::string(who) + ": more than 2^31 candidate cell pairs");
+        want = (int64_t)g->ctrl_pinned[0] + (int64_t)g->ctrl_pinned[0] / 8 + 1024;
+    }
+    return fail(WPCD_ERR_ALLOC, std::string(who) + ": staging area kept overflowing");
+}
+
+wpcd_status wpcd_perm_count(const wpcd_grid* g_in, const wpcd_channels* c, int n_quad, void* cuda_stream, int64_t* row_ptr_dev,
                             int32_t* geo_row_ptr_dev, int64_t* nnz_out, int64_t* nnz_geo_out)
 {
-    if (!g || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
+    if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_count: null pointer");
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_count: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_count: channel tables are not on a device (no CUDA device?)");
+    wpcd_grid* g = const_cast<wpcd_grid*>(g_in);   // the staging scratch inside the handle is mutable state
     int64_t rows = wpcd_rows(g, c);
     if (rows > (int64_t)INT32_MAX) return fail(WPCD_ERR_OVERFLOW, "wpcd_perm_count: column index would not fit int32");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    int n_geo = g->n_p * g->n_q;
-    cudaError_t err = launch_geo_count(g, geo_row_ptr_dev, st);
-    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_count(count)");
-    err = launch_scan_rowptr(g, c, geo_row_ptr_dev, row_ptr_dev, st);
-    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_count(scan)");
-    err = cudaMemcpyAsync(g->nnz_geo_pinned, geo_row_ptr_dev + n_geo, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
-    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
-    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_count(sync)");
-    int64_t nnz_geo = *g->nnz_geo_pinned;
+    wpcd_status s = run_selection(g, c, geo_row_ptr_dev, row_ptr_dev, st, "wpcd_perm_count");
+    if (s != WPCD_OK) return s;
+    int64_t nnz_geo = g->stage_nnz_geo;
     *nnz_geo_out = nnz_geo;
     *nnz_out = nnz_geo * c->total_coupled;
     {
@@ -352,34 +451,33 @@ size_t wpcd_perm_workspace_bytes(const wpcd_channels* c, int64_t nnz_geo)
     return carve_workspace(c, nnz_geo, nullptr).bytes;
 }
 
-wpcd_status wpcd_perm_build(const wpcd_grid* g, const wpcd_channels* c, int n_quad, void* cuda_stream, const int64_t* row_ptr_dev,
+wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n_quad, void* cuda_stream, const int64_t* row_ptr_dev,
                             const int32_t* geo_row_ptr_dev, void* workspace_dev, size_t workspace_bytes, int32_t* col_idx_dev,
                             double* values_dev)
 {
-    if (!g || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
+    if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_build: channel tables are not on a device (no CUDA device?)");
+    wpcd_grid* g = const_cast<wpcd_grid*>(g_in);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    int64_t nnz_geo = -1;
-    {
-        std::lock_guard<std::mutex> lock(g_hint_mutex);
-        auto it = g_nnz_hint.find(row_ptr_dev);
-        if (it != g_nnz_hint.end() && it->second.first == wpcd_rows(g, c) && c->total_coupled > 0) nnz_geo = it->second.second / c->total_coupled;
+    if (!g->stage_valid) {
+        // no selection pass has run on this handle (geo_row_ptr came from elsewhere): redo it into
+        // a scratch copy of the row pointer so that the caller's array stays untouched
+        int32_t* tmp = nullptr;
+        const int n_geo = g->n_p * g->n_q;
+        cudaError_t err = cudaMalloc(reinterpret_cast<void**>(&tmp), sizeof(int32_t) * (n_geo + 1));
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(selection scratch)");
+        wpcd_status s = run_selection(g, nullptr, tmp, nullptr, st, "wpcd_perm_build");
+        cudaFree(tmp);
+        if (s != WPCD_OK) return s;
     }
-    if (nnz_geo < 0 || c->total_coupled == 0) {   // row_ptr not produced by this process' wpcd_perm_count: read the count back
-        int32_t v = 0;
-        cudaError_t err = cudaMemcpyAsync(g->nnz_geo_pinned, geo_row_ptr_dev + g->n_p * g->n_q, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
-        if (err == cudaSuccess) err = cudaStreamSynchronize(st);
-        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(read nnz_geo)");
-        v = *g->nnz_geo_pinned;
-        nnz_geo = v;
-    }
+    const int64_t nnz_geo = g->stage_nnz_geo;
     if (nnz_geo == 0 || c->total_coupled == 0) return WPCD_OK;
     if (!workspace_dev || !col_idx_dev || !values_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null output or workspace");
     if ((reinterpret_cast<uintptr_t>(workspace_dev) & 255) != 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: workspace must be 256-byte aligned");
     Workspace ws = carve_workspace(c, nnz_geo, workspace_dev);
     if (workspace_bytes < ws.bytes) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: workspace too small");
-    cudaError_t err = launch_geo_index(g, geo_row_ptr_dev, ws.geo_col, ws.geo_row, ws.geo_phi, st);
+    cudaError_t err = launch_geo_gather(g, geo_row_ptr_dev, ws.geo_col, ws.geo_row, ws.geo_phi, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(index)");
     double xi[WPCD_MAX_QUAD], w[WPCD_MAX_QUAD];
     wpcd_host::gauss_legendre(n_quad, xi, w);

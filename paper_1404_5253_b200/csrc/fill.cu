@@ -21,9 +21,11 @@ __constant__ double c_xi[WPCD_MAX_QUAD];
 __constant__ double c_w[WPCD_MAX_QUAD];
 
 // ------------------------------------------------------------------ s-wave
-template <int LPE>
+// NQ > 0: rule order fixed at compile time (loops unrolled, nodes and weights become immediates
+// of the constant bank); NQ = 0: any order.
+template <int LPE, int NQ>
 __global__ void __launch_bounds__(256)
-fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n, double g0,
+fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n_rt, double g0,
                   int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                   const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
@@ -31,6 +33,7 @@ fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, in
     const int64_t e = t / LPE;
     const int sub = (int)(t - e * LPE);
     const bool valid = e < nnz_geo;
+    const int n = NQ > 0 ? NQ : n_rt;
     double acc = 0.0;
     double norm = 0.0;
     int col = 0;
@@ -39,18 +42,23 @@ fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, in
         const int row = geo_row[e];
         const double2 ph = geo_phi[e];
         const Cell z = load_cell(p, q, n_q, row, col);
+        const CellSq zs = square_cell(z);
         norm = cell_norm(z);
         const double half_phi = 0.5 * (ph.y - ph.x), mid_phi = 0.5 * (ph.x + ph.y);
         if (ph.x < ph.y) {
+#pragma unroll 1
             for (int m = sub; m < n; m += LPE) {
-                PhiNode s;
-                if (!phi_node(z, mid_phi + half_phi * c_xi[m], s)) continue;
+                PhiNodeSq s;
+                if (!phi_node_sq(z, zs, mid_phi + half_phi * c_xi[m], s)) continue;
                 const double half_u = 0.5 * (s.u_hi - s.u_lo), mid_u = 0.5 * (s.u_lo + s.u_hi);
                 double inner = 0.0;
+#pragma unroll
                 for (int r = 0; r < n; ++r) {
                     const double u = mid_u + half_u * c_xi[r];
-                    const double iz1 = rsqrt(s.b1 + s.beta * u), iz2 = rsqrt(s.b2 + s.beta * u);
-                    inner += c_w[r] * F_A14(z, s, iz1, iz2) * iz1 * iz2;
+                    const double z1 = s.b1 + s.beta * u, z2 = s.b2 + s.beta * u;    // zeta1^2, zeta2^2 (A11)
+                    const double t = rsqrt(z1 * z2);                                // 1/(zeta1 zeta2)
+                    const double t2 = t * t;
+                    inner += c_w[r] * twoF_A14_sq(zs, s, t2 * z2, t2 * z1) * t;
                 }
                 acc += half_phi * c_w[m] * half_u * s.beta * inner;    // cos*sin = beta
             }
@@ -59,7 +67,7 @@ fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, in
 #pragma unroll
     for (int o = LPE / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (valid && sub == 0) {
-        values[e] = g0 * norm * acc;
+        values[e] = 0.5 * g0 * norm * acc;    // the 1/2 of (A14)
         col_idx[e] = col;
     }
 }
@@ -81,13 +89,15 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     int64_t threads = nnz_geo * lpe;
     int blocks = (int)((threads + 255) / 256);
     StageTimer timer(WPCD_STAGE_FILL_SWAVE, st);
-#define WPCD_LAUNCH_SW(L) fill_swave_kernel<L><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
-                                                                       ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
-    switch (lpe) {
-    case 8: WPCD_LAUNCH_SW(8); break;
-    case 4: WPCD_LAUNCH_SW(4); break;
-    case 2: WPCD_LAUNCH_SW(2); break;
-    default: WPCD_LAUNCH_SW(1); break;
+#define WPCD_LAUNCH_SW(L, Q) fill_swave_kernel<L, Q><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
+                                                                            ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
+    if (n_quad == 8) WPCD_LAUNCH_SW(8, 8);
+    else if (n_quad == 10) WPCD_LAUNCH_SW(2, 10);
+    else switch (lpe) {
+    case 8: WPCD_LAUNCH_SW(8, 0); break;
+    case 4: WPCD_LAUNCH_SW(4, 0); break;
+    case 2: WPCD_LAUNCH_SW(2, 0); break;
+    default: WPCD_LAUNCH_SW(1, 0); break;
     }
 #undef WPCD_LAUNCH_SW
     ++g_launches;

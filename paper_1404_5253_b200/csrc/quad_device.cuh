@@ -62,6 +62,82 @@ __device__ __forceinline__ double F_A14(const Cell& z, const PhiNode& s, double 
     return Qmax > Qmin ? 0.5 * (Qmax - Qmin) * (Qmax + Qmin) : 0.0;
 }
 
+// ---- the same rule in squared variables (no square roots, one reciprocal per limit).
+// Q-limits enter (A14) only through their squares: F = 1/2 (min Q^2 - max Q^2), and squaring is
+// monotone on Q >= 0, so F needs 1/zeta^2 only; u-limits need (L/U_q)^2 = L^2 / U_q^2.
+struct CellSq { double a2, b2, c2, d2, L1s, U1s, L2s, U2s; };
+
+__device__ __forceinline__ CellSq square_cell(const Cell& z)
+{
+    CellSq s;
+    s.a2 = z.a * z.a; s.b2 = z.b * z.b; s.c2 = z.c * z.c; s.d2 = z.d * z.d;
+    s.L1s = z.L1 * z.L1; s.U1s = z.U1 * z.U1; s.L2s = z.L2 * z.L2; s.U2s = z.U2 * z.U2;
+    return s;
+}
+
+struct PhiNodeSq {
+    double C, S;
+    double Lq2, Uq2;      // squares of the Q-limits of (A12)
+    double b1, b2, beta;
+    double u_lo, u_hi;
+};
+
+__device__ __forceinline__ bool phi_node_sq(const Cell& z, const CellSq& zs, double phi, PhiNodeSq& s)
+{
+    sincos(phi, &s.S, &s.C);
+    const double C2 = s.C * s.C, S2 = s.S * s.S;
+    s.beta = s.C * s.S;
+    const double ib2 = __drcp_rn(C2 * S2);          // 1/beta^2  ->  1/C^2 = S^2 ib2, 1/S^2 = C^2 ib2, 1/beta = beta ib2
+    const double iC2 = S2 * ib2, iS2 = C2 * ib2, ibeta = s.beta * ib2;
+    s.Lq2 = fmax(zs.a2 * iC2, zs.c2 * iS2);
+    s.Uq2 = fmin(zs.b2 * iC2, zs.d2 * iS2);
+    if (!(s.Lq2 < s.Uq2)) return false;
+    {
+        const double d1 = s.C - 0.5 * s.S, d2 = 0.5 * s.C - s.S;
+        s.b1 = d1 * d1; s.b2 = d2 * d2;
+    }
+    double u_lo = 0.0, u_hi = 2.0;
+    if (z.L1 > 0.0 || z.L2 > 0.0) {
+        const double iUq2 = __drcp_rn(s.Uq2);
+        if (z.L1 > 0.0) u_lo = fmax(u_lo, (zs.L1s * iUq2 - s.b1) * ibeta);
+        if (z.L2 > 0.0) u_lo = fmax(u_lo, (zs.L2s * iUq2 - s.b2) * ibeta);
+    }
+    if (s.Lq2 > 0.0) {
+        const double iLq2 = __drcp_rn(s.Lq2);
+        u_hi = fmin(u_hi, (zs.U1s * iLq2 - s.b1) * ibeta);
+        u_hi = fmin(u_hi, (zs.U2s * iLq2 - s.b2) * ibeta);
+    }
+    {   // L1/zeta1 < U2/zeta2  <=>  beta u (L1^2-U2^2) < U2^2 b1 - L1^2 b2; sign of D on unfused products
+        const double D = __dsub_rn(__dmul_rn(z.L1, z.L1), __dmul_rn(z.U2, z.U2));
+        const double R = zs.U2s * s.b1 - zs.L1s * s.b2;
+        if (D > 0.0) u_hi = fmin(u_hi, R * ibeta / D);
+        else if (D < 0.0) u_lo = fmax(u_lo, R * ibeta / D);
+        else if (!(0.0 < R)) return false;
+    }
+    {   // L2/zeta2 < U1/zeta1  <=>  beta u (L2^2-U1^2) < U1^2 b2 - L2^2 b1
+        const double D = __dsub_rn(__dmul_rn(z.L2, z.L2), __dmul_rn(z.U1, z.U1));
+        const double R = zs.U1s * s.b2 - zs.L2s * s.b1;
+        if (D > 0.0) u_hi = fmin(u_hi, R * ibeta / D);
+        else if (D < 0.0) u_lo = fmax(u_lo, R * ibeta / D);
+        else if (!(0.0 < R)) return false;
+    }
+    s.u_lo = u_lo; s.u_hi = u_hi;
+    return u_lo < u_hi;
+}
+
+// 2 F of (A14) from r1 = 1/zeta1^2, r2 = 1/zeta2^2 (clamped at 0, R5)
+__device__ __forceinline__ double twoF_A14_sq(const CellSq& zs, const PhiNodeSq& s, double r1, double r2)
+{
+    // plain compare-and-select (all operands are finite here; fmin/fmax would add NaN handling)
+    const double pU1 = zs.U1s * r1, pU2 = zs.U2s * r2, pL1 = zs.L1s * r1, pL2 = zs.L2s * r2;
+    double Qmax2 = pU1 < s.Uq2 ? pU1 : s.Uq2;
+    Qmax2 = pU2 < Qmax2 ? pU2 : Qmax2;
+    double Qmin2 = pL1 > s.Lq2 ? pL1 : s.Lq2;
+    Qmin2 = pL2 > Qmin2 ? pL2 : Qmin2;
+    const double F2 = Qmax2 - Qmin2;
+    return F2 > 0.0 ? F2 : 0.0;
+}
+
 __device__ __forceinline__ Cell load_cell(const double* __restrict__ p, const double* __restrict__ q, int n_q, int row, int col)
 {
     int i = row / n_q, j = row - i * n_q;

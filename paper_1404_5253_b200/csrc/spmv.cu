@@ -3,7 +3,11 @@
 // HBM-bound: 12 B per nonzero streamed once, x gathered through L2.
 // LPR lanes cooperate on one row (coalesced col/value loads), chosen from the mean row
 // length; up to 4 right-hand sides share one pass over the matrix.
+#include <stdlib.h>
+
 #include "wpcd_internal.h"
+
+namespace wpcd_detail { bool use_pdl(); }
 
 namespace {
 
@@ -12,6 +16,10 @@ __global__ void __launch_bounds__(256)
 spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
             const double* __restrict__ values, const double* __restrict__ x, double* __restrict__ y, int64_t ldx)
 {
+    // Programmatic dependent launch: this grid may be scheduled while the previous kernel of the
+    // stream drains; nothing is read or written before the wait, so the usual stream order holds.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = t / LPR;
     const int sub = (int)(t - row * LPR);
@@ -20,11 +28,24 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
     for (int v = 0; v < NV; ++v) acc[v] = 0.0;
     if (row < rows) {
         const int64_t beg = row_ptr[row], end = row_ptr[row + 1];
-        for (int64_t e = beg + sub; e < end; e += LPR) {
-            const double a = values[e];
-            const int c = col_idx[e];
+        // batches of UNR entries per lane: all column/value loads of a batch are issued before the
+        // gathers of x, so a long row costs ~2 memory latencies per batch instead of per entry
+        constexpr int UNR = 8 / NV > 1 ? 8 / NV : 2;
+        for (int64_t e0 = beg + sub; e0 < end; e0 += (int64_t)UNR * LPR) {
+            double a[UNR];
+            int c[UNR];
 #pragma unroll
-            for (int v = 0; v < NV; ++v) acc[v] = fma(a, __ldg(x + v * ldx + c), acc[v]);
+            for (int k = 0; k < UNR; ++k) {
+                const int64_t e = e0 + (int64_t)k * LPR;
+                const bool in = e < end;
+                a[k] = in ? values[e] : 0.0;
+                c[k] = in ? col_idx[e] : 0;
+            }
+#pragma unroll
+            for (int k = 0; k < UNR; ++k) {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], __ldg(x + v * ldx + c[k]), acc[v]);
+            }
         }
     }
 #pragma unroll
@@ -44,18 +65,33 @@ cudaError_t launch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx,
 {
     int64_t threads = rows * LPR;
     int64_t blocks = (threads + 255) / 256;
-    spmv_kernel<LPR, NV><<<(unsigned)blocks, 256, 0, st>>>(rows, row_ptr, col_idx, values, x, y, rows);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = wpcd_detail::use_pdl() ? 1 : 0;
     ++wpcd_detail::g_launches;
-    return cudaGetLastError();
+    return cudaLaunchKernelEx(&cfg, spmv_kernel<LPR, NV>, rows, row_ptr, col_idx, values, x, y, rows);
 }
 
 template <int NV>
 cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
                      double* y, double mean_row, cudaStream_t st)
 {
-    if (mean_row <= 6.0) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (mean_row <= 16.0) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (mean_row <= 48.0) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    static const int forced = [] { const char* e = getenv("WPCD_SPMV_LPR"); return e ? atoi(e) : 0; }();   // tuning knob
+    if (forced == 4) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (forced == 8) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (forced == 16) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (forced == 32) return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    // Row lengths of P0 are very skewed (median 11, max ~400 per coupled channel at N = 100), and a small
+    // matrix is latency-bound by its longest row: prefer wide rows early.
+    if (mean_row <= 3.0) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (mean_row <= 6.0) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    if (mean_row <= 12.0) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
     return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
 }
 
@@ -75,6 +111,12 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, 
 }  // namespace
 
 namespace wpcd_detail {
+
+bool use_pdl()
+{
+    static const bool on = [] { const char* e = getenv("WPCD_NO_PDL"); return !(e && e[0] == '1'); }();
+    return on;
+}
 
 cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                         const double* x, double* y, int n_vec, double mean_row, cudaStream_t st)

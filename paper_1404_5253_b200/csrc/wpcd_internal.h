@@ -11,9 +11,21 @@
 struct wpcd_grid {
     int n_p = 0, n_q = 0;
     std::vector<double> p, q;   // host copies
+    char* block_dev = nullptr;  // one device allocation holding p, q, ctrl, stage_off, stage_len
     double* p_dev = nullptr;    // [n_p+1]
     double* q_dev = nullptr;    // [n_q+1]
-    int32_t* nnz_geo_pinned = nullptr;  // pinned host word for the count read-back
+    // Staged result of the last selection pass on this grid (scratch owned by the handle,
+    // written by wpcd_perm_count, consumed by wpcd_perm_build): one slot per box-test candidate.
+    int32_t* stage_col = nullptr;       // [stage_cap]  column index, or -1 for a rejected candidate
+    double4* stage_ext = nullptr;       // [stage_cap]  vertices of smallest / largest polar angle of Pi (survivors)
+    int32_t* stage_off = nullptr;       // [n_p*n_q]    first slot of a geometric row
+    int32_t* stage_len = nullptr;       // [n_p*n_q]    number of candidates of a geometric row
+    int32_t* ctrl = nullptr;            // [4] device: slot cursor, overflow flag, nnz_geo
+    int32_t* ctrl_pinned = nullptr;     // [4] pinned host copy
+    int64_t stage_cap = 0;
+    bool stage_valid = false;
+    bool select_ready = false;          // kernel attributes set
+    int64_t stage_nnz_geo = 0;
 };
 
 // monomial mu = (k, A, l, l'):  P_k(x) cos^{A+1} sin^{l+l'-A+1} / (zeta1^{l'+1} zeta2^{l+1})
@@ -62,6 +74,11 @@ struct StageTimer {
     int stage; cudaStream_t st; cudaEvent_t e0 = nullptr, e1 = nullptr;
 };
 
+// Small process-wide cache of device / pinned buffers used for the scratch inside the handles, so
+// that creating and destroying handles in a loop does not pay cudaMalloc / cudaFree every time.
+void* pool_alloc(size_t bytes, bool pinned, cudaError_t* err);
+void pool_free(void* ptr);
+
 // workspace layout for nnz_geo geometric entries (all 256-byte aligned)
 struct Workspace {
     int32_t* geo_col;    // [nnz_geo]
@@ -74,11 +91,12 @@ struct Workspace {
 Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base);
 
 // pattern.cu  (compiled with -fmad=false: the predicate is an IEEE contract)
-cudaError_t launch_geo_count(const wpcd_grid* g, int32_t* geo_counts_dev, cudaStream_t st);
-cudaError_t launch_geo_index(const wpcd_grid* g, const int32_t* geo_row_ptr_dev, int32_t* geo_col, int32_t* geo_row,
-                             double2* geo_phi, cudaStream_t st);
-cudaError_t launch_scan_rowptr(const wpcd_grid* g, const wpcd_channels* ch, int32_t* geo_row_ptr_dev /* in: counts, out: ptr */,
-                               int64_t* row_ptr_dev, cudaStream_t st);
+cudaError_t ensure_stage(wpcd_grid* g, int64_t want_cap);
+cudaError_t launch_geo_select(wpcd_grid* g, int32_t* geo_row_ptr_dev /* out: ptr */, cudaStream_t st);
+cudaError_t launch_rowptr(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr_dev, int64_t* row_ptr_dev,
+                          cudaStream_t st);
+cudaError_t launch_geo_gather(const wpcd_grid* g, const int32_t* geo_row_ptr_dev, int32_t* geo_col, int32_t* geo_row,
+                              double2* geo_phi, cudaStream_t st);
 
 // fill.cu
 cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, const double* xi, const double* w,

@@ -6,6 +6,7 @@
 #include <map>
 #include <mutex>
 #include <new>
+#include <set>
 #include <tuple>
 
 #include "wigner_host.h"
@@ -122,9 +123,11 @@ Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base)
     ws.geo_phi = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)nnz_geo));
     ws.chunk = 0;
     ws.moments = nullptr;
+    ws.slab_tab = nullptr;
     if (ch && !ch->swave_single) {
-        // moment block: at most ~512 MiB, a multiple of 32 elements
-        int64_t chunk = (int64_t)((512ull << 20) / (sizeof(double) * (size_t)std::max(ch->n_mu, 1)));
+        ws.slab_tab = take(16 * std::max<size_t>(ch->slabs.size(), 1));
+        // moment block: at most ~256 MiB, a multiple of 32 elements
+        int64_t chunk = (int64_t)((256ull << 20) / (sizeof(double) * (size_t)std::max(ch->n_mu, 1)));
         chunk = std::max<int64_t>(32, (chunk / 32) * 32);
         chunk = std::min<int64_t>(chunk, ((nnz_geo + 31) / 32) * 32);
         chunk = std::max<int64_t>(chunk, 32);
@@ -140,8 +143,8 @@ static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_p
 
 static void free_channels_device(wpcd_channels* c)
 {
-    cudaFree(c->ncoupled_dev); cudaFree(c->chan_off_dev); cudaFree(c->pair_gamma_dev); cudaFree(c->pair_gammap_dev);
-    cudaFree(c->pair_ci_dev); cudaFree(c->mu_dev); cudaFree(c->mterm_ptr_dev); cudaFree(c->mterm_mu_dev); cudaFree(c->mterm_g_dev);
+    cudaFree(c->ncoupled_dev); cudaFree(c->chan_off_dev); cudaFree(c->ll_pack_dev); cudaFree(c->trip_pack_dev);
+    cudaFree(c->mu_pack_dev); cudaFree(c->slab_blob_dev);
 }
 
 template <class T>
@@ -168,42 +171,23 @@ static wpcd_status finalize_channels(wpcd_channels* c)
             return fail(WPCD_ERR_INVALID_ARG, "pairs must be sorted ascending by (gamma, gamma') without repeats");
         if (c->term_ptr[pidx + 1] < c->term_ptr[pidx]) return fail(WPCD_ERR_INVALID_ARG, "term_ptr not monotone");
     }
-    // merged monomials mu = (k, A, l, l'), A = l1 + l1'
-    std::map<std::tuple<int, int, int, int>, int> mu_index;   // key (l, l', A, k)
+    // ---- merged coefficients per pair, monomial (A, k) = (l1 + l1', k)
     c->k_max = 0; c->l_max = 0;
+    typedef std::pair<int, int> Mono;                           // (A, k)
+    std::vector<std::map<Mono, double>> pair_coef(c->n_pairs);
+    std::map<std::pair<int, int>, std::set<Mono>> ll_mono;      // (l, l') -> monomials used by any pair
     for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
         int l = c->channel_l[c->pair_gamma[pidx]], lp = c->channel_l[c->pair_gammap[pidx]];
         c->l_max = std::max(c->l_max, std::max(l, lp));
-        std::map<std::tuple<int, int, int, int>, double> acc;
         for (int64_t t = c->term_ptr[pidx]; t < c->term_ptr[pidx + 1]; ++t) {
             int k = c->term_k[t], l1 = c->term_l1[t], l1p = c->term_l1p[t];
             if (k < 0 || k > WPCD_MAX_K) return fail(WPCD_ERR_UNSUPPORTED, "Legendre order k beyond WPCD_MAX_K");
             if (l1 < 0 || l1 > l || l1p < 0 || l1p > lp) return fail(WPCD_ERR_INVALID_ARG, "l1 / l1' out of range");
             c->k_max = std::max(c->k_max, k);
-            acc[std::make_tuple(l, lp, l1 + l1p, k)] += c->term_g[t];
+            pair_coef[pidx][Mono(l1 + l1p, k)] += c->term_g[t];
         }
-        for (auto& kv : acc) mu_index.emplace(kv.first, 0);   // indices assigned once the set is complete
+        for (auto& kv : pair_coef[pidx]) ll_mono[std::make_pair(l, lp)].insert(kv.first);
     }
-    int idx = 0;
-    c->mu.clear();
-    for (auto& kv : mu_index) {
-        kv.second = idx++;
-        c->mu.push_back({(int16_t)std::get<3>(kv.first), (int16_t)std::get<2>(kv.first), (int16_t)std::get<0>(kv.first),
-                         (int16_t)std::get<1>(kv.first)});
-    }
-    c->n_mu = idx;
-    c->mterm_ptr.assign(c->n_pairs + 1, 0);
-    c->mterm_mu.clear(); c->mterm_g.clear();
-    for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
-        int l = c->channel_l[c->pair_gamma[pidx]], lp = c->channel_l[c->pair_gammap[pidx]];
-        std::map<std::tuple<int, int, int, int>, double> acc;
-        for (int64_t t = c->term_ptr[pidx]; t < c->term_ptr[pidx + 1]; ++t)
-            acc[std::make_tuple(l, lp, c->term_l1[t] + c->term_l1p[t], c->term_k[t])] += c->term_g[t];
-        for (auto& kv : acc) { c->mterm_mu.push_back(mu_index[kv.first]); c->mterm_g.push_back(kv.second); }
-        c->mterm_ptr[pidx + 1] = (int32_t)c->mterm_mu.size();
-    }
-    c->swave_single = (c->n_ch == 1 && c->n_pairs == 1 && c->n_terms == 1 && c->channel_l[0] == 0 && c->term_k[0] == 0);
-    if (c->swave_single) c->g0 = c->term_g[0];
     // coupling structure
     c->ncoupled.assign(c->n_ch, 0);
     std::vector<int32_t> pair_ci(c->n_pairs);
@@ -211,6 +195,126 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     std::vector<int64_t> chan_off(c->n_ch + 1, 0);
     for (int a = 0; a < c->n_ch; ++a) chan_off[a + 1] = chan_off[a] + c->ncoupled[a];
     c->total_coupled = chan_off[c->n_ch];
+    // ---- moment row: one block per (l, l') with its distinct monomials; (l,l') list; (k,l,l') triples
+    std::map<std::pair<int, int>, int> ll_index;
+    c->ll_pack.clear();
+    for (auto& kv : ll_mono) { ll_index[kv.first] = (int)c->ll_pack.size(); c->ll_pack.push_back(kv.first.first | (kv.first.second << 8)); }
+    c->n_ll = (int)c->ll_pack.size();
+    std::map<std::pair<int, int>, int> trip_index;   // (ll, k), sorted by (ll, k)
+    for (auto& kv : ll_mono)
+        for (auto& ak : kv.second) trip_index.emplace(std::make_pair(ll_index[kv.first], ak.second), 0);
+    c->trip_pack.clear();
+    for (auto& kv : trip_index) { kv.second = (int)c->trip_pack.size(); c->trip_pack.push_back(kv.first.second | (kv.first.first << 8)); }
+    c->n_trip = (int)c->trip_pack.size();
+    if (c->n_trip >= 65536) return fail(WPCD_ERR_UNSUPPORTED, "too many (k,l,l') combinations");
+    std::map<std::tuple<int, int, int, int>, int> mu_index;   // (l, l', A, k) -> position in the moment row
+    c->mu_pack.clear();
+    for (auto& kv : ll_mono) {
+        int l = kv.first.first, lp = kv.first.second, ll = ll_index[kv.first];
+        for (auto& ak : kv.second) {
+            int A = ak.first, k = ak.second, B = l + lp - A;
+            mu_index[std::make_tuple(l, lp, A, k)] = (int)c->mu_pack.size();
+            c->mu_pack.push_back(trip_index[std::make_pair(ll, k)] | ((A + 1) << 16) | ((B + 1) << 24));
+        }
+    }
+    c->n_mu = (int)c->mu_pack.size();
+    // ---- contraction classes: pairs of one (l, l') that use exactly the same monomial set (for the nd
+    // tables this separates the (lambda, lambda') values, whose k-ranges differ); a set of more than
+    // WPCD_MAX_NM monomials is cut into pieces, the first stores, the others accumulate
+    typedef std::tuple<int, int, std::vector<Mono>> ClassKey;
+    std::map<ClassKey, std::vector<int>> class_pairs;
+    for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
+        int l = c->channel_l[c->pair_gamma[pidx]], lp = c->channel_l[c->pair_gammap[pidx]];
+        std::vector<Mono> sig;
+        for (auto& kv : pair_coef[pidx]) sig.push_back(kv.first);
+        class_pairs[ClassKey(l, lp, sig)].push_back(pidx);
+    }
+    // ---- slabs: class pieces (split at pair granularity when needed) packed into <= WPCD_SLAB_BYTES blobs
+    c->slabs.clear(); c->slab_blob.clear();
+    {
+        struct Piece { const ClassKey* key; int m_first, m_count, nm, p_first, p_count, flags; };
+        auto piece_fixed = [](int nm) { return sizeof(wpcd_class_desc) + ((sizeof(int32_t) * nm + 15) & ~(size_t)15); };
+        auto per_pair = [](int nm) { return sizeof(wpcd_pair_meta) + sizeof(double) * nm; };
+        // pieces beyond the first WPCD_MAX_NM monomials of a class accumulate into stored values: they go
+        // to later PASSES (separate launches), so that no accumulation can overtake its store
+        std::vector<std::vector<Piece>> slab_pieces;
+        std::vector<int> slab_pass;
+        size_t max_sig = 0;
+        for (auto& kv : class_pairs) max_sig = std::max(max_sig, std::get<2>(kv.first).size());
+        for (int pass = 0; pass * WPCD_MAX_NM < (int)max_sig || pass == 0; ++pass) {
+            slab_pieces.emplace_back(); slab_pass.push_back(pass);
+            size_t used = sizeof(wpcd_slab_header);
+            for (auto& kv : class_pairs) {
+                const std::vector<Mono>& sig = std::get<2>(kv.first);
+                const int m_first = pass * WPCD_MAX_NM;
+                const int m_count = std::min<int>(WPCD_MAX_NM, (int)sig.size() - m_first);
+                if (m_count <= 0) continue;
+                const int total_p = (int)kv.second.size();
+                int nm = 4 * ((m_count + 3) / 4), p_first = 0;
+                while (p_first < total_p) {
+                    size_t room = WPCD_SLAB_BYTES > used ? WPCD_SLAB_BYTES - used : 0;
+                    int fit = room > piece_fixed(nm) + per_pair(nm) ? (int)((room - piece_fixed(nm)) / per_pair(nm)) : 0;
+                    if (fit == 0) {
+                        if (slab_pieces.back().empty()) return fail(WPCD_ERR_UNSUPPORTED, "a single channel pair does not fit a contraction slab");
+                        slab_pieces.emplace_back(); slab_pass.push_back(pass); used = sizeof(wpcd_slab_header); continue;
+                    }
+                    int p_count = std::min(fit, total_p - p_first);
+                    slab_pieces.back().push_back({&kv.first, m_first, m_count, nm, p_first, p_count, pass > 0 ? 1 : 0});
+                    used += piece_fixed(nm) + per_pair(nm) * p_count;
+                    p_first += p_count;
+                }
+            }
+            if (slab_pieces.back().empty()) { slab_pieces.pop_back(); slab_pass.pop_back(); }
+        }
+        size_t slab_no = 0;
+        for (auto& pieces : slab_pieces) {
+            // layout: header | descs | index lists | metas | G
+            size_t off_desc = sizeof(wpcd_slab_header);
+            size_t off_idx = off_desc + sizeof(wpcd_class_desc) * pieces.size();
+            size_t idx_bytes = 0, n_meta = 0, n_g = 0;
+            for (auto& pc : pieces) { idx_bytes += (sizeof(int32_t) * pc.nm + 15) & ~(size_t)15; n_meta += pc.p_count; n_g += (size_t)pc.p_count * pc.nm; }
+            size_t off_meta = off_idx + idx_bytes;
+            size_t off_g = off_meta + sizeof(wpcd_pair_meta) * n_meta;
+            size_t bytes = (off_g + sizeof(double) * n_g + 15) & ~(size_t)15;
+            size_t start = c->slab_blob.size();
+            c->slab_blob.resize(start + bytes, 0);
+            unsigned char* base = c->slab_blob.data() + start;
+            wpcd_slab_header hdr = {(int32_t)pieces.size(), 0, 0, 0};
+            std::memcpy(base, &hdr, sizeof(hdr));
+            size_t cur_idx = off_idx, cur_meta = off_meta, cur_g = off_g;
+            double cost = 0.0;
+            for (size_t pi = 0; pi < pieces.size(); ++pi) {
+                const Piece& pc = pieces[pi];
+                int l = std::get<0>(*pc.key), lp = std::get<1>(*pc.key);
+                const std::vector<Mono>& sig = std::get<2>(*pc.key);
+                wpcd_class_desc d = {(int32_t)cur_idx, pc.nm, pc.p_count, (int32_t)cur_meta, (int32_t)cur_g, pc.flags, 0, 0};
+                std::memcpy(base + off_desc + sizeof(d) * pi, &d, sizeof(d));
+                std::vector<int32_t> idx(pc.nm);
+                for (int m = 0; m < pc.nm; ++m) {
+                    const Mono& mo = sig[pc.m_first + std::min(m, pc.m_count - 1)];   // padding repeats the last one (G = 0 there)
+                    idx[m] = mu_index[std::make_tuple(l, lp, mo.first, mo.second)];
+                }
+                std::memcpy(base + cur_idx, idx.data(), sizeof(int32_t) * pc.nm);
+                cur_idx += (sizeof(int32_t) * pc.nm + 15) & ~(size_t)15;
+                const std::vector<int>& plist = class_pairs[*pc.key];
+                for (int q = 0; q < pc.p_count; ++q) {
+                    int pidx = plist[pc.p_first + q];
+                    int ga = c->pair_gamma[pidx];
+                    wpcd_pair_meta m = {(int32_t)chan_off[ga], c->ncoupled[ga], pair_ci[pidx], c->pair_gammap[pidx]};
+                    std::memcpy(base + cur_meta, &m, sizeof(m));
+                    cur_meta += sizeof(m);
+                    std::vector<double> row(pc.nm, 0.0);
+                    for (int mi = 0; mi < pc.m_count; ++mi) row[mi] = pair_coef[pidx][sig[pc.m_first + mi]];
+                    std::memcpy(base + cur_g, row.data(), sizeof(double) * pc.nm);
+                    cur_g += sizeof(double) * pc.nm;
+                }
+                cost += (double)pc.p_count * (pc.nm + 12) + 2.0 * pc.nm + 20.0;
+            }
+            c->slabs.push_back({start, bytes, (int)pieces.size(), cost, slab_pass[slab_no++]});
+        }
+    }
+    c->swave_single = (c->n_ch == 1 && c->n_pairs == 1 && c->n_terms == 1 && c->channel_l[0] == 0 && c->term_k[0] == 0);
+    if (c->swave_single) c->g0 = c->term_g[0];
     // device tables (skipped when the process has no CUDA device: the host-side table stays
     // inspectable, every compute call then fails with WPCD_ERR_CUDA)
     int n_dev = 0;
@@ -218,13 +322,10 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     cudaError_t err;
     if ((err = upload(&c->ncoupled_dev, c->ncoupled)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->chan_off_dev, chan_off)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->pair_gamma_dev, c->pair_gamma)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->pair_gammap_dev, c->pair_gammap)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->pair_ci_dev, pair_ci)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->mu_dev, c->mu)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->mterm_ptr_dev, c->mterm_ptr)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->mterm_mu_dev, c->mterm_mu)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->mterm_g_dev, c->mterm_g)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->ll_pack_dev, c->ll_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->trip_pack_dev, c->trip_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->mu_pack_dev, c->mu_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->slab_blob_dev, c->slab_blob)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     return WPCD_OK;
 }
 

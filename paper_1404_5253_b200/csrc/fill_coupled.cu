@@ -4,14 +4,19 @@
 // B = l+l'-A).  The geometry (F, zeta, limits) is shared by ALL channel pairs of a geometric
 // element, so the work is split in two kernels:
 //
-//   moments_kernel   one warp per geometric element: monomial moments
-//                      M[mu] = norm * sum_nodes w F P_k(x) cos^{A+1} sin^{B+1} zeta1^{-(l'+1)} zeta2^{-(l+1)}
-//                    for the n_mu distinct mu = (k, A, l, l') of the channel set (152 .. 524),
-//                    written to a scratch block [element][mu].
-//   contract_kernel  one CTA per tile of 32 consecutive geometric elements: the moment tile is
-//                    staged in shared memory ([mu][33] doubles), the (g, mu) term lists of the
-//                    coupled pairs stream through shared memory in groups, lane = element, and
-//                    every pair writes 32 consecutive CSR values + column indices (coalesced).
+//   moments_kernel   one warp per geometric element.  With the x-sum factored out,
+//                      M[k,A,l,l'] = sum_m  W_m c_m^{A+1} s_m^{B+1}  I_m[k,l,l'],
+//                      I_m[k,l,l'] = sum_r  P_k(x_r) T_r[l,l'],   T_r[l,l'] = w_r F_r zeta1^{-(l'+1)} zeta2^{-(l+1)},
+//                    so a phi-node costs n_trip * n + n_mu multiply-adds instead of n_mu * n * 3.
+//                    lanes = (phi-node, x-node) pairs for the node set-up, = (k,l,l') triples for I,
+//                    = monomials for M.  The moment row [element][n_mu] is written coalesced.
+//   contract_kernel  value[pair][element] = sum_m G[pair][m] M[element][m] class by class
+//                    (wpcd_internal.h): lane = element, the class block of the moment row lives in
+//                    REGISTERS, the dense coefficient rows G stream from shared memory as broadcast
+//                    128-bit loads.  A CTA owns one slab of classes (copied to shared memory once,
+//                    by a TMA bulk copy) and walks over many 32-element tiles, so that the table is
+//                    read from L2 a few hundred times in all and every moment exactly once.  Each
+//                    pair writes 32 consecutive CSR values + column indices per warp (coalesced).
 #include <math.h>
 
 #include <algorithm>
@@ -27,96 +32,147 @@ __constant__ double k_xi[WPCD_MAX_QUAD];
 __constant__ double k_w[WPCD_MAX_QUAD];
 
 constexpr int MOM_WARPS = 4;
+constexpr int NODE_F = 10;   // doubles per staged phi-node
 
-__device__ __forceinline__ double ipow(double b, int e)
+struct MomentShape {
+    int n;        // quadrature order
+    int G;        // phi-nodes handled together by the node set-up (32 / n, at least 1)
+    int K1;       // k_max + 1
+    int LM1;      // l_max + 1
+    int CP;       // 2 l_max + 2 powers of cos / sin
+    int n_ll, n_trip, n_mu;
+};
+
+__host__ __device__ inline int moment_smem_doubles(const MomentShape& s)
 {
-    double r = 1.0;
-    for (int i = 0; i < e; ++i) r *= b;
-    return r;
+    const int GN = s.G * s.n;
+    return s.n * NODE_F + GN * (s.K1 + s.n_ll) + s.n_trip + 2 * s.G * s.CP;
 }
 
-// packed monomial: k | A<<8 | l<<16 | l'<<24
 template <int MAXS>
 __global__ void __launch_bounds__(MOM_WARPS * 32)
-moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n,
+moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
-               const double2* __restrict__ geo_phi, const wpcd_monomial* __restrict__ mu_tab, int n_mu, int K1, int LP, int CP,
-               double* __restrict__ moments)
+               const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
+               const int32_t* __restrict__ mu_pack, double* __restrict__ moments)
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n = sh.n, G = sh.G, K1 = sh.K1, LM1 = sh.LM1, CP = sh.CP, n_ll = sh.n_ll, n_trip = sh.n_trip, n_mu = sh.n_mu;
+    const int GN = G * n;
+    // block-shared tables: ll_of[(l, l')] -> ll index (or -1), trip_pack
+    int32_t* ll_of = reinterpret_cast<int32_t*>(sm);                     // [LM1*LM1]
+    int32_t* trip_s = ll_of + LM1 * LM1;                                  // [n_trip]
+    double* wbase = sm + ((LM1 * LM1 + n_trip + 1) >> 1);
+    for (int t = threadIdx.x; t < LM1 * LM1; t += blockDim.x) ll_of[t] = -1;
+    __syncthreads();
+    for (int t = threadIdx.x; t < n_ll; t += blockDim.x) { const int v = ll_pack[t]; ll_of[(v & 0xff) * LM1 + (v >> 8)] = t; }
+    for (int t = threadIdx.x; t < n_trip; t += blockDim.x) trip_s[t] = trip_pack[t];
+    __syncthreads();
     const int64_t e = e_begin + (int64_t)blockIdx.x * MOM_WARPS + warp;
     if (e >= e_end) return;
-    const int per_warp = n * (1 + K1 + 2 * LP) + 2 * CP;
-    double* wF = sm + (size_t)warp * per_warp;   // [n]
-    double* Pk = wF + n;                         // [n][K1]
-    double* z1p = Pk + n * K1;                   // [n][LP]   (1/zeta1)^e
-    double* z2p = z1p + n * LP;                  // [n][LP]
-    double* cpw = z2p + n * LP;                  // [CP]      cos^e
-    double* spw = cpw + CP;                      // [CP]      sin^e
+    double* nodeS = wbase + (size_t)warp * moment_smem_doubles(sh);   // [n][NODE_F]
+    double* Pk = nodeS + n * NODE_F;                                  // [GN][K1]
+    double* T = Pk + GN * K1;                                         // [GN][n_ll]
+    double* Ib = T + GN * n_ll;                                       // [n_trip]
+    double* cs = Ib + n_trip;                                         // [G][2][CP]
 
-    int packed[MAXS];
+    int pk[MAXS];
     double acc[MAXS];
 #pragma unroll
     for (int s = 0; s < MAXS; ++s) {
         const int m = lane + 32 * s;
         acc[s] = 0.0;
-        packed[s] = 0;
-        if (m < n_mu) {
-            const wpcd_monomial t = mu_tab[m];
-            packed[s] = (int)t.k | ((int)t.A << 8) | ((int)t.l << 16) | ((int)t.lp << 24);
-        }
+        pk[s] = m < n_mu ? mu_pack[m] : -1;
     }
     const int col = geo_col[e], row = geo_row[e];
     const double2 ph = geo_phi[e];
     const Cell z = load_cell(p, q, n_q, row, col);
+    const CellSq zs = square_cell(z);
     const double norm = cell_norm(z);
     const double half_phi = 0.5 * (ph.y - ph.x), mid_phi = 0.5 * (ph.x + ph.y);
     if (ph.x < ph.y) {
-        for (int m = 0; m < n; ++m) {
-            PhiNode s;
-            if (!phi_node(z, mid_phi + half_phi * k_xi[m], s)) continue;   // warp-uniform
-            const double half_u = 0.5 * (s.u_hi - s.u_lo), mid_u = 0.5 * (s.u_lo + s.u_hi);
-            const double wphi = half_phi * k_w[m] * half_u * norm;
-            if (lane < CP) { cpw[lane] = ipow(s.C, lane); spw[lane] = ipow(s.S, lane); }
-            for (int r = lane; r < n; r += 32) {
+        // ---- step 1: everything that depends on phi only, one lane per phi-node
+        for (int m = lane; m < n; m += 32) {
+            PhiNodeSq s;
+            const bool ok = phi_node_sq(z, zs, mid_phi + half_phi * k_xi[m], s);
+            double* o = nodeS + m * NODE_F;
+            o[0] = ok ? 1.0 : 0.0; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
+            o[5] = s.b1; o[6] = s.b2; o[7] = s.beta; o[8] = s.u_lo; o[9] = s.u_hi;
+        }
+        __syncwarp();
+        for (int m0 = 0; m0 < n; m0 += G) {
+            const int cnt = min(G, n - m0);
+            // ---- step 2: node set-up, lane = (phi-node g, x-node r)
+            for (int idx = lane; idx < cnt * n; idx += 32) {
+                const int g = idx / n, r = idx - g * n;
+                const double* o = nodeS + (m0 + g) * NODE_F;
+                if (o[0] == 0.0) continue;
+                PhiNodeSq s;
+                s.Lq2 = o[3]; s.Uq2 = o[4];
+                const double b1 = o[5], b2 = o[6], beta = o[7], u_lo = o[8], u_hi = o[9];
+                const double half_u = 0.5 * (u_hi - u_lo), mid_u = 0.5 * (u_lo + u_hi);
                 const double u = mid_u + half_u * k_xi[r];
                 const double x = u - 1.0;
-                const double iz1 = rsqrt(s.b1 + s.beta * u), iz2 = rsqrt(s.b2 + s.beta * u);
-                wF[r] = wphi * k_w[r] * F_A14(z, s, iz1, iz2);
+                const double iz1 = rsqrt(b1 + beta * u), iz2 = rsqrt(b2 + beta * u);
+                const double wF = (half_phi * k_w[m0 + g] * norm) * (half_u * k_w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
+                double* Pr = Pk + (g * n + r) * K1;
                 double p0 = 1.0, p1 = x;
-                Pk[r * K1] = 1.0;
-                if (K1 > 1) Pk[r * K1 + 1] = x;
+                Pr[0] = 1.0;
+                if (K1 > 1) Pr[1] = x;
                 for (int k = 2; k < K1; ++k) {
                     const double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) / k;
-                    Pk[r * K1 + k] = p2;
+                    Pr[k] = p2;
                     p0 = p1; p1 = p2;
                 }
-                double a1 = 1.0, a2 = 1.0;
-                for (int ex = 0; ex < LP; ++ex) {
-                    z1p[r * LP + ex] = a1; z2p[r * LP + ex] = a2;
-                    a1 *= iz1; a2 *= iz2;
+                double* Tr = T + (g * n + r) * n_ll;
+                double z2pow = wF * iz2;                                  // wF zeta2^{-(l+1)}
+                for (int l = 0; l < LM1; ++l) {
+                    double both = z2pow * iz1;                            // ... zeta1^{-(l'+1)}
+                    for (int lp = 0; lp < LM1; ++lp) {
+                        const int ll = ll_of[l * LM1 + lp];
+                        if (ll >= 0) Tr[ll] = both;
+                        both *= iz1;
+                    }
+                    z2pow *= iz2;
                 }
             }
+            for (int idx = lane; idx < cnt * CP; idx += 32) {
+                const int g = idx / CP, ex = idx - g * CP;
+                const double* o = nodeS + (m0 + g) * NODE_F;
+                double pc = 1.0, ps = 1.0;
+                for (int i = 0; i < ex; ++i) { pc *= o[1]; ps *= o[2]; }
+                cs[(g * 2 + 0) * CP + ex] = pc;
+                cs[(g * 2 + 1) * CP + ex] = ps;
+            }
             __syncwarp();
+            for (int g = 0; g < cnt; ++g) {
+                if (nodeS[(m0 + g) * NODE_F] == 0.0) continue;           // warp-uniform
+                // ---- step 3: I[k,l,l'] = sum_r P_k(x_r) T_r[l,l'], lane = triple
+                for (int t = lane; t < n_trip; t += 32) {
+                    const int tp = trip_s[t];
+                    const double* Pc = Pk + g * n * K1 + (tp & 0xff);
+                    const double* Tc = T + g * n * n_ll + (tp >> 8);
+                    double a = 0.0;
+                    for (int r = 0; r < n; ++r) a = fma(Pc[r * K1], Tc[r * n_ll], a);
+                    Ib[t] = a;
+                }
+                __syncwarp();
+                // ---- step 4: M[mu] += c^{A+1} s^{B+1} I[triple(mu)], lane = monomial
+                const double* cg = cs + g * 2 * CP;
 #pragma unroll
-            for (int sl = 0; sl < MAXS; ++sl) {
-                if (lane + 32 * sl < n_mu) {
-                    const int pk = packed[sl];
-                    const int k = pk & 0xff, A = (pk >> 8) & 0xff, l = (pk >> 16) & 0xff, lp = (pk >> 24) & 0xff;
-                    double inner = 0.0;
-                    for (int r = 0; r < n; ++r)
-                        inner = fma(wF[r] * Pk[r * K1 + k], z1p[r * LP + lp + 1] * z2p[r * LP + l + 1], inner);
-                    acc[sl] = fma(cpw[A + 1] * spw[l + lp - A + 1], inner, acc[sl]);
+                for (int s = 0; s < MAXS; ++s) {
+                    const int v = pk[s];
+                    if (v >= 0) acc[s] = fma(cg[(v >> 16) & 0xff] * cg[CP + (v >> 24)], Ib[v & 0xffff], acc[s]);
                 }
+                __syncwarp();
             }
-            __syncwarp();
         }
     }
     double* out = moments + (size_t)(e - e_begin) * n_mu;
 #pragma unroll
-    for (int sl = 0; sl < MAXS; ++sl)
-        if (lane + 32 * sl < n_mu) out[lane + 32 * sl] = acc[sl];
+    for (int s = 0; s < MAXS; ++s)
+        if (lane + 32 * s < n_mu) out[lane + 32 * s] = acc[s];
 }
 
 }  // namespace
@@ -125,58 +181,129 @@ namespace {
 
 constexpr int CT_THREADS = 256;
 constexpr int CT_WARPS = CT_THREADS / 32;
-constexpr int TILE = 32;
-constexpr int MS_LD = TILE + 1;   // padded leading dimension of the moment tile
 
-__global__ void __launch_bounds__(CT_THREADS)
+__device__ __forceinline__ uint32_t smem_u32(const void* ptr) { return (uint32_t)__cvta_generic_to_shared(ptr); }
+
+// One slab of classes, global -> shared, as a single TMA bulk copy tracked by an mbarrier.
+__device__ __forceinline__ void slab_to_smem(unsigned char* dst, const unsigned char* src, uint32_t bytes, uint64_t* mbar)
+{
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(mbar)) : "memory");
+    }
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(mbar)) : "memory");
+}
+
+struct TileLane {
+    bool valid;
+    int grp, cnt, pos, gcol;
+    const double* mrow;
+};
+
+// All pairs of one class for the 32 elements of a warp tile.  NM = padded monomial count.
+template <int NM>
+__device__ __forceinline__ void contract_class(const wpcd_class_desc& d, const unsigned char* slab, const TileLane& tl,
+                                               int64_t nnz_geo, int n_geo, int32_t* __restrict__ col_idx,
+                                               double* __restrict__ values)
+{
+    double M[NM];
+    const int4* idx = reinterpret_cast<const int4*>(slab + d.idx_off);
+#pragma unroll
+    for (int m = 0; m < NM / 4; ++m) {
+        const int4 i4 = idx[m];
+        M[4 * m] = __ldg(tl.mrow + i4.x); M[4 * m + 1] = __ldg(tl.mrow + i4.y);
+        M[4 * m + 2] = __ldg(tl.mrow + i4.z); M[4 * m + 3] = __ldg(tl.mrow + i4.w);
+    }
+    const bool add = (d.flags & 1) != 0;
+    const int4* meta = reinterpret_cast<const int4*>(slab + d.meta_off);
+    const double2* G = reinterpret_cast<const double2*>(slab + d.g_off);
+    const int n_pairs = d.n_pairs;
+    int pi = 0;
+    for (; pi + 1 < n_pairs; pi += 2) {
+        const double2* g0 = G + (size_t)pi * (NM / 2);
+        const double2* g1 = g0 + NM / 2;
+        double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+#pragma unroll
+        for (int m = 0; m < NM / 2; ++m) {
+            const double2 u = g0[m], v = g1[m];
+            a0 = fma(u.x, M[2 * m], a0); a1 = fma(u.y, M[2 * m + 1], a1);
+            b0 = fma(v.x, M[2 * m], b0); b1 = fma(v.y, M[2 * m + 1], b1);
+        }
+        const int4 ma = meta[pi], mb = meta[pi + 1];
+        if (tl.valid) {
+            const int64_t oa = (int64_t)ma.x * nnz_geo + (int64_t)ma.y * tl.grp + (int64_t)ma.z * tl.cnt + tl.pos;
+            const int64_t ob = (int64_t)mb.x * nnz_geo + (int64_t)mb.y * tl.grp + (int64_t)mb.z * tl.cnt + tl.pos;
+            values[oa] = add ? values[oa] + (a0 + a1) : a0 + a1; col_idx[oa] = ma.w * n_geo + tl.gcol;
+            values[ob] = add ? values[ob] + (b0 + b1) : b0 + b1; col_idx[ob] = mb.w * n_geo + tl.gcol;
+        }
+    }
+    if (pi < n_pairs) {
+        const double2* g0 = G + (size_t)pi * (NM / 2);
+        double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+        for (int m = 0; m < NM / 2; ++m) { const double2 u = g0[m]; a0 = fma(u.x, M[2 * m], a0); a1 = fma(u.y, M[2 * m + 1], a1); }
+        const int4 ma = meta[pi];
+        if (tl.valid) {
+            const int64_t oa = (int64_t)ma.x * nnz_geo + (int64_t)ma.y * tl.grp + (int64_t)ma.z * tl.cnt + tl.pos;
+            values[oa] = add ? values[oa] + (a0 + a1) : a0 + a1; col_idx[oa] = ma.w * n_geo + tl.gcol;
+        }
+    }
+}
+
+// slab_tab[s] = (blob offset, bytes, first CTA, CTA count)
+__global__ void __launch_bounds__(CT_THREADS, 2)
 contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, const int32_t* __restrict__ geo_col,
                 const int32_t* __restrict__ geo_row, const int32_t* __restrict__ geo_row_ptr,
-                const double* __restrict__ moments, int n_mu, int n_pairs, int pair_group, int stage_cap,
-                const int32_t* __restrict__ mterm_ptr, const int32_t* __restrict__ mterm_mu, const double* __restrict__ mterm_g,
-                const int32_t* __restrict__ pair_gamma, const int32_t* __restrict__ pair_gammap, const int32_t* __restrict__ pair_ci,
-                const int32_t* __restrict__ ncoupled, const int64_t* __restrict__ chan_off,
-                int32_t* __restrict__ col_idx, double* __restrict__ values)
+                const double* __restrict__ moments, int n_mu, const unsigned char* __restrict__ slab_blob,
+                const int4* __restrict__ slab_tab, int n_slabs, int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
-    extern __shared__ double sm[];
-    double* Ms = sm;                                   // [n_mu][MS_LD]
-    double* sg = Ms + (size_t)n_mu * MS_LD;            // [stage_cap]
-    int32_t* smu = reinterpret_cast<int32_t*>(sg + stage_cap);   // [stage_cap]
+    extern __shared__ __align__(128) unsigned char slab[];
+    __shared__ __align__(8) uint64_t mbar;
+    int s = 0;
+    while (s + 1 < n_slabs && (int)blockIdx.x >= slab_tab[s + 1].z) ++s;
+    const int4 st = slab_tab[s];
+    slab_to_smem(slab, slab_blob + st.x, (uint32_t)st.y, &mbar);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t tile0 = e_begin + (int64_t)blockIdx.x * TILE;
-    const int n_here = (int)min((int64_t)TILE, e_end - tile0);
-
-    // moment tile: global [element][mu] -> shared [mu][element]
-    for (int idx = threadIdx.x; idx < TILE * n_mu; idx += CT_THREADS) {
-        const int el = idx / n_mu, m = idx - el * n_mu;
-        Ms[m * MS_LD + el] = el < n_here ? moments[(size_t)(tile0 - e_begin + el) * n_mu + m] : 0.0;
-    }
-    // this lane's element
-    const bool valid = lane < n_here;
-    int64_t grp = 0, cnt = 0, pos = 0;
-    int gcol = 0;
-    if (valid) {
-        const int64_t e = tile0 + lane;
-        const int r = geo_row[e];
-        gcol = geo_col[e];
-        grp = geo_row_ptr[r];
-        cnt = geo_row_ptr[r + 1] - grp;
-        pos = e - grp;
-    }
-    for (int c0 = 0; c0 < n_pairs; c0 += pair_group) {
-        const int c1 = min(n_pairs, c0 + pair_group);
-        const int t0 = mterm_ptr[c0], t1 = mterm_ptr[c1];
-        __syncthreads();                                // previous group consumed / Ms complete
-        for (int t = t0 + threadIdx.x; t < t1; t += CT_THREADS) { sg[t - t0] = mterm_g[t]; smu[t - t0] = mterm_mu[t]; }
-        __syncthreads();
-        for (int c = c0 + warp; c < c1; c += CT_WARPS) {
-            const int ta = mterm_ptr[c] - t0, tb = mterm_ptr[c + 1] - t0;
-            double acc = 0.0;
-            for (int t = ta; t < tb; ++t) acc = fma(sg[t], Ms[smu[t] * MS_LD + lane], acc);
-            if (valid) {
-                const int ga = pair_gamma[c];
-                const int64_t out = chan_off[ga] * nnz_geo + (int64_t)ncoupled[ga] * grp + (int64_t)pair_ci[c] * cnt + pos;
-                values[out] = acc;
-                col_idx[out] = pair_gammap[c] * n_geo + gcol;
+    const int n_classes = reinterpret_cast<const wpcd_slab_header*>(slab)->n_classes;
+    const wpcd_class_desc* desc = reinterpret_cast<const wpcd_class_desc*>(slab + sizeof(wpcd_slab_header));
+    const int64_t n_tiles = (e_end - e_begin + 31) / 32;
+    const int64_t warps_here = (int64_t)st.w * CT_WARPS;
+    for (int64_t tile = (int64_t)((int)blockIdx.x - st.z) * CT_WARPS + warp; tile < n_tiles; tile += warps_here) {
+        const int64_t e = e_begin + tile * 32 + lane;
+        TileLane tl;
+        tl.valid = e < e_end;
+        const int64_t ec = tl.valid ? e : e_end - 1;      // idle lanes shadow the last element (loads stay in range)
+        const int r = geo_row[ec];
+        tl.gcol = geo_col[ec];
+        tl.grp = geo_row_ptr[r];
+        tl.cnt = geo_row_ptr[r + 1] - tl.grp;
+        tl.pos = (int)(ec - tl.grp);
+        tl.mrow = moments + (size_t)(ec - e_begin) * n_mu;
+        for (int ci = 0; ci < n_classes; ++ci) {
+            const wpcd_class_desc d = desc[ci];
+            switch (d.nm) {
+            case 4: contract_class<4>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 8: contract_class<8>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 12: contract_class<12>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 16: contract_class<16>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 20: contract_class<20>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 24: contract_class<24>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 28: contract_class<28>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            default: contract_class<32>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
             }
         }
     }
@@ -195,33 +322,48 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     err = cudaMemcpyToSymbolAsync(k_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
     if (err != cudaSuccess) return err;
     if (nnz_geo == 0 || ch->n_pairs == 0) return cudaSuccess;
-    const int n_mu = ch->n_mu, K1 = ch->k_max + 1, LP = ch->l_max + 2, CP = 2 * ch->l_max + 2;
-    if (CP > 32 || n_mu > 32 * 32) return cudaErrorInvalidValue;
-    // moments kernel shared memory
-    const size_t mom_smem = sizeof(double) * (size_t)MOM_WARPS * ((size_t)n_quad * (1 + K1 + 2 * LP) + 2 * CP);
-    // contraction kernel: pair group so that moment tile + staged terms fit
-    const size_t ms_bytes = sizeof(double) * (size_t)n_mu * MS_LD;
-    int pair_group = 128, stage_cap = 0;
-    for (;; pair_group /= 2) {
-        stage_cap = 0;
-        for (int c0 = 0; c0 < ch->n_pairs; c0 += pair_group) {
-            int c1 = std::min(ch->n_pairs, c0 + pair_group);
-            stage_cap = std::max(stage_cap, ch->mterm_ptr[c1] - ch->mterm_ptr[c0]);
+    if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
+    MomentShape sh;
+    sh.n = n_quad; sh.G = std::max(1, 32 / n_quad); sh.K1 = ch->k_max + 1; sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3;
+    sh.n_ll = ch->n_ll; sh.n_trip = ch->n_trip; sh.n_mu = ch->n_mu;
+    const size_t mom_smem = sizeof(double) * ((size_t)((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + (size_t)MOM_WARPS * moment_smem_doubles(sh));
+    size_t ct_smem = 0;
+    double cost_sum = 0.0;
+    for (auto& sl : ch->slabs) { ct_smem = std::max(ct_smem, sl.bytes); cost_sum += sl.cost; }
+    if (ct_smem > 200 * 1024 || mom_smem > 227 * 1024) return cudaErrorInvalidValue;
+    // CTAs per slab in proportion to its cost, two CTAs per SM per pass
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int n_slabs = (int)ch->slabs.size();
+    int n_pass = 0;
+    for (auto& sl : ch->slabs) n_pass = std::max(n_pass, sl.pass + 1);
+    std::vector<int4> tab(n_slabs);
+    std::vector<int> pass_first(n_pass + 1, 0), pass_ctas(n_pass, 0);
+    for (int pass = 0, s = 0; pass < n_pass; ++pass) {       // slabs are stored pass by pass
+        double cost_pass = 0.0;
+        pass_first[pass] = s;
+        for (int t = s; t < n_slabs && ch->slabs[t].pass == pass; ++t) cost_pass += ch->slabs[t].cost;
+        for (; s < n_slabs && ch->slabs[s].pass == pass; ++s) {
+            int cnt = std::max(1, (int)llround(2.0 * sms * ch->slabs[s].cost / std::max(cost_pass, 1.0)));
+            tab[s] = make_int4((int)ch->slabs[s].offset, (int)ch->slabs[s].bytes, pass_ctas[pass], cnt);
+            pass_ctas[pass] += cnt;
         }
-        stage_cap = (stage_cap + 1) & ~1;
-        if (ms_bytes + 12 * (size_t)stage_cap <= 200 * 1024 || pair_group == 1) break;
+        pass_first[pass + 1] = s;
     }
-    const size_t ct_smem = ms_bytes + 12 * (size_t)stage_cap;
-    if (ct_smem > 227 * 1024 || mom_smem > 227 * 1024) return cudaErrorInvalidValue;
+    (void)cost_sum;
+    int4* tab_dev = reinterpret_cast<int4*>(ws.slab_tab);
+    err = cudaMemcpyAsync(tab_dev, tab.data(), sizeof(int4) * n_slabs, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return err;
     const int n_geo = g->n_p * g->n_q;
-    const int maxs = (n_mu + 31) / 32;
+    const int maxs = (ch->n_mu + 31) / 32;
 #define WPCD_MOM(MS)                                                                                                          \
     do {                                                                                                                      \
         err = cudaFuncSetAttribute(moments_kernel<MS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
         if (err != cudaSuccess) return err;                                                                                   \
-        moments_kernel<MS><<<blocks, MOM_WARPS * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, e0, e1, ws.geo_col,  \
-                                                                     ws.geo_row, ws.geo_phi, ch->mu_dev, n_mu, K1, LP, CP,    \
-                                                                     ws.moments);                                             \
+        moments_kernel<MS><<<blocks, MOM_WARPS * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
+                                                                     ws.geo_row, ws.geo_phi, ch->ll_pack_dev,                 \
+                                                                     ch->trip_pack_dev, ch->mu_pack_dev, ws.moments);         \
     } while (0)
     err = cudaFuncSetAttribute(contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem);
     if (err != cudaSuccess) return err;
@@ -234,22 +376,21 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
             else if (maxs <= 8) WPCD_MOM(8);
             else if (maxs <= 12) WPCD_MOM(12);
             else if (maxs <= 16) WPCD_MOM(16);
-            else if (maxs <= 20) WPCD_MOM(20);
             else if (maxs <= 24) WPCD_MOM(24);
             else WPCD_MOM(32);
             ++g_launches;
             if ((err = cudaGetLastError()) != cudaSuccess) return err;
         }
         {
-            const unsigned blocks = (unsigned)((e1 - e0 + TILE - 1) / TILE);
             StageTimer timer(WPCD_STAGE_CONTRACT, st);
-            contract_kernel<<<blocks, CT_THREADS, ct_smem, st>>>(e0, e1, nnz_geo, n_geo, ws.geo_col, ws.geo_row, geo_row_ptr, ws.moments,
-                                                                 n_mu, ch->n_pairs, pair_group, stage_cap, ch->mterm_ptr_dev,
-                                                                 ch->mterm_mu_dev, ch->mterm_g_dev, ch->pair_gamma_dev,
-                                                                 ch->pair_gammap_dev, ch->pair_ci_dev, ch->ncoupled_dev, ch->chan_off_dev,
-                                                                 col_idx, values);
-            ++g_launches;
-            if ((err = cudaGetLastError()) != cudaSuccess) return err;
+            for (int pass = 0; pass < n_pass; ++pass) {
+                contract_kernel<<<pass_ctas[pass], CT_THREADS, ct_smem, st>>>(e0, e1, nnz_geo, n_geo, ws.geo_col, ws.geo_row, geo_row_ptr,
+                                                                              ws.moments, ch->n_mu, ch->slab_blob_dev,
+                                                                              tab_dev + pass_first[pass],
+                                                                              pass_first[pass + 1] - pass_first[pass], col_idx, values);
+                ++g_launches;
+                if ((err = cudaGetLastError()) != cudaSuccess) return err;
+            }
         }
     }
 #undef WPCD_MOM

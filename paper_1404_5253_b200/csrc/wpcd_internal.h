@@ -28,8 +28,21 @@ struct wpcd_grid {
     int64_t stage_nnz_geo = 0;
 };
 
-// monomial mu = (k, A, l, l'):  P_k(x) cos^{A+1} sin^{l+l'-A+1} / (zeta1^{l'+1} zeta2^{l+1})
-struct wpcd_monomial { int16_t k, A, l, lp; };
+// ---- tables of the coupled-channel fill --------------------------
+// The moment row of a geometric element holds, (l, l') block after block, the distinct monomials
+//   mu = (k, A):  P_k(x) cos^{A+1} sin^{l+l'-A+1} / (zeta1^{l'+1} zeta2^{l+1}).
+// A contraction CLASS is a set of channel pairs of one (l, l') that use exactly the same monomials
+// (at most WPCD_MAX_NM per piece): its coefficients form a dense matrix G[pair][monomial], nm =
+// 4 ceil(n/4) columns.  The classes are packed into SLABS (<= WPCD_SLAB_BYTES of shared memory each),
+// one byte blob per slab that the contraction kernel copies to shared memory verbatim:
+//   SlabHeader | ClassDesc[n_classes] | index lists | PairMeta ... | G ...   (every piece 16-byte aligned)
+struct wpcd_slab_header { int32_t n_classes, pad0, pad1, pad2; };
+struct wpcd_class_desc { int32_t idx_off, nm, n_pairs, meta_off, g_off, flags, pad1, pad2; };   // offsets in bytes from the slab start; idx = positions in the moment row; flags bit 0: add to the stored value
+struct wpcd_pair_meta { int32_t chan_off, ncoup, ci, gammap; };   // row-block offset, #coupled of gamma, rank of gamma', gamma'
+constexpr size_t WPCD_SLAB_BYTES = 100 * 1024;
+constexpr int WPCD_MAX_NM = 32;          // monomials per class the register kernel handles
+
+struct wpcd_slab { size_t offset, bytes; int n_classes; double cost; int pass; };
 
 struct wpcd_channels {
     int model = 0;
@@ -42,22 +55,23 @@ struct wpcd_channels {
     std::vector<int32_t> pair_gamma, pair_gammap, term_k, term_l1, term_l1p;
     std::vector<int64_t> term_ptr;
     std::vector<double> term_g;
-    // merged monomial form used by the fill kernels
-    int n_mu = 0, k_max = 0, l_max = 0;
-    std::vector<wpcd_monomial> mu;            // [n_mu]
-    std::vector<int32_t> mterm_ptr;           // [n_pairs+1]
-    std::vector<int32_t> mterm_mu;            // merged terms: monomial index
-    std::vector<double> mterm_g;              //               coefficient
+    // moment tables
+    int n_mu = 0;                 // length of a moment row (class blocks with padding)
+    int k_max = 0, l_max = 0;
+    int n_ll = 0, n_trip = 0;
+    std::vector<int32_t> ll_pack;     // [n_ll]   l | l' << 8            distinct (l, l')
+    std::vector<int32_t> trip_pack;   // [n_trip] k | ll << 8            distinct (k, l, l'), sorted by (ll, k)
+    std::vector<int32_t> mu_pack;     // [n_mu]   trip | (A+1) << 16 | (B+1) << 24
+    // contraction slabs
+    std::vector<wpcd_slab> slabs;
+    std::vector<unsigned char> slab_blob;
     // device tables
     int32_t* ncoupled_dev = nullptr;          // [n_ch]   number of gamma' coupled to gamma
     int64_t* chan_off_dev = nullptr;          // [n_ch+1] prefix of ncoupled
-    int32_t* pair_gamma_dev = nullptr;        // [n_pairs]
-    int32_t* pair_gammap_dev = nullptr;       // [n_pairs]
-    int32_t* pair_ci_dev = nullptr;           // [n_pairs] rank of gamma' among the coupled of gamma
-    wpcd_monomial* mu_dev = nullptr;          // [n_mu]
-    int32_t* mterm_ptr_dev = nullptr;         // [n_pairs+1]
-    int32_t* mterm_mu_dev = nullptr;
-    double* mterm_g_dev = nullptr;
+    int32_t* ll_pack_dev = nullptr;
+    int32_t* trip_pack_dev = nullptr;
+    int32_t* mu_pack_dev = nullptr;
+    unsigned char* slab_blob_dev = nullptr;
     std::vector<int32_t> ncoupled;
     int64_t total_coupled = 0;
 };
@@ -85,6 +99,7 @@ struct Workspace {
     int32_t* geo_row;    // [nnz_geo]
     double2* geo_phi;    // [nnz_geo]  (phi_a, phi_b)
     double* moments;     // [chunk * n_mu] (coupled channels only)
+    void* slab_tab;      // [n_slabs] int4 (coupled channels only)
     int64_t chunk;       // geometric elements per moment chunk
     size_t bytes;
 };

@@ -34,21 +34,67 @@ __constant__ double k_w[WPCD_MAX_QUAD];
 constexpr int MOM_WARPS = 4;
 constexpr int NODE_F = 10;   // doubles per staged phi-node
 
+__constant__ double k_invk[WPCD_MAX_K + 2];   // 1/k for the Legendre recurrence
+
 struct MomentShape {
     int n;        // quadrature order
-    int G;        // phi-nodes handled together by the node set-up (32 / n, at least 1)
+    int G;        // phi-nodes handled together by the node set-up
     int K1;       // k_max + 1
+    int SP;       // row stride of the P_k table:  8 ceil(K1 / 8) + 4   (conflict-free fragment loads)
+    int ST;       // row stride of the T table:    8 ceil(n_ll / 8) + 4
+    int IS;       // row stride of the I table:    8 ceil(n_ll / 8) + 2
     int LM1;      // l_max + 1
-    int CP;       // 2 l_max + 2 powers of cos / sin
+    int CP;       // 2 l_max + 3 powers of cos / sin
+    int CSH;      // log2 of the row stride of the c^a s^b table (16 or 32 columns)
     int n_ll, n_trip, n_mu;
 };
 
 __host__ __device__ inline int moment_smem_doubles(const MomentShape& s)
 {
-    const int GN = s.G * s.n;
-    return s.n * NODE_F + GN * (s.K1 + s.n_ll) + s.n_trip + 2 * s.G * s.CP;
+    const int rows = s.G * s.n, K1P = (s.SP - 4);
+    return (s.n * NODE_F + rows * (s.SP + s.ST) + K1P * s.IS + s.G * 2 * s.CP + (s.CP << s.CSH) + 1) & ~1;   // even: 16-byte pieces
 }
 
+// D (8x8) += A (8x4, row) * B (4x8, col), FP64 tensor-core MMA.  Fragment layout: a = A[lane/4][lane%4],
+// b = B[lane%4][lane/4], (c0, c1) = C[lane/4][2 (lane%4) + {0,1}].
+__device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] for one phi-node: (K1 x n) (n x n_ll) in 8x8x4 MMAs.
+// Pg / Tg point at this lane's fragment element of x-node (lane % 4); rows r >= n read as zero.
+template <int KT>
+__device__ __forceinline__ void node_mma(const double* __restrict__ Pg, const double* __restrict__ Tg, int n, int SP, int ST,
+                                         int MT, int NT, double* __restrict__ Ib, int IS, int lane)
+{
+    bool live[KT];
+#pragma unroll
+    for (int kt = 0; kt < KT; ++kt) live[kt] = kt * 4 + (lane & 3) < n;
+    double* Io = Ib + (lane >> 2) * IS + 2 * (lane & 3);
+    for (int mt = 0; mt < MT; ++mt) {
+        double a[KT];
+#pragma unroll
+        for (int kt = 0; kt < KT; ++kt) a[kt] = live[kt] ? Pg[kt * 4 * SP + mt * 8] : 0.0;
+        for (int nt = 0; nt < NT; ++nt) {
+            double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) dmma_884(c0, c1, a[kt], live[kt] ? Tg[kt * 4 * ST + nt * 8] : 0.0);
+            *reinterpret_cast<double2*>(Io + mt * 8 * IS + nt * 8) = make_double2(c0, c1);
+        }
+    }
+}
+
+__device__ __forceinline__ double ipow_small(double b, int e)   // e < 64
+{
+    double r = 1.0;
+#pragma unroll
+    for (int bit = 0; bit < 6; ++bit) { if (e & (1 << bit)) r *= b; b *= b; }
+    return r;
+}
+
+// Moment layout: [tile of 32 elements][mu][element in tile] (the contraction reads 32 elements of
+// one monomial as one 256-byte line).
 template <int MAXS>
 __global__ void __launch_bounds__(MOM_WARPS * 32)
 moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
@@ -58,12 +104,12 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n = sh.n, G = sh.G, K1 = sh.K1, LM1 = sh.LM1, CP = sh.CP, n_ll = sh.n_ll, n_trip = sh.n_trip, n_mu = sh.n_mu;
-    const int GN = G * n;
+    const int n = sh.n, G = sh.G, K1 = sh.K1, SP = sh.SP, ST = sh.ST, IS = sh.IS, LM1 = sh.LM1, CP = sh.CP, CSH = sh.CSH;
+    const int n_ll = sh.n_ll, n_trip = sh.n_trip, n_mu = sh.n_mu;
     // block-shared tables: ll_of[(l, l')] -> ll index (or -1), trip_pack
     int32_t* ll_of = reinterpret_cast<int32_t*>(sm);                     // [LM1*LM1]
     int32_t* trip_s = ll_of + LM1 * LM1;                                  // [n_trip]
-    double* wbase = sm + ((LM1 * LM1 + n_trip + 1) >> 1);
+    double* wbase = sm + ((((LM1 * LM1 + n_trip + 1) >> 1) + 1) & ~1);
     for (int t = threadIdx.x; t < LM1 * LM1; t += blockDim.x) ll_of[t] = -1;
     __syncthreads();
     for (int t = threadIdx.x; t < n_ll; t += blockDim.x) { const int v = ll_pack[t]; ll_of[(v & 0xff) * LM1 + (v >> 8)] = t; }
@@ -71,19 +117,26 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     __syncthreads();
     const int64_t e = e_begin + (int64_t)blockIdx.x * MOM_WARPS + warp;
     if (e >= e_end) return;
+    const bool full_ll = n_ll == LM1 * LM1;                           // every (l, l') present: ll = l * LM1 + l'
     double* nodeS = wbase + (size_t)warp * moment_smem_doubles(sh);   // [n][NODE_F]
-    double* Pk = nodeS + n * NODE_F;                                  // [GN][K1]
-    double* T = Pk + GN * K1;                                         // [GN][n_ll]
-    double* Ib = T + GN * n_ll;                                       // [n_trip]
-    double* cs = Ib + n_trip;                                         // [G][2][CP]
+    double* Pk = nodeS + n * NODE_F;                                  // [G*n][SP]    P_k(x_r)
+    double* T = Pk + G * n * SP;                                      // [G*n][ST]    T_r[l,l']
+    double* Ib = T + G * n * ST;                                      // [K1P][IS]    I[k][l,l'] of one phi-node
+    double* cs = Ib + (SP - 4) * IS;                                  // [G][2][CP]   powers of cos, sin
+    double* csp = cs + G * 2 * CP;                                    // [CP][1<<CSH] c^a s^b of one phi-node
 
+    // per monomial: offset into Ib (low 16 bits) and into csp (high 16 bits)
     int pk[MAXS];
     double acc[MAXS];
 #pragma unroll
     for (int s = 0; s < MAXS; ++s) {
         const int m = lane + 32 * s;
         acc[s] = 0.0;
-        pk[s] = m < n_mu ? mu_pack[m] : -1;
+        pk[s] = -1;
+        if (m < n_mu) {
+            const int v = mu_pack[m], tp = trip_s[v & 0xffff];
+            pk[s] = ((tp & 0xff) * IS + (tp >> 8)) | (((((v >> 16) & 0xff) << CSH) + (v >> 24)) << 16);
+        }
     }
     const int col = geo_col[e], row = geo_row[e];
     const double2 ph = geo_phi[e];
@@ -91,6 +144,7 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     const CellSq zs = square_cell(z);
     const double norm = cell_norm(z);
     const double half_phi = 0.5 * (ph.y - ph.x), mid_phi = 0.5 * (ph.x + ph.y);
+    const int MT = (SP - 4) >> 3, NT = (ST - 4) >> 3, KT = (n + 3) >> 2;
     if (ph.x < ph.y) {
         // ---- step 1: everything that depends on phi only, one lane per phi-node
         for (int m = lane; m < n; m += 32) {
@@ -116,63 +170,85 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                 const double x = u - 1.0;
                 const double iz1 = rsqrt(b1 + beta * u), iz2 = rsqrt(b2 + beta * u);
                 const double wF = (half_phi * k_w[m0 + g] * norm) * (half_u * k_w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
-                double* Pr = Pk + (g * n + r) * K1;
+                double* Pr = Pk + (g * n + r) * SP;
                 double p0 = 1.0, p1 = x;
                 Pr[0] = 1.0;
                 if (K1 > 1) Pr[1] = x;
                 for (int k = 2; k < K1; ++k) {
-                    const double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) / k;
+                    const double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) * k_invk[k];
                     Pr[k] = p2;
                     p0 = p1; p1 = p2;
                 }
-                double* Tr = T + (g * n + r) * n_ll;
+                double* Tr = T + (g * n + r) * ST;
                 double z2pow = wF * iz2;                                  // wF zeta2^{-(l+1)}
-                for (int l = 0; l < LM1; ++l) {
-                    double both = z2pow * iz1;                            // ... zeta1^{-(l'+1)}
-                    for (int lp = 0; lp < LM1; ++lp) {
-                        const int ll = ll_of[l * LM1 + lp];
-                        if (ll >= 0) Tr[ll] = both;
-                        both *= iz1;
+                if (full_ll) {
+                    for (int l = 0; l < LM1; ++l) {
+                        double both = z2pow * iz1;                        // ... zeta1^{-(l'+1)}
+                        for (int lp = 0; lp < LM1; ++lp) { Tr[l * LM1 + lp] = both; both *= iz1; }
+                        z2pow *= iz2;
                     }
-                    z2pow *= iz2;
+                } else {
+                    for (int l = 0; l < LM1; ++l) {
+                        double both = z2pow * iz1;
+                        for (int lp = 0; lp < LM1; ++lp) {
+                            const int ll = ll_of[l * LM1 + lp];
+                            if (ll >= 0) Tr[ll] = both;
+                            both *= iz1;
+                        }
+                        z2pow *= iz2;
+                    }
                 }
             }
             for (int idx = lane; idx < cnt * CP; idx += 32) {
                 const int g = idx / CP, ex = idx - g * CP;
                 const double* o = nodeS + (m0 + g) * NODE_F;
-                double pc = 1.0, ps = 1.0;
-                for (int i = 0; i < ex; ++i) { pc *= o[1]; ps *= o[2]; }
-                cs[(g * 2 + 0) * CP + ex] = pc;
-                cs[(g * 2 + 1) * CP + ex] = ps;
+                cs[(g * 2 + 0) * CP + ex] = ipow_small(o[1], ex);
+                cs[(g * 2 + 1) * CP + ex] = ipow_small(o[2], ex);
             }
             __syncwarp();
             for (int g = 0; g < cnt; ++g) {
                 if (nodeS[(m0 + g) * NODE_F] == 0.0) continue;           // warp-uniform
-                // ---- step 3: I[k,l,l'] = sum_r P_k(x_r) T_r[l,l'], lane = triple
-                for (int t = lane; t < n_trip; t += 32) {
-                    const int tp = trip_s[t];
-                    const double* Pc = Pk + g * n * K1 + (tp & 0xff);
-                    const double* Tc = T + g * n * n_ll + (tp >> 8);
-                    double a = 0.0;
-                    for (int r = 0; r < n; ++r) a = fma(Pc[r * K1], Tc[r * n_ll], a);
-                    Ib[t] = a;
+                // c^a s^b table of this phi-node
+                for (int idx = lane; idx < (CP << CSH); idx += 32) {
+                    const int ea = idx >> CSH, eb = idx & ((1 << CSH) - 1);
+                    if (eb < CP) csp[idx] = cs[(g * 2 + 0) * CP + ea] * cs[(g * 2 + 1) * CP + eb];
+                }
+                // ---- step 3: I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] on the FP64 tensor cores
+                const double* Pg = Pk + (g * n + (lane & 3)) * SP + (lane >> 2);
+                const double* Tg = T + (g * n + (lane & 3)) * ST + (lane >> 2);
+                switch (KT) {
+                case 1: node_mma<1>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 2: node_mma<2>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 3: node_mma<3>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 4: node_mma<4>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
+                default:
+                    for (int mt = 0; mt < MT; ++mt)
+                        for (int nt = 0; nt < NT; ++nt) {
+                            double c0 = 0.0, c1 = 0.0;
+                            for (int kt = 0; kt < KT; ++kt) {
+                                const bool live = kt * 4 + (lane & 3) < n;
+                                dmma_884(c0, c1, live ? Pg[kt * 4 * SP + mt * 8] : 0.0, live ? Tg[kt * 4 * ST + nt * 8] : 0.0);
+                            }
+                            *reinterpret_cast<double2*>(Ib + (mt * 8 + (lane >> 2)) * IS + nt * 8 + 2 * (lane & 3)) = make_double2(c0, c1);
+                        }
+                    break;
                 }
                 __syncwarp();
-                // ---- step 4: M[mu] += c^{A+1} s^{B+1} I[triple(mu)], lane = monomial
-                const double* cg = cs + g * 2 * CP;
+                // ---- step 4: M[mu] += c^{A+1} s^{B+1} I[k][l,l'], lane = monomial
 #pragma unroll
                 for (int s = 0; s < MAXS; ++s) {
                     const int v = pk[s];
-                    if (v >= 0) acc[s] = fma(cg[(v >> 16) & 0xff] * cg[CP + (v >> 24)], Ib[v & 0xffff], acc[s]);
+                    if (v >= 0) acc[s] = fma(csp[v >> 16], Ib[v & 0xffff], acc[s]);
                 }
                 __syncwarp();
             }
         }
     }
-    double* out = moments + (size_t)(e - e_begin) * n_mu;
+    const int64_t el = e - e_begin;
+    double* out = moments + ((size_t)(el >> 5) * n_mu) * 32 + (el & 31);
 #pragma unroll
     for (int s = 0; s < MAXS; ++s)
-        if (lane + 32 * s < n_mu) out[lane + 32 * s] = acc[s];
+        if (lane + 32 * s < n_mu) out[(size_t)(lane + 32 * s) * 32] = acc[s];
 }
 
 }  // namespace
@@ -211,7 +287,7 @@ __device__ __forceinline__ void slab_to_smem(unsigned char* dst, const unsigned 
 struct TileLane {
     bool valid;
     int grp, cnt, pos, gcol;
-    const double* mrow;
+    const double* mrow;     // moments of this tile, [mu][32], offset by the lane
 };
 
 // All pairs of one class for the 32 elements of a warp tile.  NM = padded monomial count.
@@ -225,8 +301,8 @@ __device__ __forceinline__ void contract_class(const wpcd_class_desc& d, const u
 #pragma unroll
     for (int m = 0; m < NM / 4; ++m) {
         const int4 i4 = idx[m];
-        M[4 * m] = __ldg(tl.mrow + i4.x); M[4 * m + 1] = __ldg(tl.mrow + i4.y);
-        M[4 * m + 2] = __ldg(tl.mrow + i4.z); M[4 * m + 3] = __ldg(tl.mrow + i4.w);
+        M[4 * m] = __ldg(tl.mrow + i4.x * 32); M[4 * m + 1] = __ldg(tl.mrow + i4.y * 32);
+        M[4 * m + 2] = __ldg(tl.mrow + i4.z * 32); M[4 * m + 3] = __ldg(tl.mrow + i4.w * 32);
     }
     const bool add = (d.flags & 1) != 0;
     const int4* meta = reinterpret_cast<const int4*>(slab + d.meta_off);
@@ -292,9 +368,17 @@ contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, cons
         tl.grp = geo_row_ptr[r];
         tl.cnt = geo_row_ptr[r + 1] - tl.grp;
         tl.pos = (int)(ec - tl.grp);
-        tl.mrow = moments + (size_t)(ec - e_begin) * n_mu;
+        tl.mrow = moments + (size_t)tile * n_mu * 32 + lane;
         for (int ci = 0; ci < n_classes; ++ci) {
             const wpcd_class_desc d = desc[ci];
+            if (ci + 1 < n_classes) {       // pull the next class's moment lines towards the SM while this one computes
+                const wpcd_class_desc dn = desc[ci + 1];
+                if (lane < dn.nm) {
+                    const double* nxt = tl.mrow - lane + (size_t)reinterpret_cast<const int32_t*>(slab + dn.idx_off)[lane] * 32;
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(nxt));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(nxt + 16));
+                }
+            }
             switch (d.nm) {
             case 4: contract_class<4>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
             case 8: contract_class<8>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
@@ -324,9 +408,20 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if (nnz_geo == 0 || ch->n_pairs == 0) return cudaSuccess;
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
-    sh.n = n_quad; sh.G = std::max(1, 32 / n_quad); sh.K1 = ch->k_max + 1; sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3;
+    sh.n = n_quad; sh.G = std::max(1, std::min(32 / n_quad, 2));
+    sh.K1 = ch->k_max + 1; sh.SP = 8 * ((sh.K1 + 7) / 8) + 4;
+    sh.ST = 8 * ((ch->n_ll + 7) / 8) + 4; sh.IS = 8 * ((ch->n_ll + 7) / 8) + 2;
+    sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.CSH = sh.CP <= 16 ? 4 : 5;
     sh.n_ll = ch->n_ll; sh.n_trip = ch->n_trip; sh.n_mu = ch->n_mu;
-    const size_t mom_smem = sizeof(double) * ((size_t)((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + (size_t)MOM_WARPS * moment_smem_doubles(sh));
+    if ((sh.SP - 4) * sh.IS >= 65536 || sh.CP > 32) return cudaErrorInvalidValue;
+    {
+        double invk[WPCD_MAX_K + 2];
+        invk[0] = 0.0;
+        for (int k = 1; k < WPCD_MAX_K + 2; ++k) invk[k] = 1.0 / k;
+        err = cudaMemcpyToSymbolAsync(k_invk, invk, sizeof(invk), 0, cudaMemcpyHostToDevice, st);
+        if (err != cudaSuccess) return err;
+    }
+    const size_t mom_smem = sizeof(double) * ((size_t)((((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + 1) & ~1) + (size_t)MOM_WARPS * moment_smem_doubles(sh));
     size_t ct_smem = 0;
     double cost_sum = 0.0;
     for (auto& sl : ch->slabs) { ct_smem = std::max(ct_smem, sl.bytes); cost_sum += sl.cost; }

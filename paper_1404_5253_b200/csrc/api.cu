@@ -144,7 +144,7 @@ static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_p
 static void free_channels_device(wpcd_channels* c)
 {
     cudaFree(c->ncoupled_dev); cudaFree(c->chan_off_dev); cudaFree(c->ll_pack_dev); cudaFree(c->trip_pack_dev);
-    cudaFree(c->mu_pack_dev); cudaFree(c->slab_blob_dev);
+    cudaFree(c->mu_pack_dev); cudaFree(c->ab_pack_dev); cudaFree(c->slab_blob_dev);
 }
 
 template <class T>
@@ -208,15 +208,20 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->n_trip = (int)c->trip_pack.size();
     if (c->n_trip >= 65536) return fail(WPCD_ERR_UNSUPPORTED, "too many (k,l,l') combinations");
     std::map<std::tuple<int, int, int, int>, int> mu_index;   // (l, l', A, k) -> position in the moment row
-    c->mu_pack.clear();
+    c->mu_pack.clear(); c->ab_pack.clear();
+    std::map<std::pair<int, int>, int> ab_index;
     for (auto& kv : ll_mono) {
         int l = kv.first.first, lp = kv.first.second, ll = ll_index[kv.first];
         for (auto& ak : kv.second) {
             int A = ak.first, k = ak.second, B = l + lp - A;
+            auto ab = ab_index.emplace(std::make_pair(A + 1, B + 1), (int)c->ab_pack.size());
+            if (ab.second) c->ab_pack.push_back((A + 1) | ((B + 1) << 8));
             mu_index[std::make_tuple(l, lp, A, k)] = (int)c->mu_pack.size();
-            c->mu_pack.push_back(trip_index[std::make_pair(ll, k)] | ((A + 1) << 16) | ((B + 1) << 24));
+            c->mu_pack.push_back(trip_index[std::make_pair(ll, k)] | (ab.first->second << 16));
         }
     }
+    c->n_ab = (int)c->ab_pack.size();
+    if (c->n_ab >= 32768) return fail(WPCD_ERR_UNSUPPORTED, "too many cos/sin exponent pairs");
     c->n_mu = (int)c->mu_pack.size();
     // ---- contraction classes: pairs of one (l, l') that use exactly the same monomial set (for the nd
     // tables this separates the (lambda, lambda') values, whose k-ranges differ); a set of more than
@@ -325,6 +330,7 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     if ((err = upload(&c->ll_pack_dev, c->ll_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->trip_pack_dev, c->trip_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->mu_pack_dev, c->mu_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->ab_pack_dev, c->ab_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->slab_blob_dev, c->slab_blob)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     return WPCD_OK;
 }

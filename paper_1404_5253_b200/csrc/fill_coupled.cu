@@ -18,6 +18,7 @@
 //                    read from L2 a few hundred times in all and every moment exactly once.  Each
 //                    pair writes 32 consecutive CSR values + column indices per warp (coalesced).
 #include <math.h>
+#include <stdlib.h>
 
 #include <algorithm>
 
@@ -45,14 +46,14 @@ struct MomentShape {
     int IS;       // row stride of the I table:    8 ceil(n_ll / 8) + 2
     int LM1;      // l_max + 1
     int CP;       // 2 l_max + 3 powers of cos / sin
-    int CSH;      // log2 of the row stride of the c^a s^b table (16 or 32 columns)
+    int n_ab;     // distinct (A+1, B+1) exponent pairs
     int n_ll, n_trip, n_mu;
 };
 
 __host__ __device__ inline int moment_smem_doubles(const MomentShape& s)
 {
     const int rows = s.G * s.n, K1P = (s.SP - 4);
-    return (s.n * NODE_F + rows * (s.SP + s.ST) + K1P * s.IS + s.G * 2 * s.CP + (s.CP << s.CSH) + 1) & ~1;   // even: 16-byte pieces
+    return (s.n * NODE_F + rows * (s.SP + s.ST) + K1P * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;   // even: 16-byte pieces
 }
 
 // D (8x8) += A (8x4, row) * B (4x8, col), FP64 tensor-core MMA.  Fragment layout: a = A[lane/4][lane%4],
@@ -100,11 +101,11 @@ __global__ void __launch_bounds__(MOM_WARPS * 32)
 moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
-               const int32_t* __restrict__ mu_pack, double* __restrict__ moments)
+               const int32_t* __restrict__ mu_pack, const int32_t* __restrict__ ab_pack, double* __restrict__ moments)
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n = sh.n, G = sh.G, K1 = sh.K1, SP = sh.SP, ST = sh.ST, IS = sh.IS, LM1 = sh.LM1, CP = sh.CP, CSH = sh.CSH;
+    const int n = sh.n, G = sh.G, K1 = sh.K1, SP = sh.SP, ST = sh.ST, IS = sh.IS, LM1 = sh.LM1, CP = sh.CP, n_ab = sh.n_ab;
     const int n_ll = sh.n_ll, n_trip = sh.n_trip, n_mu = sh.n_mu;
     // block-shared tables: ll_of[(l, l')] -> ll index (or -1), trip_pack
     int32_t* ll_of = reinterpret_cast<int32_t*>(sm);                     // [LM1*LM1]
@@ -123,7 +124,7 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     double* T = Pk + G * n * SP;                                      // [G*n][ST]    T_r[l,l']
     double* Ib = T + G * n * ST;                                      // [K1P][IS]    I[k][l,l'] of one phi-node
     double* cs = Ib + (SP - 4) * IS;                                  // [G][2][CP]   powers of cos, sin
-    double* csp = cs + G * 2 * CP;                                    // [CP][1<<CSH] c^a s^b of one phi-node
+    double* csp = cs + G * 2 * CP;                                    // [n_ab]       c^a s^b of one phi-node
 
     // per monomial: offset into Ib (low 16 bits) and into csp (high 16 bits)
     int pk[MAXS];
@@ -135,7 +136,7 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
         pk[s] = -1;
         if (m < n_mu) {
             const int v = mu_pack[m], tp = trip_s[v & 0xffff];
-            pk[s] = ((tp & 0xff) * IS + (tp >> 8)) | (((((v >> 16) & 0xff) << CSH) + (v >> 24)) << 16);
+            pk[s] = ((tp & 0xff) * IS + (tp >> 8)) | ((v >> 16) << 16);     // mu_pack: triple | ab index << 16
         }
     }
     const int col = geo_col[e], row = geo_row[e];
@@ -209,9 +210,9 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
             for (int g = 0; g < cnt; ++g) {
                 if (nodeS[(m0 + g) * NODE_F] == 0.0) continue;           // warp-uniform
                 // c^a s^b table of this phi-node
-                for (int idx = lane; idx < (CP << CSH); idx += 32) {
-                    const int ea = idx >> CSH, eb = idx & ((1 << CSH) - 1);
-                    if (eb < CP) csp[idx] = cs[(g * 2 + 0) * CP + ea] * cs[(g * 2 + 1) * CP + eb];
+                for (int idx = lane; idx < n_ab; idx += 32) {
+                    const int ab = ab_pack[idx];
+                    csp[idx] = cs[(g * 2 + 0) * CP + (ab & 0xff)] * cs[(g * 2 + 1) * CP + (ab >> 8)];
                 }
                 // ---- step 3: I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] on the FP64 tensor cores
                 const double* Pg = Pk + (g * n + (lane & 3)) * SP + (lane >> 2);
@@ -408,12 +409,13 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if (nnz_geo == 0 || ch->n_pairs == 0) return cudaSuccess;
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
-    sh.n = n_quad; sh.G = std::max(1, std::min(32 / n_quad, 2));
+    static const int g_forced = [] { const char* e = getenv("WPCD_MOM_G"); return e ? atoi(e) : 0; }();   // tuning knob
+    sh.n = n_quad; sh.G = std::max(1, std::min(32 / n_quad, g_forced > 0 ? g_forced : 2));
     sh.K1 = ch->k_max + 1; sh.SP = 8 * ((sh.K1 + 7) / 8) + 4;
     sh.ST = 8 * ((ch->n_ll + 7) / 8) + 4; sh.IS = 8 * ((ch->n_ll + 7) / 8) + 2;
-    sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.CSH = sh.CP <= 16 ? 4 : 5;
+    sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.n_ab = ch->n_ab;
     sh.n_ll = ch->n_ll; sh.n_trip = ch->n_trip; sh.n_mu = ch->n_mu;
-    if ((sh.SP - 4) * sh.IS >= 65536 || sh.CP > 32) return cudaErrorInvalidValue;
+    if ((sh.SP - 4) * sh.IS >= 65536) return cudaErrorInvalidValue;
     {
         double invk[WPCD_MAX_K + 2];
         invk[0] = 0.0;
@@ -458,7 +460,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         if (err != cudaSuccess) return err;                                                                                   \
         moments_kernel<MS><<<blocks, MOM_WARPS * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
                                                                      ws.geo_row, ws.geo_phi, ch->ll_pack_dev,                 \
-                                                                     ch->trip_pack_dev, ch->mu_pack_dev, ws.moments);         \
+                                                                     ch->trip_pack_dev, ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);         \
     } while (0)
     err = cudaFuncSetAttribute(contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem);
     if (err != cudaSuccess) return err;

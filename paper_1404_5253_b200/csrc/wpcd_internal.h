@@ -61,7 +61,9 @@ struct wpcd_channels {
     int n_ll = 0, n_trip = 0;
     std::vector<int32_t> ll_pack;     // [n_ll]   l | l' << 8            distinct (l, l')
     std::vector<int32_t> trip_pack;   // [n_trip] k | ll << 8            distinct (k, l, l'), sorted by (ll, k)
-    std::vector<int32_t> mu_pack;     // [n_mu]   trip | (A+1) << 16 | (B+1) << 24
+    std::vector<int32_t> mu_pack;     // [n_mu]   trip | ab << 16
+    std::vector<int32_t> ab_pack;     // [n_ab]   (A+1) | (B+1) << 8       distinct exponent pairs of cos, sin
+    int n_ab = 0;
     // contraction slabs
     std::vector<wpcd_slab> slabs;
     std::vector<unsigned char> slab_blob;
@@ -71,6 +73,7 @@ struct wpcd_channels {
     int32_t* ll_pack_dev = nullptr;
     int32_t* trip_pack_dev = nullptr;
     int32_t* mu_pack_dev = nullptr;
+    int32_t* ab_pack_dev = nullptr;
     unsigned char* slab_blob_dev = nullptr;
     std::vector<int32_t> ncoupled;
     int64_t total_coupled = 0;

@@ -209,9 +209,9 @@ def run_ours(args):
 
     from paper_1404_5253_b200 import build as _build
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1404_5253_b200 import shard
+
+    rank, local_rank, world = shard.rank_world()
     if rank == 0:
         _build.build()
     import paper_1404_5253_b200 as wpcd
@@ -225,7 +225,7 @@ def run_ours(args):
         dist.barrier()
     wpcd.load()
     wl = wi.WORKLOADS[args.workload]
-    p = wl.grid(seed_offset=rank)           # independent lattice per rank (weak scaling)
+    p = wl.grid(seed_offset=shard.lattice_seed_offset(rank))   # independent lattice per rank (weak scaling)
     stream = torch.cuda.current_stream()
     grid = wpcd.wpcd_grid_create(p, p)
 
@@ -315,14 +315,9 @@ def run_ours(args):
     sampler.join()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     spmv_ms = sum(a.elapsed_time(b) for a, b in sp_ev)
-    t_local = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    nnz_local = torch.tensor([float(sum(j.nnz for j in jobs))], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_local, op=dist.ReduceOp.MAX)
-        dist.all_reduce(nnz_local, op=dist.ReduceOp.SUM)
-    ms_per_step = t_local.item() / args.steps
-    nnz_all = nnz_local.item()
-    value = nnz_all / (ms_per_step * 1e-3)
+    ms_max, nnz_all = shard.reduce_step(dist, "cuda", total_ms, sum(j.nnz for j in jobs))
+    ms_per_step = ms_max / args.steps
+    value = shard.throughput(ms_per_step, nnz_all)
 
     # ---- end to end through the C-ABI with HOST buffers (handles, tables and vectors from the host)
     def e2e_step():

@@ -79,10 +79,20 @@ namespace wpcd_detail {
 cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, const double* xi, const double* w,
                               int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st)
 {
-    cudaError_t err = cudaMemcpyToSymbolAsync(c_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) return err;
-    err = cudaMemcpyToSymbolAsync(c_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) return err;
+    // the rule's nodes and weights live in constant memory; they are uploaded again only when the
+    // order, the stream or the device changes (a constant table, not a result)
+    static int up_n = -1, up_dev = -1;
+    static cudaStream_t up_st = nullptr;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaError_t err = cudaSuccess;
+    if (up_n != n_quad || up_st != st || up_dev != dev) {
+        err = cudaMemcpyToSymbolAsync(c_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
+        if (err != cudaSuccess) return err;
+        err = cudaMemcpyToSymbolAsync(c_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
+        if (err != cudaSuccess) return err;
+        up_n = n_quad; up_st = st; up_dev = dev;
+    }
     if (nnz_geo == 0) return cudaSuccess;
     // lanes per element: whole phi-nodes per lane, no idle lanes when n is a multiple of LPE
     int lpe = (n_quad % 8 == 0) ? 8 : (n_quad % 4 == 0) ? 4 : (n_quad % 2 == 0) ? 2 : 1;

@@ -288,23 +288,34 @@ __device__ __forceinline__ void slab_to_smem(unsigned char* dst, const unsigned 
 struct TileLane {
     bool valid;
     int grp, cnt, pos, gcol;
-    const double* mrow;     // moments of this tile, [mu][32], offset by the lane
+    const double* stage;    // this warp's staged class block, [m][32], offset by the lane
 };
+
+// Asynchronous copy (cp.async, 8 bytes per lane and monomial) of one class block of a tile's moment
+// row into the warp's staging buffer: it flies while the previous class is being contracted.
+__device__ __forceinline__ void stage_class(const wpcd_class_desc& d, const unsigned char* slab, const double* mrow_lane,
+                                            double* stage_lane)
+{
+    const int4* idx = reinterpret_cast<const int4*>(slab + d.idx_off);
+    uint32_t dst = smem_u32(stage_lane);
+    const int quads = d.nm >> 2;
+#pragma unroll 2
+    for (int m = 0; m < quads; ++m, dst += 1024) {
+        const int4 i4 = idx[m];
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(mrow_lane + i4.x * 32) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 256), "l"(mrow_lane + i4.y * 32) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 512), "l"(mrow_lane + i4.z * 32) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 768), "l"(mrow_lane + i4.w * 32) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
 
 // All pairs of one class for the 32 elements of a warp tile.  NM = padded monomial count.
 template <int NM>
 __device__ __forceinline__ void contract_class(const wpcd_class_desc& d, const unsigned char* slab, const TileLane& tl,
-                                               int64_t nnz_geo, int n_geo, int32_t* __restrict__ col_idx,
-                                               double* __restrict__ values)
+                                               const double (&M)[NM], int64_t nnz_geo, int n_geo,
+                                               int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
-    double M[NM];
-    const int4* idx = reinterpret_cast<const int4*>(slab + d.idx_off);
-#pragma unroll
-    for (int m = 0; m < NM / 4; ++m) {
-        const int4 i4 = idx[m];
-        M[4 * m] = __ldg(tl.mrow + i4.x * 32); M[4 * m + 1] = __ldg(tl.mrow + i4.y * 32);
-        M[4 * m + 2] = __ldg(tl.mrow + i4.z * 32); M[4 * m + 3] = __ldg(tl.mrow + i4.w * 32);
-    }
     const bool add = (d.flags & 1) != 0;
     const int4* meta = reinterpret_cast<const int4*>(slab + d.meta_off);
     const double2* G = reinterpret_cast<const double2*>(slab + d.g_off);
@@ -346,7 +357,8 @@ __global__ void __launch_bounds__(CT_THREADS, 2)
 contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, const int32_t* __restrict__ geo_col,
                 const int32_t* __restrict__ geo_row, const int32_t* __restrict__ geo_row_ptr,
                 const double* __restrict__ moments, int n_mu, const unsigned char* __restrict__ slab_blob,
-                const int4* __restrict__ slab_tab, int n_slabs, int32_t* __restrict__ col_idx, double* __restrict__ values)
+                const int4* __restrict__ slab_tab, int n_slabs, int stage_off, int32_t* __restrict__ col_idx,
+                double* __restrict__ values)
 {
     extern __shared__ __align__(128) unsigned char slab[];
     __shared__ __align__(8) uint64_t mbar;
@@ -359,7 +371,11 @@ contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, cons
     const wpcd_class_desc* desc = reinterpret_cast<const wpcd_class_desc*>(slab + sizeof(wpcd_slab_header));
     const int64_t n_tiles = (e_end - e_begin + 31) / 32;
     const int64_t warps_here = (int64_t)st.w * CT_WARPS;
-    for (int64_t tile = (int64_t)((int)blockIdx.x - st.z) * CT_WARPS + warp; tile < n_tiles; tile += warps_here) {
+    // staging buffers behind the slab: [warp][32 monomials][32 lanes]
+    double* stage_lane = reinterpret_cast<double*>(slab + stage_off) + (size_t)warp * (WPCD_MAX_NM * 32) + lane;
+    int64_t tile = (int64_t)((int)blockIdx.x - st.z) * CT_WARPS + warp;
+    if (tile < n_tiles && n_classes > 0) stage_class(desc[0], slab, moments + (size_t)tile * n_mu * 32 + lane, stage_lane);
+    for (; tile < n_tiles; tile += warps_here) {
         const int64_t e = e_begin + tile * 32 + lane;
         TileLane tl;
         tl.valid = e < e_end;
@@ -369,27 +385,35 @@ contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, cons
         tl.grp = geo_row_ptr[r];
         tl.cnt = geo_row_ptr[r + 1] - tl.grp;
         tl.pos = (int)(ec - tl.grp);
-        tl.mrow = moments + (size_t)tile * n_mu * 32 + lane;
+        tl.stage = stage_lane;
+        const double* mrow_lane = moments + (size_t)tile * n_mu * 32 + lane;
         for (int ci = 0; ci < n_classes; ++ci) {
             const wpcd_class_desc d = desc[ci];
-            if (ci + 1 < n_classes) {       // pull the next class's moment lines towards the SM while this one computes
-                const wpcd_class_desc dn = desc[ci + 1];
-                if (lane < dn.nm) {
-                    const double* nxt = tl.mrow - lane + (size_t)reinterpret_cast<const int32_t*>(slab + dn.idx_off)[lane] * 32;
-                    asm volatile("prefetch.global.L1 [%0];" ::"l"(nxt));
-                    asm volatile("prefetch.global.L1 [%0];" ::"l"(nxt + 16));
-                }
-            }
+            // the block of class ci has been copied to the staging buffer: move it to registers, then let
+            // the copy of the next block (next class, or first class of this warp's next tile) fly
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();
+#define WPCD_CT(NMV)                                                                                              \
+    {                                                                                                             \
+        double M[NMV];                                                                                            \
+        _Pragma("unroll") for (int m = 0; m < NMV; ++m) M[m] = stage_lane[m * 32];                                \
+        __syncwarp();                                                                                             \
+        if (ci + 1 < n_classes) stage_class(desc[ci + 1], slab, mrow_lane, stage_lane);                           \
+        else if (tile + warps_here < n_tiles)                                                                     \
+            stage_class(desc[0], slab, moments + (size_t)(tile + warps_here) * n_mu * 32 + lane, stage_lane);      \
+        contract_class<NMV>(d, slab, tl, M, nnz_geo, n_geo, col_idx, values);                                     \
+    }
             switch (d.nm) {
-            case 4: contract_class<4>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            case 8: contract_class<8>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            case 12: contract_class<12>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            case 16: contract_class<16>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            case 20: contract_class<20>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            case 24: contract_class<24>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            case 28: contract_class<28>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
-            default: contract_class<32>(d, slab, tl, nnz_geo, n_geo, col_idx, values); break;
+            case 4: WPCD_CT(4) break;
+            case 8: WPCD_CT(8) break;
+            case 12: WPCD_CT(12) break;
+            case 16: WPCD_CT(16) break;
+            case 20: WPCD_CT(20) break;
+            case 24: WPCD_CT(24) break;
+            case 28: WPCD_CT(28) break;
+            default: WPCD_CT(32) break;
             }
+#undef WPCD_CT
         }
     }
 }
@@ -402,10 +426,19 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
                                 int64_t nnz_geo, const Workspace& ws, const int64_t* /*row_ptr*/, const int32_t* geo_row_ptr,
                                 int32_t* col_idx, double* values, cudaStream_t st)
 {
-    cudaError_t err = cudaMemcpyToSymbolAsync(k_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) return err;
-    err = cudaMemcpyToSymbolAsync(k_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) return err;
+    static int up_n = -1, up_dev = -1;      // constant tables are uploaded again only when order, stream or device change
+    static cudaStream_t up_st = nullptr;
+    int cur_dev = 0;
+    cudaGetDevice(&cur_dev);
+    cudaError_t err = cudaSuccess;
+    const bool upload_consts = up_n != n_quad || up_st != st || up_dev != cur_dev;
+    if (upload_consts) {
+        err = cudaMemcpyToSymbolAsync(k_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
+        if (err != cudaSuccess) return err;
+        err = cudaMemcpyToSymbolAsync(k_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
+        if (err != cudaSuccess) return err;
+        up_n = n_quad; up_st = st; up_dev = cur_dev;
+    }
     if (nnz_geo == 0 || ch->n_pairs == 0) return cudaSuccess;
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
@@ -416,7 +449,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.n_ab = ch->n_ab;
     sh.n_ll = ch->n_ll; sh.n_trip = ch->n_trip; sh.n_mu = ch->n_mu;
     if ((sh.SP - 4) * sh.IS >= 65536) return cudaErrorInvalidValue;
-    {
+    if (upload_consts) {
         double invk[WPCD_MAX_K + 2];
         invk[0] = 0.0;
         for (int k = 1; k < WPCD_MAX_K + 2; ++k) invk[k] = 1.0 / k;
@@ -427,7 +460,9 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     size_t ct_smem = 0;
     double cost_sum = 0.0;
     for (auto& sl : ch->slabs) { ct_smem = std::max(ct_smem, sl.bytes); cost_sum += sl.cost; }
-    if (ct_smem > 200 * 1024 || mom_smem > 227 * 1024) return cudaErrorInvalidValue;
+    const int stage_off = (int)((ct_smem + 127) & ~(size_t)127);
+    ct_smem = (size_t)stage_off + sizeof(double) * CT_WARPS * WPCD_MAX_NM * 32;
+    if (ct_smem > 227 * 1024 || mom_smem > 227 * 1024) return cudaErrorInvalidValue;
     // CTAs per slab in proportion to its cost, two CTAs per SM per pass
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
@@ -484,7 +519,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
                 contract_kernel<<<pass_ctas[pass], CT_THREADS, ct_smem, st>>>(e0, e1, nnz_geo, n_geo, ws.geo_col, ws.geo_row, geo_row_ptr,
                                                                               ws.moments, ch->n_mu, ch->slab_blob_dev,
                                                                               tab_dev + pass_first[pass],
-                                                                              pass_first[pass + 1] - pass_first[pass], col_idx, values);
+                                                                              pass_first[pass + 1] - pass_first[pass], stage_off, col_idx, values);
                 ++g_launches;
                 if ((err = cudaGetLastError()) != cudaSuccess) return err;
             }

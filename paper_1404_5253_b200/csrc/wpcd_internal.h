@@ -39,7 +39,7 @@ struct wpcd_grid {
 struct wpcd_slab_header { int32_t n_classes, pad0, pad1, pad2; };
 struct wpcd_class_desc { int32_t idx_off, nm, n_pairs, meta_off, g_off, flags, pad1, pad2; };   // offsets in bytes from the slab start; idx = positions in the moment row; flags bit 0: add to the stored value
 struct wpcd_pair_meta { int32_t chan_off, ncoup, ci, gammap; };   // row-block offset, #coupled of gamma, rank of gamma', gamma'
-constexpr size_t WPCD_SLAB_BYTES = 100 * 1024;
+constexpr size_t WPCD_SLAB_BYTES = 46 * 1024;   // + 64 KB of staging buffers per CTA: two CTAs per SM
 constexpr int WPCD_MAX_NM = 32;          // monomials per class the register kernel handles
 
 struct wpcd_slab { size_t offset, bytes; int n_classes; double cost; int pass; };

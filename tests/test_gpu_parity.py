@@ -267,3 +267,38 @@ def test_cfg5_largest_sampled(wpcd):
     m, worst = _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, 7, -1), tab,
                                 np.arange(5, wl.n_bins ** 2, 2503))
     assert m.nnz > 2_000_000_000
+
+
+def test_coupled_wide_classes_from_table(wpcd):
+    """A user table whose (l,l') = (5,5) pair uses far more than 32 distinct (k, A) monomials: the
+    contraction cuts such a class into pieces handled in successive passes (store, then add)."""
+    rng = np.random.default_rng(20140521)
+    chan_l = [5, 2, 0]
+    pairs = []
+    for ga in range(3):
+        for gb in range(3):
+            if (ga, gb) == (2, 1):
+                continue                      # one uncoupled pair
+            l, lp = chan_l[ga], chan_l[gb]
+            terms = [(k, l1, l1p, float(rng.uniform(-1, 1)))
+                     for l1 in range(l + 1) for l1p in range(lp + 1) for k in range(0, 8)]
+            pairs.append((ga, gb, terms))
+    chs = [(l, 0, 0, 0, 0, 0) for l in chan_l]
+    tab = operm.PairTable(chs, pairs)
+    n_mono = len({(t[1] + t[2], t[0]) for t in pairs[0][2]})
+    assert n_mono > 64                        # (5,5): A = 0..10, k = 0..7 -> 88 monomials, 3 passes
+    gch = wpcd.wpcd_channels_create_from_table(np.array(chan_l), tab.gamma, tab.gammap, tab.term_ptr,
+                                               tab.term_k, tab.term_l1, tab.term_l1p, tab.term_g)
+    p = wi.tan2_grid(4, 1.0, 0.1, seed=41)
+    q = wi.tan2_grid(5, 0.7, 0.1, seed=42)
+    _compare_full(wpcd, p, q, 6, gch, tab)
+
+
+@pytest.mark.parametrize("n_quad", [1, 5, 8, 16, 33, 64])
+def test_coupled_quadrature_orders(wpcd, n_quad):
+    # phi-node groups, masked MMA rows (n not a multiple of 4), n > 32 lanes
+    chs = och.enumerate_channels(3, -1, 2)
+    tab = operm.PairTable(chs, och.g_table(chs, 3, 1))
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=-1, two_T=1, j_pair_max=2)
+    p = wi.tan2_grid(4, 1.0, 0.1, seed=51)
+    _compare_full(wpcd, p, p, n_quad, gch, tab)

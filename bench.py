@@ -23,6 +23,14 @@ sys.path.insert(0, ROOT)
 
 import wpcd_inputs as wi  # noqa: E402
 
+# DRAM bytes per launch of the dominant kernel from one `ncu --set full` capture (dram__bytes_read.sum +
+# dram__bytes_write.sum), profiles/r01g_ncu_full.md; null where no capture of that workload exists.
+NCU_TRAFFIC = {
+    ("cfg2", "spmv"): 3.59e6,            # spmv_kernel<32,1>, 3.4 MB matrix (L2-resident after the first product)
+    ("cfg2", "fill_swave"): 6.88e6,
+    ("cfg4", "spmv"): 6.29e9,            # J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
+}
+
 METRIC = "P-matrix nonzeros/sec (FP64 build + the workload's P*vector SpMVs per step)"
 UNIT = "nnz/s"
 FLOPS_PER_NODE = 70.0          # algorithmic FP64 flops per (phi,x) quadrature node, s-wave
@@ -113,7 +121,7 @@ def oracle_pass(wl, tabs, row_stride):
     rows = np.arange(0, n_geo, row_stride)
     done = 0
     for tab in tabs:
-        if wl.model == "swave" and row_stride == 1:
+        if wl.model == "swave":
             rp, ci, v, _ = operm.build_csr(p, p, wl.n_quad, tab, geo=geo)
             done += len(v)
             for k in range(wl.n_spmv):
@@ -130,7 +138,8 @@ def oracle_pass(wl, tabs, row_stride):
 
 
 def reference_row_stride(wl):
-    return 1 if wl.model == "swave" else (16 if wl.name == "cfg3" else 256)
+    # bounded oracle sample, sized for roughly 5-30 s of CPU work on a 16-core host
+    return {"cfg1": 1, "cfg2": 1, "cfg3": 1, "cfg4": 24, "cfg5": 64}[wl.name]
 
 
 def run_reference(args):
@@ -384,6 +393,8 @@ def run_ours(args):
     share["spmv_sweep"] = spmv_ms / steps
     dominant = max(share, key=share.get)
     key = {"fill_swave": "fill_swave", "moments": "fill_coupled", "contract": "fill_coupled", "spmv_sweep": "spmv"}.get(dominant)
+    for name, rf in roofs.items():
+        rf["traffic"] = NCU_TRAFFIC.get((wl.name, name))
     roofline = dict(roofs[key]) if key in roofs else {
         "bound": "alu", "achieved": None, "peak": fp64_peak / 1e12, "unit": "TFLOP/s", "frac": None, "traffic": None}
     roofline["kernel"] = dominant

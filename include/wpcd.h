@@ -111,23 +111,32 @@ int64_t wpcd_geo_rows(const wpcd_grid* grid);
  *   geo_row_ptr_dev [n_p*n_q + 1] int32 dev, out: CSR row pointer of the geometric pattern
  *   row_ptr_dev     [rows + 1]    int64 dev, out: CSR row pointer of P0
  *   nnz_out, nnz_geo_out          host, out
+ * The pass evaluates the predicate once and keeps its verdicts (one slot per candidate cell pair) in
+ * scratch memory owned by the GRID handle, for the wpcd_perm_build that follows; the handle grows that
+ * scratch on demand (a first call on a large lattice may run the pass twice).
  * Synchronises the stream once. */
 wpcd_status wpcd_perm_count(const wpcd_grid* grid, const wpcd_channels* channels, int n_quad, void* cuda_stream,
                             int64_t* row_ptr_dev, int32_t* geo_row_ptr_dev, int64_t* nnz_out, int64_t* nnz_geo_out);
 
 /* Scratch needed by wpcd_perm_build for a pattern with nnz_geo geometric entries
  * (geometric column / row / phi-range lists, and for coupled channels a block of monomial
- * moments).  0 on invalid arguments. */
+ * moments of at most 256 MiB plus a small launch table).  0 on invalid arguments. */
 size_t wpcd_perm_workspace_bytes(const wpcd_channels* channels, int64_t nnz_geo);
 
 /* Steps 2b+3 (l.312): column indices and values.
- *   row_ptr_dev, geo_row_ptr_dev   as written by wpcd_perm_count for the same arguments
+ *   row_ptr_dev, geo_row_ptr_dev   as written by wpcd_perm_count for the same arguments.  The verdicts staged
+ *                                  in the grid handle by the last wpcd_perm_count on it are consumed here (the
+ *                                  geometric pattern depends on the grid only, so any channel set may follow any
+ *                                  count on the same grid); a handle that has not been counted yet runs the
+ *                                  selection itself first (and then synchronises the stream once)
  *   workspace_dev                  >= wpcd_perm_workspace_bytes(channels, nnz_geo) bytes, dev, 256-byte aligned
  *   col_idx_dev [nnz] int32, values_dev [nnz] double: dev, out
  * Value = (d_i dbar_j d_i' dbar_j')^{-1/2} * double integral (A15) of F (A14) times the
  * channel-pair sum (A3), by the rule R(n_quad) of DESIGN.md R7: n_quad-point Gauss-Legendre
  * in phi over the angular extent of the overlap polygon, and at every phi-node n_quad-point
  * Gauss-Legendre in x over the closed-form support of F.  1 <= n_quad <= WPCD_MAX_QUAD.
+ * Coupled channels: a channel pair may use any number of (k, l1+l1') monomials (more than 32 are
+ * handled in several passes); WPCD_ERR_CUDA "invalid argument" if the tables exceed shared memory.
  * Asynchronous on the stream. */
 wpcd_status wpcd_perm_build(const wpcd_grid* grid, const wpcd_channels* channels, int n_quad, void* cuda_stream,
                             const int64_t* row_ptr_dev, const int32_t* geo_row_ptr_dev,
@@ -158,9 +167,9 @@ wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out);
  * the last read into ms_out[WPCD_TRACE_STAGES] (host) and the launch counts into
  * launches_out[WPCD_TRACE_STAGES] (host, may be NULL), then clears the record. */
 #define WPCD_TRACE_STAGES 6
-#define WPCD_STAGE_GEO_COUNT 0   /* predicate + per-row counts            (step a1) */
-#define WPCD_STAGE_SCAN 1        /* scan -> geo_row_ptr, row_ptr          (step a2) */
-#define WPCD_STAGE_GEO_INDEX 2   /* predicate + compaction of column list (step a3) */
+#define WPCD_STAGE_GEO_COUNT 0   /* predicate, per-row counts, staged verdicts, scan (steps a1, a2) */
+#define WPCD_STAGE_SCAN 1        /* geo_row_ptr -> row_ptr of the full matrix        (step a2) */
+#define WPCD_STAGE_GEO_INDEX 2   /* compaction of the staged verdicts -> column list (step a3) */
 #define WPCD_STAGE_FILL_SWAVE 3  /* single-channel quadrature fill        (step a4) */
 #define WPCD_STAGE_MOMENTS 4     /* coupled channels: monomial moments    (step a4) */
 #define WPCD_STAGE_CONTRACT 5    /* coupled channels: g-contraction+store (step a4) */

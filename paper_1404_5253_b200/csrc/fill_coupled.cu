@@ -32,7 +32,7 @@ namespace {
 __constant__ double k_xi[WPCD_MAX_QUAD];
 __constant__ double k_w[WPCD_MAX_QUAD];
 
-constexpr int MOM_WARPS = 4;
+constexpr int MOM_WARPS = 2;
 constexpr int NODE_F = 10;   // doubles per staged phi-node
 
 __constant__ double k_invk[WPCD_MAX_K + 2];   // 1/k for the Legendre recurrence
@@ -52,8 +52,8 @@ struct MomentShape {
 
 __host__ __device__ inline int moment_smem_doubles(const MomentShape& s)
 {
-    const int rows = s.G * s.n, K1P = (s.SP - 4);
-    return (s.n * NODE_F + rows * (s.SP + s.ST) + K1P * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;   // even: 16-byte pieces
+    const int rows = s.G * s.n;
+    return (s.n * NODE_F + rows * (s.SP + s.ST) + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;   // even: 16-byte pieces
 }
 
 // D (8x8) += A (8x4, row) * B (4x8, col), FP64 tensor-core MMA.  Fragment layout: a = A[lane/4][lane%4],
@@ -66,7 +66,7 @@ __device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, doubl
 // I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] for one phi-node: (K1 x n) (n x n_ll) in 8x8x4 MMAs.
 // Pg / Tg point at this lane's fragment element of x-node (lane % 4); rows r >= n read as zero.
 template <int KT>
-__device__ __forceinline__ void node_mma(const double* __restrict__ Pg, const double* __restrict__ Tg, int n, int SP, int ST,
+__device__ __forceinline__ void node_mma(const double* __restrict__ Pg, const double* __restrict__ Tg, int n, int K1, int SP, int ST,
                                          int MT, int NT, double* __restrict__ Ib, int IS, int lane)
 {
     bool live[KT];
@@ -81,7 +81,7 @@ __device__ __forceinline__ void node_mma(const double* __restrict__ Pg, const do
             double c0 = 0.0, c1 = 0.0;
 #pragma unroll
             for (int kt = 0; kt < KT; ++kt) dmma_884(c0, c1, a[kt], live[kt] ? Tg[kt * 4 * ST + nt * 8] : 0.0);
-            *reinterpret_cast<double2*>(Io + mt * 8 * IS + nt * 8) = make_double2(c0, c1);
+            if (mt * 8 + (lane >> 2) < K1) *reinterpret_cast<double2*>(Io + mt * 8 * IS + nt * 8) = make_double2(c0, c1);
         }
     }
 }
@@ -122,8 +122,8 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     double* nodeS = wbase + (size_t)warp * moment_smem_doubles(sh);   // [n][NODE_F]
     double* Pk = nodeS + n * NODE_F;                                  // [G*n][SP]    P_k(x_r)
     double* T = Pk + G * n * SP;                                      // [G*n][ST]    T_r[l,l']
-    double* Ib = T + G * n * ST;                                      // [K1P][IS]    I[k][l,l'] of one phi-node
-    double* cs = Ib + (SP - 4) * IS;                                  // [G][2][CP]   powers of cos, sin
+    double* Ib = T + G * n * ST;                                      // [K1][IS]     I[k][l,l'] of one phi-node
+    double* cs = Ib + K1 * IS;                                        // [G][2][CP]   powers of cos, sin
     double* csp = cs + G * 2 * CP;                                    // [n_ab]       c^a s^b of one phi-node
 
     // per monomial: offset into Ib (low 16 bits) and into csp (high 16 bits)
@@ -218,10 +218,10 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                 const double* Pg = Pk + (g * n + (lane & 3)) * SP + (lane >> 2);
                 const double* Tg = T + (g * n + (lane & 3)) * ST + (lane >> 2);
                 switch (KT) {
-                case 1: node_mma<1>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
-                case 2: node_mma<2>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
-                case 3: node_mma<3>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
-                case 4: node_mma<4>(Pg, Tg, n, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 1: node_mma<1>(Pg, Tg, n, K1, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 2: node_mma<2>(Pg, Tg, n, K1, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 3: node_mma<3>(Pg, Tg, n, K1, SP, ST, MT, NT, Ib, IS, lane); break;
+                case 4: node_mma<4>(Pg, Tg, n, K1, SP, ST, MT, NT, Ib, IS, lane); break;
                 default:
                     for (int mt = 0; mt < MT; ++mt)
                         for (int nt = 0; nt < NT; ++nt) {
@@ -230,7 +230,7 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                                 const bool live = kt * 4 + (lane & 3) < n;
                                 dmma_884(c0, c1, live ? Pg[kt * 4 * SP + mt * 8] : 0.0, live ? Tg[kt * 4 * ST + nt * 8] : 0.0);
                             }
-                            *reinterpret_cast<double2*>(Ib + (mt * 8 + (lane >> 2)) * IS + nt * 8 + 2 * (lane & 3)) = make_double2(c0, c1);
+                            if (mt * 8 + (lane >> 2) < K1) *reinterpret_cast<double2*>(Ib + (mt * 8 + (lane >> 2)) * IS + nt * 8 + 2 * (lane & 3)) = make_double2(c0, c1);
                         }
                     break;
                 }

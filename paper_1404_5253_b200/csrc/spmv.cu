@@ -11,7 +11,7 @@ namespace wpcd_detail { bool use_pdl(); }
 
 namespace {
 
-template <int LPR, int NV>
+template <int LPR, int NV, bool PIPE>
 __global__ void __launch_bounds__(256)
 spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
             const double* __restrict__ values, const double* __restrict__ x, double* __restrict__ y, int64_t ldx)
@@ -31,6 +31,37 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
         // batches of UNR entries per lane: all column/value loads of a batch are issued before the
         // gathers of x, so a long row costs ~2 memory latencies per batch instead of per entry
         constexpr int UNR = 8 / NV > 1 ? 8 / NV : 2;
+        if (PIPE) {
+            // long rows streamed from HBM: the index/value loads of batch b+1 are in flight while the
+            // gathers and multiply-adds of batch b run (software pipeline, two batches of registers)
+            double a[UNR], a2[UNR];
+            int c[UNR], c2[UNR];
+            int64_t e0 = beg + sub;
+#pragma unroll
+            for (int k = 0; k < UNR; ++k) {
+                const int64_t e = e0 + (int64_t)k * LPR;
+                const bool in = e < end;
+                a[k] = in ? __ldcs(values + e) : 0.0;
+                c[k] = in ? __ldcs(col_idx + e) : 0;
+            }
+            for (; e0 < end; e0 += (int64_t)UNR * LPR) {
+                const int64_t n0 = e0 + (int64_t)UNR * LPR;
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+                    const int64_t e = n0 + (int64_t)k * LPR;
+                    const bool in = e < end;
+                    a2[k] = in ? __ldcs(values + e) : 0.0;
+                    c2[k] = in ? __ldcs(col_idx + e) : 0;
+                }
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], __ldg(x + v * ldx + c[k]), acc[v]);
+                }
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) { a[k] = a2[k]; c[k] = c2[k]; }
+            }
+        } else {
         for (int64_t e0 = beg + sub; e0 < end; e0 += (int64_t)UNR * LPR) {
             double a[UNR];
             int c[UNR];
@@ -47,6 +78,7 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
                 for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], __ldg(x + v * ldx + c[k]), acc[v]);
             }
         }
+        }
     }
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
@@ -59,7 +91,7 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
     }
 }
 
-template <int LPR, int NV>
+template <int LPR, int NV, bool PIPE = false>
 cudaError_t launch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
                    double* y, cudaStream_t st)
 {
@@ -75,7 +107,7 @@ cudaError_t launch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx,
     cfg.attrs = attr;
     cfg.numAttrs = wpcd_detail::use_pdl() ? 1 : 0;
     ++wpcd_detail::g_launches;
-    return cudaLaunchKernelEx(&cfg, spmv_kernel<LPR, NV>, rows, row_ptr, col_idx, values, x, y, rows);
+    return cudaLaunchKernelEx(&cfg, spmv_kernel<LPR, NV, PIPE>, rows, row_ptr, col_idx, values, x, y, rows);
 }
 
 template <int NV>
@@ -92,6 +124,8 @@ cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_id
     if (mean_row <= 3.0) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
     if (mean_row <= 6.0) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
     if (mean_row <= 12.0) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    static const int pipe = [] { const char* e = getenv("WPCD_SPMV_PIPE"); return e ? atoi(e) : 1; }();   // tuning knob
+    if (pipe && mean_row >= 128.0) return launch<32, NV, true>(rows, row_ptr, col_idx, values, x, y, st);
     return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
 }
 

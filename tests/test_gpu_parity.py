@@ -302,3 +302,25 @@ def test_coupled_quadrature_orders(wpcd, n_quad):
     gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=-1, two_T=1, j_pair_max=2)
     p = wi.tan2_grid(4, 1.0, 0.1, seed=51)
     _compare_full(wpcd, p, p, n_quad, gch, tab)
+
+
+def test_apply_long_rows_pipelined(wpcd):
+    """Coupled matrix with mean row length >= 128: the software-pipelined SpMV variant (HBM-streaming
+    path of configs 3-5), 1, 2 and 4 right-hand sides, against the sequential oracle product."""
+    torch = _torch()
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=1, two_T=1, j_pair_max=2)
+    p = wi.tan2_grid(10, 1.0, 0.1, seed=61)
+    grid = wpcd.wpcd_grid_create(p, p)
+    m = wpcd.build_perm(grid, gch, 6)
+    rows = m.rows
+    assert m.nnz / rows >= 128
+    rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    for n_vec in (1, 2, 4, 5):
+        xh = np.stack([wi.normal_vector(rows, k=70 + k) for k in range(n_vec)])
+        x = torch.from_numpy(xh).cuda().contiguous()
+        y = torch.empty_like(x)
+        wpcd.wpcd_perm_apply(rows, m.row_ptr, m.col_idx, m.values, x, y, n_vec=n_vec)
+        for k in range(n_vec):
+            ref = operm.spmv(rp, ci, v, xh[k])
+            scale = operm.spmv(rp, ci, np.abs(v), np.abs(xh[k]))
+            assert np.all(np.abs(y[k].cpu().numpy() - ref) <= 1e-12 * scale + 1e-300)

@@ -324,3 +324,58 @@ def test_apply_long_rows_pipelined(wpcd):
             ref = operm.spmv(rp, ci, v, xh[k])
             scale = operm.spmv(rp, ci, np.abs(v), np.abs(xh[k]))
             assert np.all(np.abs(y[k].cpu().numpy() - ref) <= 1e-12 * scale + 1e-300)
+
+
+def test_full_size_properties_cfg2_and_cfg3(wpcd):
+    """Properties that hold at any size, checked on the GPU result at full size: the matrix of the
+    Hermitian operator P in a real basis is symmetric (pattern exactly, values to rounding), the
+    columns ascend strictly inside every row, and the spectrum of the s-wave matrix g0*P lies in
+    [-g0, 2 g0] (checked through its largest eigenvalue by power iteration with the CUDA SpMV)."""
+    torch = _torch()
+    import scipy.sparse as sp
+
+    wl = wi.WORKLOADS["cfg2"]
+    p = wl.grid()
+    grid = wpcd.wpcd_grid_create(p, p)
+    m = wpcd.build_perm(grid, _gpu_channels(wpcd, wl), wl.n_quad)
+    rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    assert np.all(np.diff(rp) >= 0)
+    inner = np.ones(len(ci), bool)
+    inner[rp[:-1][np.diff(rp) > 0]] = False                 # first entry of every non-empty row
+    assert np.all(np.diff(ci)[inner[1:]] > 0)               # strictly ascending inside rows
+    A = sp.csr_matrix((v, ci, rp), shape=(m.rows, m.rows))
+    D = (A - A.T).tocsr()
+    assert D.nnz == 0 or np.abs(D.data).max() <= 1e-12 * np.abs(v).max()
+    assert (A != 0).astype(np.int8).nnz == ((A + A.T) != 0).astype(np.int8).nnz      # symmetric pattern
+    x = torch.from_numpy(wi.normal_vector(m.rows, k=5)).cuda()
+    y = torch.empty_like(x)
+    lam = 0.0
+    for _ in range(60):
+        wpcd.wpcd_perm_apply(m.rows, m.row_ptr, m.col_idx, m.values, x, y)
+        lam = float(torch.dot(x, y) / torch.dot(x, x))
+        x = y / torch.linalg.norm(y)
+    assert -wl.g0 - 1e-9 <= lam <= 2.0 * wl.g0 + 1e-9 and lam > 0.9 * wl.g0      # top of the spectrum ~ g0 * 2... of the s-wave block ~ g0
+    # cfg3 (18 channels): full pattern symmetry from the row pointer and a symmetric-value sample
+    wl3 = wi.WORKLOADS["cfg3"]
+    p3 = wl3.grid()
+    grid3 = wpcd.wpcd_grid_create(p3, p3)
+    m3 = wpcd.build_perm(grid3, _gpu_channels(wpcd, wl3, 1, 1), wl3.n_quad)
+    rp3 = m3.row_ptr.cpu().numpy()
+    rng = np.random.default_rng(7)
+    rows = rng.integers(0, m3.rows, 200)
+    # values are symmetric up to the rounding of rule R(n), which on cells touching p = 0 or p' = 0 is
+    # amplified by the cancellation between the (k,l1,l1') terms (DESIGN.md R8, R9): absolute scale
+    vmax = float(m3.values.abs().max().item())
+    for r in rows:
+        lo, hi = rp3[r], rp3[r + 1]
+        if hi == lo:
+            continue
+        k = int(rng.integers(lo, hi))
+        c = int(m3.col_idx[k].item())
+        val = float(m3.values[k].item())
+        cl, ch = rp3[c], rp3[c + 1]
+        cols_c = m3.col_idx[cl:ch].cpu().numpy()
+        pos = np.searchsorted(cols_c, r)
+        assert pos < len(cols_c) and cols_c[pos] == r                      # (c, r) is stored too
+        vt = float(m3.values[cl + pos].item())
+        assert abs(vt - val) <= 1e-10 * abs(val) + 1e-6 * vmax

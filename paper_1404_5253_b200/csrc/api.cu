@@ -170,6 +170,7 @@ static wpcd_status finalize_channels(wpcd_channels* c)
         if (pidx > 0 && std::make_pair(c->pair_gamma[pidx - 1], c->pair_gammap[pidx - 1]) >= std::make_pair(ga, gb))
             return fail(WPCD_ERR_INVALID_ARG, "pairs must be sorted ascending by (gamma, gamma') without repeats");
         if (c->term_ptr[pidx + 1] < c->term_ptr[pidx]) return fail(WPCD_ERR_INVALID_ARG, "term_ptr not monotone");
+        if (c->term_ptr[pidx + 1] == c->term_ptr[pidx]) return fail(WPCD_ERR_INVALID_ARG, "a listed channel pair has no terms (leave uncoupled pairs out)");
     }
     // ---- merged coefficients per pair, monomial (A, k) = (l1 + l1', k)
     c->k_max = 0; c->l_max = 0;

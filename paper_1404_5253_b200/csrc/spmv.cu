@@ -30,7 +30,7 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
         const int64_t beg = row_ptr[row], end = row_ptr[row + 1];
         // batches of UNR entries per lane: all column/value loads of a batch are issued before the
         // gathers of x, so a long row costs ~2 memory latencies per batch instead of per entry
-        constexpr int UNR = 8 / NV > 1 ? 8 / NV : 2;
+        constexpr int UNR = NV == 1 ? 8 : 4;
         if (PIPE) {
             // long rows streamed from HBM: the index/value loads of batch b+1 are in flight while the
             // gathers and multiply-adds of batch b run (software pipeline, two batches of registers)

@@ -50,6 +50,8 @@ def test_channel_argument_checks(wpcd):
         wpcd.wpcd_channels_create_from_table([0, 0], [1, 0], [0, 0], [0, 1, 2], [0, 0], [0, 0], [0, 0], [1.0, 1.0])
     with pytest.raises(wpcd.WpcdError, match="WPCD_MAX_K"):
         wpcd.wpcd_channels_create_from_table([0], [0], [0], [0, 1], [99], [0], [0], [1.0])
+    with pytest.raises(wpcd.WpcdError, match="no terms"):
+        wpcd.wpcd_channels_create_from_table([0, 0], [0, 1], [0, 1], [0, 1, 1], [0], [0], [0], [1.0])
 
 
 @pytest.mark.parametrize("two_J,parity,jmax", [(1, 1, 2), (1, -1, 2), (3, 1, 2), (5, -1, 3)])

@@ -346,6 +346,19 @@ def run_ours(args):
         ms4 = a.elapsed_time(b) / reps
         spmm = {"n_vec": 4, "ms_per_pass": ms4, "products_per_s": 4.0 / (ms4 * 1e-3),
                 "matrix_GBps": (12.0 * job.nnz + 8.0 * job.rows) / (ms4 * 1e-3) / 1e9, "nnz": job.nnz}
+        # complex right-hand side (the transition operator is complex): one 16-byte gather, two FMAs per entry
+        xc = torch.complex(x4[0], x4[1]).contiguous()
+        yc = torch.empty_like(xc)
+        for _ in range(3):
+            wpcd.wpcd_perm_apply_complex(job.rows, job.row_ptr, job.col_idx, job.values, xc, yc)
+        a.record()
+        for _ in range(reps):
+            wpcd.wpcd_perm_apply_complex(job.rows, job.row_ptr, job.col_idx, job.values, xc, yc)
+        b.record()
+        torch.cuda.synchronize()
+        msc = a.elapsed_time(b) / reps
+        spmm["complex_ms_per_product"] = msc
+        spmm["complex_matrix_GBps"] = (12.0 * job.nnz + 8.0 * job.rows) / (msc * 1e-3) / 1e9
 
     # ---- end to end through the C-ABI with HOST buffers (handles, tables and vectors from the host)
     def e2e_step():

@@ -149,6 +149,14 @@ wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int3
                             const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
                             void* cuda_stream);
 
+/* y = P0 x for n_vec COMPLEX vectors (the transition operator is complex, P0 is real;
+ * next step of SURVEY.md section 8(f)): x_dev / y_dev hold interleaved (re, im) doubles,
+ * x_dev[2 * (v*rows + c)], 16-byte aligned, dev.  One 16-byte gather and two multiply-adds per entry.
+ * Asynchronous. */
+wpcd_status wpcd_perm_apply_complex(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                                    const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
+                                    void* cuda_stream);
+
 /* Same product with HOST vectors: copies x_host -> x_dev (scratch, dev, n_vec*rows doubles),
  * applies, copies y_dev (scratch) -> y_host, all on the stream, then synchronises it.
  * Pinned host memory makes the copies asynchronous. */

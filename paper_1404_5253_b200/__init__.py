@@ -9,7 +9,7 @@ present, compute calls raise ``WpcdError``.
 Function names mirror the C-ABI (PAPER.md citations live in include/wpcd.h):
     wpcd_grid_create, wpcd_channels_create, wpcd_channels_create_from_table,
     wpcd_perm_count, wpcd_perm_workspace_bytes, wpcd_perm_build, wpcd_perm_apply,
-    wpcd_perm_apply_host, wpcd_fp64_peak, wpcd_launch_count.
+    wpcd_perm_apply_host, wpcd_perm_apply_complex, wpcd_fp64_peak, wpcd_launch_count.
 ``build_perm`` strings count -> allocate -> build together and returns a ``PermCSR``.
 """
 import ctypes
@@ -30,7 +30,7 @@ EXPORTS = [
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
+    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
 
@@ -76,6 +76,7 @@ def load():
     L.wpcd_perm_build.argtypes = [vp, vp, i32, vp, vp, vp, vp, sz, vp, vp]
     L.wpcd_perm_apply.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_host.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp, vp, vp]
+    L.wpcd_perm_apply_complex.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_fp64_peak.argtypes = [vp, ctypes.POINTER(dbl)]
     L.wpcd_launch_count.restype = i64
     L.wpcd_trace_enable.argtypes = [i32]
@@ -215,6 +216,15 @@ def wpcd_perm_apply(rows, row_ptr, col_idx, values, x, y, n_vec=1, stream=None):
     _check(load().wpcd_perm_apply(rows, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
                                   _dev_ptr(values, torch.float64), _dev_ptr(x, torch.float64), _dev_ptr(y, torch.float64),
                                   n_vec, _stream_ptr(stream)))
+
+
+def wpcd_perm_apply_complex(rows, row_ptr, col_idx, values, x, y, n_vec=1, stream=None):
+    """x, y: complex128 CUDA tensors [n_vec, rows] (interleaved re/im in memory)."""
+    import torch
+
+    assert x.dtype == torch.complex128 and y.dtype == torch.complex128
+    _check(load().wpcd_perm_apply_complex(rows, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
+                                          _dev_ptr(values, torch.float64), _dev_ptr(x), _dev_ptr(y), n_vec, _stream_ptr(stream)))
 
 
 def wpcd_perm_apply_host(rows, row_ptr, col_idx, values, x_host, y_host, x_dev, y_dev, n_vec=1, stream=None):

@@ -129,6 +129,91 @@ cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_id
     return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
 }
 
+// ---------------------------------------------------------------- complex right-hand side
+// y = P0 x for one complex vector stored interleaved (re, im): P0 is real, so an entry costs one 16-byte
+// gather and two multiply-adds (the transition operator of eq. 12 is complex).
+template <int LPR, bool PIPE>
+__global__ void __launch_bounds__(256)
+spmv_complex_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+                    const double* __restrict__ values, const double2* __restrict__ x, double2* __restrict__ y)
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t row = t / LPR;
+    const int sub = (int)(t - row * LPR);
+    double re = 0.0, im = 0.0;
+    if (row < rows) {
+        const int64_t beg = row_ptr[row], end = row_ptr[row + 1];
+        constexpr int UNR = 4;
+        double a[UNR], a2[UNR];
+        int c[UNR], c2[UNR];
+        int64_t e0 = beg + sub;
+#pragma unroll
+        for (int k = 0; k < UNR; ++k) {
+            const int64_t e = e0 + (int64_t)k * LPR;
+            const bool in = e < end;
+            a[k] = in ? values[e] : 0.0;
+            c[k] = in ? col_idx[e] : 0;
+        }
+        for (; e0 < end; e0 += (int64_t)UNR * LPR) {
+            if (PIPE) {
+                const int64_t n0 = e0 + (int64_t)UNR * LPR;
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+                    const int64_t e = n0 + (int64_t)k * LPR;
+                    const bool in = e < end;
+                    a2[k] = in ? __ldcs(values + e) : 0.0;
+                    c2[k] = in ? __ldcs(col_idx + e) : 0;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < UNR; ++k) {
+                const double2 xv = __ldg(x + c[k]);
+                re = fma(a[k], xv.x, re);
+                im = fma(a[k], xv.y, im);
+            }
+            if (PIPE) {
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) { a[k] = a2[k]; c[k] = c2[k]; }
+            } else {
+                const int64_t n0 = e0 + (int64_t)UNR * LPR;
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+                    const int64_t e = n0 + (int64_t)k * LPR;
+                    const bool in = e < end;
+                    a[k] = in ? values[e] : 0.0;
+                    c[k] = in ? col_idx[e] : 0;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int o = LPR / 2; o > 0; o >>= 1) {
+        re += __shfl_xor_sync(0xffffffffu, re, o);
+        im += __shfl_xor_sync(0xffffffffu, im, o);
+    }
+    if (row < rows && sub == 0) y[row] = make_double2(re, im);
+}
+
+template <int LPR, bool PIPE>
+cudaError_t launch_complex(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+                           const double2* x, double2* y, cudaStream_t st)
+{
+    int64_t blocks = (rows * LPR + 255) / 256;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = wpcd_detail::use_pdl() ? 1 : 0;
+    ++wpcd_detail::g_launches;
+    return cudaLaunchKernelEx(&cfg, spmv_complex_kernel<LPR, PIPE>, rows, row_ptr, col_idx, values, x, y);
+}
+
 // ---------------------------------------------------------------- FP64 FMA peak
 __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double seed)
 {
@@ -163,6 +248,22 @@ cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col
         if (n_vec - v >= 4) { err = dispatch<4>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 4; }
         else if (n_vec - v >= 2) { err = dispatch<2>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 2; }
         else { err = dispatch<1>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 1; }
+        if (err != cudaSuccess) return err;
+    }
+    return cudaSuccess;
+}
+
+cudaError_t launch_spmv_complex(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+                                const double* x, double* y, int n_vec, double mean_row, cudaStream_t st)
+{
+    for (int v = 0; v < n_vec; ++v) {
+        const double2* xv = reinterpret_cast<const double2*>(x) + (int64_t)v * rows;
+        double2* yv = reinterpret_cast<double2*>(y) + (int64_t)v * rows;
+        cudaError_t err;
+        if (mean_row <= 6.0) err = launch_complex<8, false>(rows, row_ptr, col_idx, values, xv, yv, st);
+        else if (mean_row <= 12.0) err = launch_complex<16, false>(rows, row_ptr, col_idx, values, xv, yv, st);
+        else if (mean_row >= 128.0) err = launch_complex<32, true>(rows, row_ptr, col_idx, values, xv, yv, st);
+        else err = launch_complex<32, false>(rows, row_ptr, col_idx, values, xv, yv, st);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;

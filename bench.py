@@ -24,11 +24,11 @@ sys.path.insert(0, ROOT)
 import wpcd_inputs as wi  # noqa: E402
 
 # DRAM bytes per launch of the dominant kernel from one `ncu --set full` capture (dram__bytes_read.sum +
-# dram__bytes_write.sum), profiles/r01g_ncu_full.md; null where no capture of that workload exists.
+# dram__bytes_write.sum), profiles/r01h_ncu_full.md; null where no capture of that workload exists.
 NCU_TRAFFIC = {
     ("cfg2", "spmv"): 3.59e6,            # spmv_kernel<32,1>, 3.4 MB matrix (L2-resident after the first product)
     ("cfg2", "fill_swave"): 6.88e6,
-    ("cfg4", "spmv"): 6.29e9,            # J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
+    ("cfg4", "spmv"): 6.19e9,            # J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
 }
 
 METRIC = "P-matrix nonzeros/sec (FP64 build + the workload's P*vector SpMVs per step)"

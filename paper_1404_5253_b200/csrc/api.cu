@@ -587,8 +587,20 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
     if (workspace_bytes < ws.bytes) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: workspace too small");
     cudaError_t err = launch_geo_gather(g, geo_row_ptr_dev, ws.geo_col, ws.geo_row, ws.geo_phi, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(index)");
+    // Gauss-Legendre nodes / weights: computed once per order (host, long double Newton), then reused
+    static std::mutex gl_mutex;
+    static std::map<int, std::vector<double>> gl_cache;
     double xi[WPCD_MAX_QUAD], w[WPCD_MAX_QUAD];
-    wpcd_host::gauss_legendre(n_quad, xi, w);
+    {
+        std::lock_guard<std::mutex> lock(gl_mutex);
+        std::vector<double>& tab = gl_cache[n_quad];
+        if (tab.empty()) {
+            tab.resize(2 * n_quad);
+            wpcd_host::gauss_legendre(n_quad, tab.data(), tab.data() + n_quad);
+        }
+        std::memcpy(xi, tab.data(), sizeof(double) * n_quad);
+        std::memcpy(w, tab.data() + n_quad, sizeof(double) * n_quad);
+    }
     if (c->swave_single) err = launch_fill_swave(g, c, n_quad, xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
     else err = launch_fill_coupled(g, c, n_quad, xi, w, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(fill)");

@@ -27,7 +27,8 @@
  *     alike with primed indices; columns strictly ascending inside a row.
  *   - there is no CPU fallback: without a CUDA device every compute call
  *     returns WPCD_ERR_CUDA.
- *   - a handle must not be used by two host threads at the same time.
+ *   - a handle must not be used by two host threads at the same time, and wpcd_perm_build calls must not
+ *     overlap in time on one device (threads or streams): the quadrature rule lives in constant memory.
  */
 #ifndef WPCD_H
 #define WPCD_H

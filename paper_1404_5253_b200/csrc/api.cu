@@ -143,15 +143,17 @@ static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_p
 
 static void free_channels_device(wpcd_channels* c)
 {
-    cudaFree(c->ncoupled_dev); cudaFree(c->chan_off_dev); cudaFree(c->ll_pack_dev); cudaFree(c->trip_pack_dev);
-    cudaFree(c->mu_pack_dev); cudaFree(c->ab_pack_dev); cudaFree(c->slab_blob_dev);
+    if (c->ncoupled_dev) cudaDeviceSynchronize();   // the tables go back to the buffer cache: no kernel may still read them
+    pool_free(c->ncoupled_dev); pool_free(c->chan_off_dev); pool_free(c->ll_pack_dev); pool_free(c->trip_pack_dev);
+    pool_free(c->mu_pack_dev); pool_free(c->ab_pack_dev); pool_free(c->slab_blob_dev);
 }
 
 template <class T>
 static cudaError_t upload(T** dst, const std::vector<T>& src)
 {
     size_t bytes = sizeof(T) * std::max<size_t>(src.size(), 1);
-    cudaError_t err = cudaMalloc(reinterpret_cast<void**>(dst), bytes);
+    cudaError_t err = cudaSuccess;
+    *dst = static_cast<T*>(pool_alloc(bytes, false, &err));
     if (err != cudaSuccess) return err;
     if (!src.empty()) err = cudaMemcpy(*dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice);
     return err;

@@ -10,6 +10,8 @@
 //    coupled channel pairs with the moment tile staged in shared memory (kernel contract).
 #include <math.h>
 
+#include <mutex>
+
 #include "quad_device.cuh"
 #include "wpcd_internal.h"
 
@@ -81,6 +83,8 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
 {
     // the rule's nodes and weights live in constant memory; they are uploaded again only when the
     // order, the stream or the device changes (a constant table, not a result)
+    static std::mutex up_mutex;
+    std::lock_guard<std::mutex> up_lock(up_mutex);
     static int up_n = -1, up_dev = -1;
     static cudaStream_t up_st = nullptr;
     int dev = 0;

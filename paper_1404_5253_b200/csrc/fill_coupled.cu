@@ -18,6 +18,8 @@
 //                    read from L2 a few hundred times in all and every moment exactly once.  Each
 //                    pair writes 32 consecutive CSR values + column indices per warp (coalesced).
 #include <math.h>
+
+#include <mutex>
 #include <stdlib.h>
 
 #include <algorithm>
@@ -426,6 +428,8 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
                                 int64_t nnz_geo, const Workspace& ws, const int64_t* /*row_ptr*/, const int32_t* geo_row_ptr,
                                 int32_t* col_idx, double* values, cudaStream_t st)
 {
+    static std::mutex up_mutex;
+    std::lock_guard<std::mutex> up_lock(up_mutex);
     static int up_n = -1, up_dev = -1;      // constant tables are uploaded again only when order, stream or device change
     static cudaStream_t up_st = nullptr;
     int cur_dev = 0;

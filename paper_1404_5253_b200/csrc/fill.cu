@@ -1,14 +1,11 @@
 // fill.cu -- "calculation of the nonzero elements of P0" (paper step 3):
 // FP64 Gauss-Legendre quadrature of (A15) over the clipped overlap region.
 //
-// Two paths:
-//  * s-wave (configs 1-2): one channel, one term; LPE lanes share one element, each lane
-//    owns whole phi-nodes and runs the inner x-rule; shuffles reduce.
-//  * coupled channels (configs 3-5): monomial moments
-//        M[mu] = sum_nodes w F P_k(x) cos^{A+1} sin^{B+1} / (zeta1^{l'+1} zeta2^{l+1})
-//    per geometric element (kernel moments), then value[pair] = sum_terms g M[mu] for all
-//    coupled channel pairs with the moment tile staged in shared memory (kernel contract).
+// This file: the s-wave path (configs 1-2: one channel, one term).  LPE lanes share one element,
+// each lane owns whole phi-nodes and runs the inner x-rule in squared variables (one rsqrt per
+// node); shuffles reduce.  The coupled-channel path (configs 3-5) is fill_coupled.cu.
 #include <math.h>
+#include <stdlib.h>
 
 #include <mutex>
 
@@ -105,7 +102,10 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     StageTimer timer(WPCD_STAGE_FILL_SWAVE, st);
 #define WPCD_LAUNCH_SW(L, Q) fill_swave_kernel<L, Q><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
                                                                             ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
-    if (n_quad == 8) WPCD_LAUNCH_SW(8, 8);
+    // order 8: two lanes per element once there are enough elements to fill the chip (the per-element
+    // prologue -- cell loads, normalisation -- is then paid twice instead of eight times), eight lanes otherwise
+    if (n_quad == 8 && nnz_geo >= 65536) { lpe = 2; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256); WPCD_LAUNCH_SW(2, 8); }
+    else if (n_quad == 8) WPCD_LAUNCH_SW(8, 8);
     else if (n_quad == 10) WPCD_LAUNCH_SW(2, 10);
     else switch (lpe) {
     case 8: WPCD_LAUNCH_SW(8, 0); break;

@@ -2,7 +2,10 @@
 // the iterative solution of eq. (12) (paper step 5; sparse storage PAPER.md:304).
 // HBM-bound: 12 B per nonzero streamed once, x gathered through L2.
 // LPR lanes cooperate on one row (coalesced col/value loads), chosen from the mean row
-// length; up to 4 right-hand sides share one pass over the matrix.
+// length; batches of entries per lane with every index/value load issued before the gathers;
+// a software-pipelined variant for long rows streamed from HBM; up to 4 right-hand sides share
+// one pass over the matrix; complex vectors (interleaved) cost one 16-byte gather per entry.
+// Launched with programmatic dependent launch (back-to-back products overlap launch latency).
 #include <stdlib.h>
 
 #include "wpcd_internal.h"

@@ -139,7 +139,7 @@ def oracle_pass(wl, tabs, row_stride):
 
 def reference_row_stride(wl):
     # bounded oracle sample, sized for roughly 5-30 s of CPU work on a 16-core host
-    return {"cfg1": 1, "cfg2": 1, "cfg3": 1, "cfg4": 24, "cfg5": 64}[wl.name]
+    return {"cfg1": 1, "cfg2": 1, "cfg3": 1, "cfg4": 24, "cfg5": 64, "fig4": 1}[wl.name]
 
 
 def run_reference(args):

@@ -57,6 +57,9 @@ WORKLOADS = {
     "cfg3": Workload("cfg3", 100, 8, 0.0, "nd", j_pair_max=2, jpis=[(1, +1)], n_spmv=0),
     "cfg4": Workload("cfg4", 150, 10, 0.0, "nd", j_pair_max=3, jpis=_BOTH([1, 3]), n_spmv=100),
     "cfg5": Workload("cfg5", 150, 10, 0.0, "nd", j_pair_max=3, jpis=_BOTH([1, 3, 5, 7]), n_spmv=20),
+    # extra, not a BASELINE.json config: the lattice size of the paper's own s-wave timing (M = N = 400,
+    # PAPER.md:334), same node formula, for context beside the paper's 2.3 s on a GTX-670
+    "fig4": Workload("fig4", 400, 8, 0.0, "swave", n_spmv=0),
 }
 
 

@@ -406,3 +406,64 @@ def test_apply_complex(wpcd):
                     ref = operm.spmv(rp, ci, v, src)
                     scale = operm.spmv(rp, ci, np.abs(v), np.abs(src))
                     assert np.all(np.abs(part - ref) <= 1e-12 * scale + 1e-300)
+
+
+def test_coupled_edge_grids(wpcd):
+    """Coupled channels on lattices that do not start at zero, with very uneven bins and n_p != n_q."""
+    chs = och.enumerate_channels(1, -1, 1)
+    tab = operm.PairTable(chs, och.g_table(chs, 1, 1))
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=-1, two_T=1, j_pair_max=1)
+    cases = [
+        (np.array([0.3, 0.5, 2.0]), np.array([0.1, 0.2, 0.9, 4.0])),
+        (np.array([0.0, 1e-3, 1.0, 50.0]), np.array([0.0, 2.0])),
+        (np.array([0.0, 0.37]), np.array([0.0, 0.37])),
+    ]
+    for p, q in cases:
+        _compare_full(wpcd, p, q, 7, gch, tab)
+
+
+def test_handle_state_between_count_and_build(wpcd):
+    """The selection staged in the grid handle by wpcd_perm_count serves any later wpcd_perm_build on that
+    grid (the geometric pattern does not depend on the channel set); a handle that was never counted runs
+    the selection inside wpcd_perm_build."""
+    torch = _torch()
+    p = wi.tan2_grid(7, 1.0, 0.1, seed=71)
+    q = wi.tan2_grid(6, 0.9, 0.1, seed=72)
+    chs_a = och.enumerate_channels(1, 1, 1)
+    tab_a = operm.PairTable(chs_a, och.g_table(chs_a, 1, 1))
+    ch_s, pairs_s = och.spinless_swave_table(0.5)
+    tab_s = operm.PairTable(ch_s, pairs_s)
+    g_a = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=1)
+    g_s = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    grid = wpcd.wpcd_grid_create(p, q)
+    n_geo = grid.n_p * grid.n_q
+
+    def buffers(ch):
+        rows = wpcd.wpcd_rows(grid, ch)
+        return (torch.empty(rows + 1, dtype=torch.int64, device="cuda"), torch.empty(n_geo + 1, dtype=torch.int32, device="cuda"))
+
+    rp_a, geo_a = buffers(g_a)
+    rp_s, geo_s = buffers(g_s)
+    nnz_a, nnz_geo = wpcd.wpcd_perm_count(grid, g_a, 6, rp_a, geo_a)
+    nnz_s, nnz_geo2 = wpcd.wpcd_perm_count(grid, g_s, 6, rp_s, geo_s)     # second count before the first build
+    assert nnz_geo == nnz_geo2
+    out = {}
+    for name, ch, rp, geo, nnz in (("a", g_a, rp_a, geo_a, nnz_a), ("s", g_s, rp_s, geo_s, nnz_s)):
+        ws = torch.empty(max(256, wpcd.wpcd_perm_workspace_bytes(ch, nnz_geo)), dtype=torch.uint8, device="cuda")
+        col = torch.empty(nnz, dtype=torch.int32, device="cuda")
+        val = torch.empty(nnz, dtype=torch.float64, device="cuda")
+        wpcd.wpcd_perm_build(grid, ch, 6, rp, geo, ws, col, val)
+        out[name] = (rp.cpu().numpy(), col.cpu().numpy(), val.cpu().numpy())
+    # a fresh handle on the same nodes, never counted: build must run the selection itself
+    grid2 = wpcd.wpcd_grid_create(p, q)
+    ws = torch.empty(max(256, wpcd.wpcd_perm_workspace_bytes(g_a, nnz_geo)), dtype=torch.uint8, device="cuda")
+    col2 = torch.empty(nnz_a, dtype=torch.int32, device="cuda")
+    val2 = torch.empty(nnz_a, dtype=torch.float64, device="cuda")
+    wpcd.wpcd_perm_build(grid2, g_a, 6, rp_a, geo_a, ws, col2, val2)
+    torch.cuda.synchronize()
+    assert np.array_equal(col2.cpu().numpy(), out["a"][1]) and np.array_equal(val2.cpu().numpy(), out["a"][2])
+    for name, tab in (("a", tab_a), ("s", tab_s)):
+        rp, ci, v, av = operm.build_csr(p, q, 6, tab)
+        assert np.array_equal(out[name][0], rp) and np.array_equal(out[name][1], ci)
+        tol = VALUE_RTOL * np.maximum(np.abs(v), av) + VALUE_FLOOR * np.abs(v).max()
+        assert np.all(np.abs(out[name][2] - v) <= tol)

@@ -21,8 +21,10 @@ Pins (tests/test_oracle_channels.py): 18 channels for J=1/2, j<=2
 s-wave collapse to the textbook doublet/quartet recoupling values; vanishing
 order G = O(p^l p'^l') at pi2 -> 0 / pi1 -> 0; G_{gg'}(q,q',x) = G_{g'g}(q',q,x); the
 orbital part against a brute-force overlap of bipolar spherical harmonics of the
-vectors p = q/2 + q', p' = q + q'/2 (fixes labels, powers of 1/2, the k-range).
-Parity of g with ref. [11] beyond these is UNPINNED (ref. [11] not available).
+vectors p = q/2 + q', p' = q + q'/2 (fixes labels, powers of 1/2, the k-range); and, for every factor at
+once, the spectrum of the multichannel lattice matrix, which must lie in [-1, 2] and approach both ends
+(tests/test_oracle_perm.py::test_multichannel_spectrum_bound).  Parity unpinned: only the relative PHASE
+convention between channels (a diagonal +-1 similarity of P0), which needs ref. [11]'s potential matrix.
 """
 from math import factorial, sqrt
 

@@ -239,3 +239,25 @@ def test_full_row_ptr_and_columns(nd_half_plus_j1):
             assert np.array_equal(cols, expect)
             assert np.all(np.diff(cols) > 0)
     assert not np.isnan(v).any()
+
+
+@pytest.mark.parametrize("two_J,parity,jmax", [(1, 1, 1), (3, -1, 1), (1, -1, 2)])
+def test_multichannel_spectrum_bound(two_J, parity, jmax):
+    """P = P12P23 + P13P23 is Hermitian with spectrum {-1, 2} on the states antisymmetric in the pair (l+s+t odd,
+    PAPER.md:62, 102); the lattice matrix of ANY truncated channel set is a compression of it, so its eigenvalues
+    must lie in [-1, 2] (up to the quadrature error) and the largest must approach 2 as the lattice is refined.
+    This involves every factor of (A4) at once -- spin and isospin 6j, both 9j, prefactor and the orbital part:
+    a wrong scale or a global sign leaves the interval at once (factor 2 -> 3.6; sign flip -> -1.8)."""
+    chs = channels.enumerate_channels(two_J, parity, jmax)
+    tab = perm.PairTable(chs, channels.g_table(chs, two_J, 1))
+    top = []
+    for N in (5, 7):
+        p = wi.tan2_grid(N)
+        rp, ci, v, _ = perm.build_csr(p, p, 12, tab)
+        M = _dense(rp, ci, v)
+        assert np.abs(M - M.T).max() < 1e-9
+        w = np.linalg.eigvalsh(0.5 * (M + M.T))
+        assert w[0] > -1.0 and w[-1] < 2.0
+        assert w[0] < -0.8 and w[-1] > 1.6            # both ends of the exact spectrum are being approached
+        top.append(w[-1])
+    assert top[1] > top[0]

@@ -158,6 +158,26 @@ wpcd_status wpcd_perm_apply_complex(int64_t rows, const int64_t* row_ptr_dev, co
                                     const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
                                     void* cuda_stream);
 
+/* Next step of SURVEY.md section 8(f): the kernel of eq. (12) in factored form.
+ * wpcd_block_apply: for every channel gamma, Y_gamma = A_gamma X_gamma (transpose = 0) or A_gamma^T X_gamma
+ * (transpose != 0), where X_gamma is the n_p x n_q block x_dev[(gamma*n_p + i)*n_q + j] of the vector and
+ * a_dev[(gamma*n_p + k)*n_p + i] a real matrix acting on the pair index -- the rotation O of eq. (8)/(10)
+ * or the pair interaction V1 in the scattering-wave-packet basis.  complex_vectors != 0:
+ * x, y hold interleaved (re, im).  x_dev must not alias y_dev.  Dense products on the FP64 tensor cores.
+ * Asynchronous. */
+wpcd_status wpcd_block_apply(int n_channels, int n_p, int n_q, const double* a_dev, int transpose, const double* x_dev,
+                             double* y_dev, int complex_vectors, void* cuda_stream);
+
+/* y = O ( P0 ( O^T ( V1 ( G1 .* x ) ) ) ): one application of the kernel K = P V1 G1 of eq. (12) with
+ * P = O P0 O^T (eq. 10).  o_dev, v_dev: [n_channels][n_p][n_p] real (V1 block-diagonal in the channel: the
+ * uncoupled-pair case); g1_dev: [rows] complex diagonal (the channel resolvent, analytic in
+ * the paper, an input here); x_dev, y_dev: [rows] complex; scratch_dev: 2*rows complex (4*rows doubles);
+ * all complex arrays interleaved (re, im), 16-byte aligned, dev.  CSR arrays of P0 as produced above.
+ * Asynchronous. */
+wpcd_status wpcd_kernel_apply(int n_channels, int n_p, int n_q, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                              const double* values_dev, const double* o_dev, const double* v_dev, const double* g1_dev,
+                              const double* x_dev, double* y_dev, double* scratch_dev, void* cuda_stream);
+
 /* Same product with HOST vectors: copies x_host -> x_dev (scratch, dev, n_vec*rows doubles),
  * applies, copies y_dev (scratch) -> y_host, all on the stream, then synchronises it.
  * Pinned host memory makes the copies asynchronous. */

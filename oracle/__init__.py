@@ -14,6 +14,7 @@ channels  channel enumeration (eq. 5) and the algebraic
           coefficients g of (A4)
 perm      ctypes front end to ``perm_oracle.c``: overlap predicate, CSR
           pattern, the quadrature rule R(n) for (A15), sequential CSR SpMV
+kernel_apply  one application of the factored kernel K = O P0 O^T V1 G1 (eq. 10, 12)
 
 Parity pins: see the header of each module and DESIGN.md section "Oracle pins".
 """

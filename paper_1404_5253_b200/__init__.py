@@ -30,7 +30,7 @@ EXPORTS = [
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
+    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
 
@@ -77,6 +77,8 @@ def load():
     L.wpcd_perm_apply.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_host.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp, vp, vp]
     L.wpcd_perm_apply_complex.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
+    L.wpcd_block_apply.argtypes = [i32, i32, i32, vp, i32, vp, vp, i32, vp]
+    L.wpcd_kernel_apply.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.wpcd_fp64_peak.argtypes = [vp, ctypes.POINTER(dbl)]
     L.wpcd_launch_count.restype = i64
     L.wpcd_trace_enable.argtypes = [i32]
@@ -225,6 +227,26 @@ def wpcd_perm_apply_complex(rows, row_ptr, col_idx, values, x, y, n_vec=1, strea
     assert x.dtype == torch.complex128 and y.dtype == torch.complex128
     _check(load().wpcd_perm_apply_complex(rows, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
                                           _dev_ptr(values, torch.float64), _dev_ptr(x), _dev_ptr(y), n_vec, _stream_ptr(stream)))
+
+
+def wpcd_block_apply(n_channels, n_p, n_q, a, x, y, transpose=False, stream=None):
+    """a: float64 [n_channels, n_p, n_p]; x, y: float64 or complex128 CUDA tensors with n_channels*n_p*n_q elements."""
+    import torch
+
+    assert a.dtype == torch.float64 and x.dtype == y.dtype and x.dtype in (torch.float64, torch.complex128)
+    _check(load().wpcd_block_apply(n_channels, n_p, n_q, _dev_ptr(a), 1 if transpose else 0, _dev_ptr(x), _dev_ptr(y),
+                                   1 if x.dtype == torch.complex128 else 0, _stream_ptr(stream)))
+
+
+def wpcd_kernel_apply(n_channels, n_p, n_q, row_ptr, col_idx, values, o, v, g1, x, y, scratch, stream=None):
+    """y = O P0 O^T V1 (G1 .* x); g1, x, y: complex128 [rows]; scratch: complex128 [2*rows]; o, v: float64 [n_ch, n_p, n_p]."""
+    import torch
+
+    assert g1.dtype == x.dtype == y.dtype == scratch.dtype == torch.complex128
+    assert scratch.numel() >= 2 * x.numel()
+    _check(load().wpcd_kernel_apply(n_channels, n_p, n_q, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
+                                    _dev_ptr(values, torch.float64), _dev_ptr(o, torch.float64), _dev_ptr(v, torch.float64),
+                                    _dev_ptr(g1), _dev_ptr(x), _dev_ptr(y), _dev_ptr(scratch), _stream_ptr(stream)))
 
 
 def wpcd_perm_apply_host(rows, row_ptr, col_idx, values, x_host, y_host, x_dev, y_dev, n_vec=1, stream=None):

@@ -654,6 +654,44 @@ wpcd_status wpcd_perm_apply_complex(int64_t rows, const int64_t* row_ptr_dev, co
     return WPCD_OK;
 }
 
+wpcd_status wpcd_block_apply(int n_channels, int n_p, int n_q, const double* a_dev, int transpose, const double* x_dev,
+                             double* y_dev, int complex_vectors, void* cuda_stream)
+{
+    if (n_channels < 0 || n_p < 0 || n_q < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_block_apply: negative size");
+    if (n_channels == 0 || n_p == 0 || n_q == 0) return WPCD_OK;
+    if (!a_dev || !x_dev || !y_dev || x_dev == y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_block_apply: null pointer or x aliases y");
+    cudaError_t err = launch_block_apply(n_channels, n_p, complex_vectors ? 2 * n_q : n_q, a_dev, transpose != 0, x_dev, y_dev,
+                                         static_cast<cudaStream_t>(cuda_stream));
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_block_apply");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_kernel_apply(int n_channels, int n_p, int n_q, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                              const double* values_dev, const double* o_dev, const double* v_dev, const double* g1_dev,
+                              const double* x_dev, double* y_dev, double* scratch_dev, void* cuda_stream)
+{
+    if (n_channels < 0 || n_p < 0 || n_q < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_kernel_apply: negative size");
+    const int64_t rows = (int64_t)n_channels * n_p * n_q;
+    if (rows == 0) return WPCD_OK;
+    if (!row_ptr_dev || !o_dev || !v_dev || !g1_dev || !x_dev || !y_dev || !scratch_dev)
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_kernel_apply: null pointer");
+    if ((reinterpret_cast<uintptr_t>(x_dev) | reinterpret_cast<uintptr_t>(y_dev) | reinterpret_cast<uintptr_t>(scratch_dev) |
+         reinterpret_cast<uintptr_t>(g1_dev)) & 15)
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_kernel_apply: complex arrays must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double* t1 = scratch_dev;                 // [rows] complex
+    double* t2 = scratch_dev + 2 * rows;      // [rows] complex
+    cudaError_t err = launch_diag_scale(rows, g1_dev, x_dev, t1, st);                                   // G1 .* x
+    if (err == cudaSuccess) err = launch_block_apply(n_channels, n_p, 2 * n_q, v_dev, false, t1, t2, st);  // V1
+    if (err == cudaSuccess) err = launch_block_apply(n_channels, n_p, 2 * n_q, o_dev, true, t2, t1, st);   // O^T
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_kernel_apply");
+    wpcd_status s = wpcd_perm_apply_complex(rows, row_ptr_dev, col_idx_dev, values_dev, t1, t2, 1, cuda_stream);   // P0
+    if (s != WPCD_OK) return s;
+    err = launch_block_apply(n_channels, n_p, 2 * n_q, o_dev, false, t2, y_dev, st);                    // O
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_kernel_apply");
+    return WPCD_OK;
+}
+
 wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
                                  const double* x_host, double* y_host, int n_vec, double* x_dev, double* y_dev, void* cuda_stream)
 {

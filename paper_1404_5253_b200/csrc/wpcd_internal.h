@@ -130,4 +130,8 @@ cudaError_t launch_spmv_complex(int64_t rows, const int64_t* row_ptr, const int3
                                 const double* x, double* y, int n_vec, double mean_row, cudaStream_t st);
 cudaError_t run_fp64_peak(cudaStream_t st, double* flops_out);
 
+// kernel_apply.cu
+cudaError_t launch_block_apply(int n_ch, int n_p, int n_cols, const double* A, bool transpose, const double* X, double* Y, cudaStream_t st);
+cudaError_t launch_diag_scale(int64_t n, const double* g, const double* x, double* y, cudaStream_t st);
+
 }  // namespace wpcd_detail

@@ -467,3 +467,40 @@ def test_handle_state_between_count_and_build(wpcd):
         assert np.array_equal(out[name][0], rp) and np.array_equal(out[name][1], ci)
         tol = VALUE_RTOL * np.maximum(np.abs(v), av) + VALUE_FLOOR * np.abs(v).max()
         assert np.all(np.abs(out[name][2] - v) <= tol)
+
+
+def test_block_apply_and_kernel_apply(wpcd):
+    """batched dense blocks (FP64 MMA) and the factored kernel K = O P0 O^T V1 G1 against
+    the numpy oracle, on a lattice whose block sizes are not multiples of the 32 x 32 tile."""
+    torch = _torch()
+    from oracle import kernel_apply as oka
+
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=1)
+    p = wi.tan2_grid(37, 1.0, 0.1, seed=91)
+    q = wi.tan2_grid(9, 0.8, 0.1, seed=92)
+    grid = wpcd.wpcd_grid_create(p, q)
+    m = wpcd.build_perm(grid, gch, 4)
+    n_ch, n_p, n_q, rows = gch.count, 37, 9, m.rows
+    assert rows == n_ch * n_p * n_q
+    o, v, g1 = wi.kernel_factors(n_ch, n_p, n_q)
+    od, vd = torch.from_numpy(o).cuda(), torch.from_numpy(v).cuda()
+    # block apply alone: real and complex, plain and transposed
+    xr = wi.normal_vector(rows, k=400)
+    xc = xr + 1j * wi.normal_vector(rows, k=401)
+    for xh in (xr, xc):
+        for tr in (False, True):
+            x = torch.from_numpy(xh).cuda()
+            y = torch.empty_like(x)
+            wpcd.wpcd_block_apply(n_ch, n_p, n_q, od, x, y, transpose=tr)
+            ref = oka.block_apply(o, xh, n_ch, n_p, n_q, transpose=tr)
+            scale = oka.block_apply(np.abs(o), np.abs(xh), n_ch, n_p, n_q, transpose=tr)
+            assert np.all(np.abs(y.cpu().numpy() - ref) <= 1e-13 * scale + 1e-300)
+    # the whole kernel, on the GPU-built CSR
+    rp, ci, vals = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    x = torch.from_numpy(xc).cuda()
+    y = torch.empty_like(x)
+    scratch = torch.empty(2 * rows, dtype=torch.complex128, device="cuda")
+    wpcd.wpcd_kernel_apply(n_ch, n_p, n_q, m.row_ptr, m.col_idx, m.values, od, vd, torch.from_numpy(g1).cuda(), x, y, scratch)
+    ref = oka.kernel_apply(rp, ci, vals, o, v, g1, xc, n_ch, n_p, n_q)
+    scale = oka.kernel_apply(rp, ci, np.abs(vals), np.abs(o), np.abs(v), np.abs(g1), np.abs(xc).astype(np.float64), n_ch, n_p, n_q)
+    assert np.all(np.abs(y.cpu().numpy() - ref) <= 1e-12 * np.abs(scale) + 1e-300)

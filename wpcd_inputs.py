@@ -66,3 +66,20 @@ WORKLOADS = {
 def normal_vector(n, seed=SEED, k=0):
     """Seeded N(0,1) vector number k of length n."""
     return np.random.default_rng([seed, 7, k]).standard_normal(n)
+
+
+def kernel_factors(n_ch, n_p, n_q, seed=SEED):
+    """Seeded synthetic factors of the kernel K = O P0 O^T V1 G1 (the real ones need the NN potential, which is
+    not available): O[g] a random orthogonal n_p x n_p matrix (QR of a Gaussian matrix), V1[g] a random symmetric
+    matrix scaled to spectral radius ~0.5, G1 a complex diagonal with |G1| ~ 1.  No method arithmetic here."""
+    rng = np.random.default_rng([seed, 11])
+    o = np.empty((n_ch, n_p, n_p))
+    v = np.empty((n_ch, n_p, n_p))
+    for g in range(n_ch):
+        qm, rm = np.linalg.qr(rng.standard_normal((n_p, n_p)))
+        o[g] = qm * np.sign(np.diag(rm))
+        a = rng.standard_normal((n_p, n_p))
+        v[g] = 0.25 * (a + a.T) / np.sqrt(n_p)
+    rows = n_ch * n_p * n_q
+    g1 = (rng.standard_normal(rows) + 1j * rng.standard_normal(rows)) / np.sqrt(2.0)
+    return o, v, g1

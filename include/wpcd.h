@@ -178,6 +178,20 @@ wpcd_status wpcd_kernel_apply(int n_channels, int n_p, int n_q, const int64_t* r
                               const double* values_dev, const double* o_dev, const double* v_dev, const double* g1_dev,
                               const double* x_dev, double* y_dev, double* scratch_dev, void* cuda_stream);
 
+/* Third step of SURVEY.md section 8(f): "solution of the resulting matrix equation by iteration using the
+ * Pade-approximant technique".  For u = b + K u (eq. 12 applied to the source column b) the
+ * elastic amplitude is one element of u (eq. 13): a = sum_n a_n, a_n = (K^n b)[element].
+ * wpcd_neumann_terms runs the iteration on the device (n_terms - 1 kernel applications) and returns the
+ * complex terms a_0 .. a_{n_terms-1} in terms_host (HOST, interleaved).  scratch_dev: (8*rows + 2*n_terms)
+ * doubles, 16-byte aligned, dev.  Synchronises the stream.
+ * wpcd_pade_sum (host only) sums the series with Wynn's epsilon algorithm -- the diagonal Pade approximants
+ * of sum_n a_n lambda^n at lambda = 1 -- which converges where the plain series does not. */
+wpcd_status wpcd_neumann_terms(int n_channels, int n_p, int n_q, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                               const double* values_dev, const double* o_dev, const double* v_dev, const double* g1_dev,
+                               const double* b_dev, int64_t element, int n_terms, double* terms_host, double* scratch_dev,
+                               void* cuda_stream);
+wpcd_status wpcd_pade_sum(const double* terms_host, int n_terms, double* sum_out);
+
 /* Same product with HOST vectors: copies x_host -> x_dev (scratch, dev, n_vec*rows doubles),
  * applies, copies y_dev (scratch) -> y_host, all on the stream, then synchronises it.
  * Pinned host memory makes the copies asynchronous. */

@@ -42,3 +42,35 @@ def kernel_apply(row_ptr, col_idx, values, o, v, g1, x, n_ch, n_p, n_q):
     t = block_apply(o, t, n_ch, n_p, n_q, transpose=True)    # SWP -> lattice basis:  sum_k' O_k'i' c_k'
     t = csr_apply(row_ptr, col_idx, values, t)               # P0
     return block_apply(o, t, n_ch, n_p, n_q)                 # lattice -> SWP basis:  sum_i O_ki
+
+
+def neumann_terms(row_ptr, col_idx, values, o, v, g1, b, element, n_terms, n_ch, n_p, n_q):
+    """a_n = (K^n b)[element], n = 0 .. n_terms-1: the terms of the iterated eq. (12) for the amplitude element
+    of eq. (13), "solution ... by iteration"."""
+    vec = np.asarray(b, np.complex128).copy()
+    out = np.zeros(n_terms, np.complex128)
+    for n in range(n_terms):
+        out[n] = vec[element]
+        if n + 1 < n_terms:
+            vec = kernel_apply(row_ptr, col_idx, values, o, v, g1, vec, n_ch, n_p, n_q)
+    return out
+
+
+def pade_sum(terms):
+    """Sum of the series by the Pade-approximant technique, in the form of Wynn's epsilon
+    algorithm on the partial sums S_n:  eps_{-1} = 0, eps_0^{(n)} = S_n,
+        eps_{k+1}^{(n)} = eps_{k-1}^{(n+1)} + 1 / (eps_k^{(n+1)} - eps_k^{(n)}),
+    whose even columns eps_{2k}^{(n)} are the Pade approximants [n+k / k] of sum a_n lambda^n at lambda = 1.
+    Returns the last entry of the highest even column that could be formed."""
+    S = np.cumsum(np.asarray(terms, np.complex128))
+    table = [np.zeros(len(S) + 1, np.complex128), S]          # eps_{-1}, eps_0
+    best = S[-1]
+    while len(table[-1]) > 1:
+        cur, prev = table[-1], table[-2]
+        d = cur[1:] - cur[:-1]
+        if np.any(d == 0):
+            break
+        table.append(prev[1:len(cur)] + 1.0 / d)
+        if (len(table) - 2) % 2 == 0:                          # column index = len(table) - 2
+            best = table[-1][-1]
+    return complex(best)

@@ -30,7 +30,8 @@ EXPORTS = [
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
+    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
+    "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
 
@@ -79,6 +80,8 @@ def load():
     L.wpcd_perm_apply_complex.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_block_apply.argtypes = [i32, i32, i32, vp, i32, vp, vp, i32, vp]
     L.wpcd_kernel_apply.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.wpcd_neumann_terms.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i64, i32, vp, vp, vp]
+    L.wpcd_pade_sum.argtypes = [vp, i32, vp]
     L.wpcd_fp64_peak.argtypes = [vp, ctypes.POINTER(dbl)]
     L.wpcd_launch_count.restype = i64
     L.wpcd_trace_enable.argtypes = [i32]
@@ -247,6 +250,28 @@ def wpcd_kernel_apply(n_channels, n_p, n_q, row_ptr, col_idx, values, o, v, g1, 
     _check(load().wpcd_kernel_apply(n_channels, n_p, n_q, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
                                     _dev_ptr(values, torch.float64), _dev_ptr(o, torch.float64), _dev_ptr(v, torch.float64),
                                     _dev_ptr(g1), _dev_ptr(x), _dev_ptr(y), _dev_ptr(scratch), _stream_ptr(stream)))
+
+
+def wpcd_neumann_terms(n_channels, n_p, n_q, row_ptr, col_idx, values, o, v, g1, b, element, n_terms, stream=None):
+    """Complex terms a_n = (K^n b)[element], n = 0 .. n_terms-1, as a numpy complex128 array."""
+    import torch
+
+    rows = n_channels * n_p * n_q
+    scratch = torch.empty(4 * rows + n_terms, dtype=torch.complex128, device=b.device)
+    terms = np.zeros(n_terms, np.complex128)
+    _check(load().wpcd_neumann_terms(n_channels, n_p, n_q, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
+                                     _dev_ptr(values, torch.float64), _dev_ptr(o, torch.float64), _dev_ptr(v, torch.float64),
+                                     _dev_ptr(g1), _dev_ptr(b), int(element), n_terms, terms.ctypes.data, _dev_ptr(scratch),
+                                     _stream_ptr(stream)))
+    return terms
+
+
+def wpcd_pade_sum(terms):
+    """Pade (Wynn epsilon) sum of the complex series `terms` (host only)."""
+    t = np.ascontiguousarray(terms, np.complex128)
+    out = np.zeros(1, np.complex128)
+    _check(load().wpcd_pade_sum(t.ctypes.data, len(t), out.ctypes.data))
+    return complex(out[0])
 
 
 def wpcd_perm_apply_host(rows, row_ptr, col_idx, values, x_host, y_host, x_dev, y_dev, n_vec=1, stream=None):

@@ -2,6 +2,7 @@
 // PAPER.md:310), argument checks and kernel launches.  No torch types, no CPU fallback.
 #include <algorithm>
 #include <cmath>
+#include <complex>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -689,6 +690,61 @@ wpcd_status wpcd_kernel_apply(int n_channels, int n_p, int n_q, const int64_t* r
     if (s != WPCD_OK) return s;
     err = launch_block_apply(n_channels, n_p, 2 * n_q, o_dev, false, t2, y_dev, st);                    // O
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_kernel_apply");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_neumann_terms(int n_channels, int n_p, int n_q, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                               const double* values_dev, const double* o_dev, const double* v_dev, const double* g1_dev,
+                               const double* b_dev, int64_t element, int n_terms, double* terms_host, double* scratch_dev,
+                               void* cuda_stream)
+{
+    const int64_t rows = (int64_t)n_channels * n_p * n_q;
+    if (n_terms < 1 || !terms_host || !b_dev || !scratch_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_neumann_terms: bad arguments");
+    if (element < 0 || element >= rows) return fail(WPCD_ERR_INVALID_ARG, "wpcd_neumann_terms: element out of range");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // scratch: [0, 2 rows) complex for wpcd_kernel_apply, then two complex vectors, then the picked terms
+    double* ka_scratch = scratch_dev;
+    double* va = scratch_dev + 4 * rows;
+    double* vb = va + 2 * rows;
+    double* picked = vb + 2 * rows;          // [n_terms] complex
+    cudaError_t err = cudaMemcpyAsync(va, b_dev, sizeof(double) * 2 * rows, cudaMemcpyDeviceToDevice, st);
+    for (int n = 0; n < n_terms && err == cudaSuccess; ++n) {
+        err = cudaMemcpyAsync(picked + 2 * n, va + 2 * element, sizeof(double) * 2, cudaMemcpyDeviceToDevice, st);   // a_n = (K^n b)[element]
+        if (err != cudaSuccess || n + 1 == n_terms) break;
+        wpcd_status s = wpcd_kernel_apply(n_channels, n_p, n_q, row_ptr_dev, col_idx_dev, values_dev, o_dev, v_dev, g1_dev, va, vb,
+                                          ka_scratch, cuda_stream);
+        if (s != WPCD_OK) return s;
+        std::swap(va, vb);
+    }
+    if (err == cudaSuccess) err = cudaMemcpyAsync(terms_host, picked, sizeof(double) * 2 * n_terms, cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_neumann_terms");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_pade_sum(const double* terms_host, int n_terms, double* sum_out)
+{
+    if (!terms_host || !sum_out || n_terms < 1) return fail(WPCD_ERR_INVALID_ARG, "wpcd_pade_sum: bad arguments");
+    // Wynn's epsilon algorithm on the partial sums: eps_{k+1}^{(n)} = eps_{k-1}^{(n+1)} + 1 / (eps_k^{(n+1)} - eps_k^{(n)});
+    // the even columns are the Pade approximants [n+k / k] of the series at lambda = 1
+    typedef std::complex<double> cplx;
+    std::vector<cplx> prev(n_terms + 1, cplx(0.0, 0.0)), cur(n_terms), nxt;
+    cplx run(0.0, 0.0);
+    for (int n = 0; n < n_terms; ++n) { run += cplx(terms_host[2 * n], terms_host[2 * n + 1]); cur[n] = run; }
+    cplx best = cur.back();
+    for (int k = 0; (int)cur.size() > 1; ++k) {
+        nxt.assign(cur.size() - 1, cplx(0.0, 0.0));
+        bool ok = true;
+        for (size_t n = 0; n + 1 < cur.size(); ++n) {
+            cplx d = cur[n + 1] - cur[n];
+            if (std::abs(d) == 0.0) { ok = false; break; }      // converged exactly: keep the last even column
+            nxt[n] = prev[n + 1] + cplx(1.0, 0.0) / d;
+        }
+        if (!ok) break;
+        prev = cur; cur = nxt;
+        if ((k & 1) == 1) best = cur.back();                   // cur is now an even column
+    }
+    sum_out[0] = best.real(); sum_out[1] = best.imag();
     return WPCD_OK;
 }
 

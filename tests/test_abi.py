@@ -83,3 +83,20 @@ def test_compute_fails_loudly_without_gpu(wpcd):
         pytest.skip("GPU present")
     with pytest.raises(wpcd.WpcdError):
         wpcd.wpcd_grid_create(np.array([0.0, 1.0]), np.array([0.0, 1.0]))
+
+
+def test_pade_sum_host(wpcd):
+    """wpcd_pade_sum is host-only code of the product: against the closed forms and the oracle's epsilon table."""
+    import numpy as np
+    from oracle import kernel_apply as oka
+
+    for r in (0.5, -2.0, 3.0 + 1.0j):
+        terms = np.array([r ** n for n in range(8)], np.complex128)
+        assert abs(wpcd.wpcd_pade_sum(terms) - 1.0 / (1.0 - r)) < 1e-9
+    rng = np.random.default_rng(3)
+    poles = np.array([-1.4, 0.7 + 0.2j, 0.3j])
+    coef = rng.standard_normal(3) + 1j * rng.standard_normal(3)
+    terms = np.array([np.sum(coef * poles ** n) for n in range(12)], np.complex128)
+    exact = np.sum(coef / (1 - poles))
+    assert abs(wpcd.wpcd_pade_sum(terms) - exact) < 1e-7
+    assert abs(wpcd.wpcd_pade_sum(terms) - oka.pade_sum(terms)) < 1e-7

@@ -504,3 +504,36 @@ def test_block_apply_and_kernel_apply(wpcd):
     ref = oka.kernel_apply(rp, ci, vals, o, v, g1, xc, n_ch, n_p, n_q)
     scale = oka.kernel_apply(rp, ci, np.abs(vals), np.abs(o), np.abs(v), np.abs(g1), np.abs(xc).astype(np.float64), n_ch, n_p, n_q)
     assert np.all(np.abs(y.cpu().numpy() - ref) <= 1e-12 * np.abs(scale) + 1e-300)
+
+
+def test_neumann_terms_and_pade(wpcd):
+    """the iteration of eq. (12) on the device and its Pade sum, against the oracle's terms and
+    the direct dense solve, for a kernel scaled beyond the unit disc (the plain series diverges)."""
+    torch = _torch()
+    from oracle import kernel_apply as oka
+
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=1)
+    p = wi.tan2_grid(4, 1.0, 0.1, seed=81)
+    q = wi.tan2_grid(3, 0.9, 0.1, seed=82)
+    m = wpcd.build_perm(wpcd.wpcd_grid_create(p, q), gch, 6)
+    n_ch, n_p, n_q, rows = gch.count, 4, 3, m.rows
+    rp, ci, vals = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    o, v, g1 = wi.kernel_factors(n_ch, n_p, n_q)
+    K = np.array([oka.kernel_apply(rp, ci, vals, o, v, g1, np.eye(rows)[:, c].astype(np.complex128), n_ch, n_p, n_q)
+                  for c in range(rows)]).T
+    rho_scale = 1.3 / np.abs(np.linalg.eigvals(K)).max()
+    g1 = g1 * rho_scale
+    b = wi.normal_vector(rows, k=5) + 1j * wi.normal_vector(rows, k=6)
+    element, n_terms = 7, 36
+    terms = wpcd.wpcd_neumann_terms(n_ch, n_p, n_q, m.row_ptr, m.col_idx, m.values, torch.from_numpy(o).cuda(),
+                                    torch.from_numpy(v).cuda(), torch.from_numpy(g1).cuda(), torch.from_numpy(b).cuda(),
+                                    element, n_terms)
+    ref = oka.neumann_terms(rp, ci, vals, o, v, g1, b, element, n_terms, n_ch, n_p, n_q)
+    growth = np.maximum.accumulate(np.abs(ref))
+    assert np.all(np.abs(terms - ref) <= 1e-10 * growth * np.arange(1, n_terms + 1))
+    exact = np.linalg.solve(np.eye(rows) - K * rho_scale, b)[element]
+    # same table on both sides for the same input terms; the sum itself is as accurate as an epsilon table of
+    # 36 terms can be for 120 poles with |lambda| up to 1.3 (the plain series is off by orders of magnitude)
+    assert abs(wpcd.wpcd_pade_sum(terms) - oka.pade_sum(terms)) < 1e-8 * max(1.0, abs(exact))
+    assert abs(wpcd.wpcd_pade_sum(terms) - exact) < 2e-3 * max(1.0, abs(exact))
+    assert abs(np.sum(terms) - exact) > 1e2 * abs(exact)

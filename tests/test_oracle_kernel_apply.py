@@ -70,3 +70,35 @@ def test_orthogonal_rotation_keeps_the_spectrum():
     assert np.allclose(np.linalg.eigvalsh(0.5 * (P + P.T)), np.linalg.eigvalsh(0.5 * (P0 + P0.T)), atol=1e-11)
     for g in range(n_ch):
         assert np.allclose(o[g] @ o[g].T, np.eye(n_p), atol=1e-13)
+
+
+def test_pade_sums_divergent_geometric_and_rational_series():
+    # sum r^n = 1/(1-r): exact for the [n/1] approximant, also where the series diverges
+    for r in (0.5, -2.0, 3.0 + 1.0j, -0.9j):
+        terms = np.array([r ** n for n in range(8)], np.complex128)
+        assert abs(ka.pade_sum(terms) - 1.0 / (1.0 - r)) < 1e-9 * max(1.0, abs(1.0 / (1.0 - r)))
+    # two poles: sum (c1 r1^n + c2 r2^n) = c1/(1-r1) + c2/(1-r2), exact from [n/2] on
+    r1, r2, c1, c2 = -1.7, 0.6 + 0.3j, 2.0, -0.5j
+    terms = np.array([c1 * r1 ** n + c2 * r2 ** n for n in range(10)], np.complex128)
+    exact = c1 / (1 - r1) + c2 / (1 - r2)
+    assert abs(ka.pade_sum(terms) - exact) < 1e-8
+
+
+def test_iteration_and_pade_against_direct_solve():
+    """u = b + K u: the amplitude element of (1 - K)^{-1} b from the Neumann terms + Pade, on a tiny lattice, for a
+    kernel inside the unit disc (the plain series converges) and for one scaled beyond it (only Pade does)."""
+    n_ch, n_p, n_q, rp, ci, v = _setup(3)
+    rows = n_ch * n_p * n_q
+    o, vv, g1 = wi.kernel_factors(n_ch, n_p, n_q)
+    K = np.array([ka.kernel_apply(rp, ci, v, o, vv, g1, np.eye(rows)[:, c].astype(np.complex128), n_ch, n_p, n_q)
+                  for c in range(rows)]).T
+    rho = np.abs(np.linalg.eigvals(K)).max()
+    b = wi.normal_vector(rows, k=5) + 1j * wi.normal_vector(rows, k=6)
+    element = 7
+    for target_rho, n_terms, tol in ((0.5, 40, 1e-9), (1.6, 40, 1e-5)):
+        scale = target_rho / rho
+        exact = np.linalg.solve(np.eye(rows) - scale * K, b)[element]
+        terms = ka.neumann_terms(rp, ci, v, o, vv, scale * g1, b, element, n_terms, n_ch, n_p, n_q)
+        assert abs(ka.pade_sum(terms) - exact) < tol * max(1.0, abs(exact))
+        if target_rho > 1:
+            assert abs(np.sum(terms) - exact) > 1e3 * abs(exact)        # the plain series has diverged

@@ -261,3 +261,19 @@ def test_multichannel_spectrum_bound(two_J, parity, jmax):
         assert w[0] < -0.8 and w[-1] > 1.6            # both ends of the exact spectrum are being approached
         top.append(w[-1])
     assert top[1] > top[0]
+
+
+def test_rule_converges_with_order(swave_table):
+    """Accuracy of the contract rule R(n) (R7): the integrand has kinks, so the error falls only
+    algebraically -- it must fall monotonically, roughly like n^-1.5 .. n^-2 (2.1e-2 at n = 8, 1e-3 at n = 32)."""
+    p = wi.tan2_grid(12, 1.0, 0.1, seed=3)
+    geo = perm.geo_pattern(p, p)
+    ref = perm.build_csr(p, p, 64, swave_table, geo=geo)[2]
+    errs = {}
+    for n in (4, 8, 16, 32):
+        v = perm.build_csr(p, p, n, swave_table, geo=geo)[2]
+        errs[n] = np.linalg.norm(v - ref) / np.linalg.norm(ref)
+    assert errs[4] > errs[8] > errs[16] > errs[32]
+    assert 1e-2 < errs[8] < 4e-2 and errs[32] < 2e-3
+    rate = np.log(errs[8] / errs[32]) / np.log(4.0)
+    assert 1.0 < rate < 3.0

@@ -537,3 +537,23 @@ def test_neumann_terms_and_pade(wpcd):
     assert abs(wpcd.wpcd_pade_sum(terms) - oka.pade_sum(terms)) < 1e-8 * max(1.0, abs(exact))
     assert abs(wpcd.wpcd_pade_sum(terms) - exact) < 2e-3 * max(1.0, abs(exact))
     assert abs(np.sum(terms) - exact) > 1e2 * abs(exact)
+
+
+def test_coupled_limits_of_the_table(wpcd):
+    """The largest orbital momentum and Legendre order the header allows (WPCD_MAX_L = 7, WPCD_MAX_K = 23)."""
+    rng = np.random.default_rng(20140522)
+    chan_l = [7, 3]
+    pairs = []
+    for ga in range(2):
+        for gb in range(2):
+            l, lp = chan_l[ga], chan_l[gb]
+            terms = [(k, l1, l1p, float(rng.uniform(-1, 1)))
+                     for l1 in range(0, l + 1, 2) for l1p in range(0, lp + 1) for k in (0, 5, 11, 23)]
+            pairs.append((ga, gb, terms))
+    chs = [(l, 0, 0, 0, 0, 0) for l in chan_l]
+    tab = operm.PairTable(chs, pairs)
+    gch = wpcd.wpcd_channels_create_from_table(np.array(chan_l), tab.gamma, tab.gammap, tab.term_ptr,
+                                               tab.term_k, tab.term_l1, tab.term_l1p, tab.term_g)
+    p = np.array([0.2, 0.5, 1.1, 2.0])          # away from p = 0: the single terms of l = 7 are not integrable there
+    q = np.array([0.1, 0.6, 1.4])
+    _compare_full(wpcd, p, q, 5, gch, tab)

@@ -145,7 +145,9 @@ wpcd_status wpcd_perm_build(const wpcd_grid* grid, const wpcd_channels* channels
                             int32_t* col_idx_dev, double* values_dev);
 
 /* y = P0 x for n_vec vectors (step 5, l.314; l.304).  x_dev[v*rows + c], y_dev[v*rows + r],
- * v = 0..n_vec-1 (vector-major), dev.  CSR arrays as produced above.  Asynchronous. */
+ * v = 0..n_vec-1 (vector-major), dev.  CSR arrays as produced above.  Asynchronous -- except that the first
+ * product on a row_ptr_dev this process has not seen from wpcd_perm_count reads nnz back once (synchronises the
+ * stream; do that call outside a CUDA-graph capture): the kernel variant is chosen from the mean row length. */
 wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
                             const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
                             void* cuda_stream);

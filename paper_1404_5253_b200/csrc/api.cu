@@ -551,6 +551,7 @@ wpcd_status wpcd_perm_count(const wpcd_grid* g_in, const wpcd_channels* c, int n
     *nnz_out = nnz_geo * c->total_coupled;
     {
         std::lock_guard<std::mutex> lock(g_hint_mutex);
+        if (g_nnz_hint.size() > 4096) g_nnz_hint.clear();   // a heuristic cache only (kernel selection): keep it bounded
         g_nnz_hint[row_ptr_dev] = {rows, *nnz_out};
     }
     return WPCD_OK;
@@ -621,6 +622,7 @@ static double mean_row_hint(int64_t rows, const int64_t* row_ptr_dev, cudaStream
     if (cudaMemcpyAsync(&nnz, row_ptr_dev + rows, sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess) return 32.0;
     cudaStreamSynchronize(st);
     std::lock_guard<std::mutex> lock(g_hint_mutex);
+    if (g_nnz_hint.size() > 4096) g_nnz_hint.clear();
     g_nnz_hint[row_ptr_dev] = {rows, nnz};
     return (double)nnz / (double)std::max<int64_t>(rows, 1);
 }

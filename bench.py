@@ -365,6 +365,19 @@ def run_ours(args):
         msc = a.elapsed_time(b) / reps
         spmm["complex_ms_per_product"] = msc
         spmm["complex_matrix_GBps"] = (12.0 * job.nnz + 8.0 * job.rows) / (msc * 1e-3) / 1e9
+        # four real vectors interleaved [rows][4]: one 32-byte gather per entry
+        xi4 = x4.t().contiguous()
+        yi4 = torch.empty_like(xi4)
+        for _ in range(3):
+            wpcd.wpcd_perm_apply_interleaved(job.rows, job.row_ptr, job.col_idx, job.values, xi4, yi4)
+        a.record()
+        for _ in range(reps):
+            wpcd.wpcd_perm_apply_interleaved(job.rows, job.row_ptr, job.col_idx, job.values, xi4, yi4)
+        b.record()
+        torch.cuda.synchronize()
+        msi = a.elapsed_time(b) / reps
+        spmm["interleaved4_ms_per_pass"] = msi
+        spmm["interleaved4_matrix_GBps"] = (12.0 * job.nnz + 8.0 * job.rows) / (msi * 1e-3) / 1e9
         # one application of the factored kernel K = O P0 O^T V1 G1 (synthetic O, V1, G1)
         n_ch = job.channels.count
         o_h, v_h, g_h = wi.kernel_factors(n_ch, grid.n_p, grid.n_q)

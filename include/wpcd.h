@@ -160,6 +160,14 @@ wpcd_status wpcd_perm_apply_complex(int64_t rows, const int64_t* row_ptr_dev, co
                                     const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
                                     void* cuda_stream);
 
+/* y = P0 x for n_inter = 2 or 4 vectors stored INTERLEAVED, x_dev[c*n_inter + v] (two complex or four real
+ * vectors for n_inter = 4): one gather of n_inter*8 bytes per entry instead of n_inter separate ones -- the
+ * layout for many right-hand sides (P0 is reused for ~100 energies).  16-byte aligned, dev.
+ * Asynchronous. */
+wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                                        const double* values_dev, const double* x_dev, double* y_dev, int n_inter,
+                                        void* cuda_stream);
+
 /* Next step of SURVEY.md section 8(f): the kernel of eq. (12) in factored form.
  * wpcd_block_apply: for every channel gamma, Y_gamma = A_gamma X_gamma (transpose = 0) or A_gamma^T X_gamma
  * (transpose != 0), where X_gamma is the n_p x n_q block x_dev[(gamma*n_p + i)*n_q + j] of the vector and

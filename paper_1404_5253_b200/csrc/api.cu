@@ -652,8 +652,25 @@ wpcd_status wpcd_perm_apply_complex(int64_t rows, const int64_t* row_ptr_dev, co
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     double mean_row = mean_row_hint(rows, row_ptr_dev, st);
     if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_complex: null matrix arrays");
-    cudaError_t err = launch_spmv_complex(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, mean_row, st);
+    cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, 2, mean_row, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_complex");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                        const double* x_dev, double* y_dev, int n_inter, void* cuda_stream)
+{
+    if (rows < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: negative size");
+    if (n_inter != 2 && n_inter != 4) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_apply_interleaved: n_inter must be 2 or 4");
+    if (rows == 0) return WPCD_OK;
+    if (!row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: null pointer");
+    if ((reinterpret_cast<uintptr_t>(x_dev) & 15) || (reinterpret_cast<uintptr_t>(y_dev) & 15))
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: x and y must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
+    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: null matrix arrays");
+    cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, 1, n_inter, mean_row, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_interleaved");
     return WPCD_OK;
 }
 

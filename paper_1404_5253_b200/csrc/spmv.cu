@@ -132,35 +132,40 @@ cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_id
     return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
 }
 
-// ---------------------------------------------------------------- complex right-hand side
-// y = P0 x for one complex vector stored interleaved (re, im): P0 is real, so an entry costs one 16-byte
-// gather and two multiply-adds (the transition operator of eq. 12 is complex).
-template <int LPR, bool PIPE>
+// ---------------------------------------------------------------- interleaved right-hand sides
+// y = P0 x for NI vectors stored interleaved, x[c*NI + v]: NI = 2 is one complex vector (re, im) -- P0 is real,
+// the transition operator of eq. 12 is complex -- NI = 4 two complex or four real vectors.
+// An entry costs ONE gather of NI*8 bytes and NI multiply-adds.
+template <int LPR, bool PIPE, int NI>
 __global__ void __launch_bounds__(256)
-spmv_complex_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
-                    const double* __restrict__ values, const double2* __restrict__ x, double2* __restrict__ y)
+spmv_interleaved_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+                        const double* __restrict__ values, const double2* __restrict__ x, double2* __restrict__ y)
 {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    constexpr int H = NI / 2;                 // 16-byte pieces per column
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = t / LPR;
     const int sub = (int)(t - row * LPR);
-    double re = 0.0, im = 0.0;
+    double acc[NI];
+#pragma unroll
+    for (int v = 0; v < NI; ++v) acc[v] = 0.0;
     if (row < rows) {
         const int64_t beg = row_ptr[row], end = row_ptr[row + 1];
         constexpr int UNR = 4;
-        double a[UNR], a2[UNR];
-        int c[UNR], c2[UNR];
-        int64_t e0 = beg + sub;
+        if (PIPE) {
+            // long rows streamed from HBM: batch b+1's index/value loads fly while batch b gathers and accumulates
+            double a[UNR], a2[UNR];
+            int c[UNR], c2[UNR];
+            int64_t e0 = beg + sub;
 #pragma unroll
-        for (int k = 0; k < UNR; ++k) {
-            const int64_t e = e0 + (int64_t)k * LPR;
-            const bool in = e < end;
-            a[k] = in ? values[e] : 0.0;
-            c[k] = in ? col_idx[e] : 0;
-        }
-        for (; e0 < end; e0 += (int64_t)UNR * LPR) {
-            if (PIPE) {
+            for (int k = 0; k < UNR; ++k) {
+                const int64_t e = e0 + (int64_t)k * LPR;
+                const bool in = e < end;
+                a[k] = in ? __ldcs(values + e) : 0.0;
+                c[k] = in ? __ldcs(col_idx + e) : 0;
+            }
+            for (; e0 < end; e0 += (int64_t)UNR * LPR) {
                 const int64_t n0 = e0 + (int64_t)UNR * LPR;
 #pragma unroll
                 for (int k = 0; k < UNR; ++k) {
@@ -169,39 +174,60 @@ spmv_complex_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int
                     a2[k] = in ? __ldcs(values + e) : 0.0;
                     c2[k] = in ? __ldcs(col_idx + e) : 0;
                 }
-            }
-#pragma unroll
-            for (int k = 0; k < UNR; ++k) {
-                const double2 xv = __ldg(x + c[k]);
-                re = fma(a[k], xv.x, re);
-                im = fma(a[k], xv.y, im);
-            }
-            if (PIPE) {
-#pragma unroll
-                for (int k = 0; k < UNR; ++k) { a[k] = a2[k]; c[k] = c2[k]; }
-            } else {
-                const int64_t n0 = e0 + (int64_t)UNR * LPR;
 #pragma unroll
                 for (int k = 0; k < UNR; ++k) {
-                    const int64_t e = n0 + (int64_t)k * LPR;
-                    const bool in = e < end;
-                    a[k] = in ? values[e] : 0.0;
-                    c[k] = in ? col_idx[e] : 0;
+#pragma unroll
+                    for (int h = 0; h < H; ++h) {
+                        const double2 xv = __ldg(x + (int64_t)c[k] * H + h);
+                        acc[2 * h] = fma(a[k], xv.x, acc[2 * h]);
+                        acc[2 * h + 1] = fma(a[k], xv.y, acc[2 * h + 1]);
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) { a[k] = a2[k]; c[k] = c2[k]; }
+            }
+        } else {
+            // The gathers are guarded by the same bounds test as the index loads. (With unguarded
+            // gathers of a default column 0, nvcc 12.9 -O3 miscompiles the unrolled loop for NI = 4:
+            // wild addresses on sm_100a as soon as a row needs a second batch; reproduced stand-alone.)
+            for (int64_t e0 = beg + sub; e0 < end; e0 += (int64_t)UNR * LPR) {
+                double a[UNR];
+                int c[UNR];
+                bool in[UNR];
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+                    const int64_t e = e0 + (int64_t)k * LPR;
+                    in[k] = e < end;
+                    a[k] = in[k] ? values[e] : 0.0;
+                    c[k] = in[k] ? col_idx[e] : 0;
+                }
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+#pragma unroll
+                    for (int h = 0; h < H; ++h) {
+                        double2 xv = make_double2(0.0, 0.0);
+                        if (in[k]) xv = __ldg(x + (int64_t)c[k] * H + h);
+                        acc[2 * h] = fma(a[k], xv.x, acc[2 * h]);
+                        acc[2 * h + 1] = fma(a[k], xv.y, acc[2 * h + 1]);
+                    }
                 }
             }
         }
     }
 #pragma unroll
-    for (int o = LPR / 2; o > 0; o >>= 1) {
-        re += __shfl_xor_sync(0xffffffffu, re, o);
-        im += __shfl_xor_sync(0xffffffffu, im, o);
+    for (int v = 0; v < NI; ++v) {
+#pragma unroll
+        for (int o = LPR / 2; o > 0; o >>= 1) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], o);
     }
-    if (row < rows && sub == 0) y[row] = make_double2(re, im);
+    if (row < rows && sub == 0) {
+#pragma unroll
+        for (int h = 0; h < H; ++h) y[row * H + h] = make_double2(acc[2 * h], acc[2 * h + 1]);
+    }
 }
 
-template <int LPR, bool PIPE>
-cudaError_t launch_complex(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                           const double2* x, double2* y, cudaStream_t st)
+template <int LPR, bool PIPE, int NI>
+cudaError_t launch_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+                               const double2* x, double2* y, cudaStream_t st)
 {
     int64_t blocks = (rows * LPR + 255) / 256;
     cudaLaunchConfig_t cfg = {};
@@ -214,7 +240,17 @@ cudaError_t launch_complex(int64_t rows, const int64_t* row_ptr, const int32_t* 
     cfg.attrs = attr;
     cfg.numAttrs = wpcd_detail::use_pdl() ? 1 : 0;
     ++wpcd_detail::g_launches;
-    return cudaLaunchKernelEx(&cfg, spmv_complex_kernel<LPR, PIPE>, rows, row_ptr, col_idx, values, x, y);
+    return cudaLaunchKernelEx(&cfg, spmv_interleaved_kernel<LPR, PIPE, NI>, rows, row_ptr, col_idx, values, x, y);
+}
+
+template <int NI>
+cudaError_t dispatch_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+                                 const double2* x, double2* y, double mean_row, cudaStream_t st)
+{
+    if (mean_row <= 6.0) return launch_interleaved<8, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
+    if (mean_row <= 12.0) return launch_interleaved<16, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
+    if (mean_row >= 128.0) return launch_interleaved<32, true, NI>(rows, row_ptr, col_idx, values, x, y, st);
+    return launch_interleaved<32, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
 }
 
 // ---------------------------------------------------------------- FP64 FMA peak
@@ -256,17 +292,15 @@ cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col
     return cudaSuccess;
 }
 
-cudaError_t launch_spmv_complex(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                                const double* x, double* y, int n_vec, double mean_row, cudaStream_t st)
+// n_vec groups of n_inter interleaved components each (group-major: x[(g*rows + c)*n_inter + v])
+cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
+                                    const double* x, double* y, int n_vec, int n_inter, double mean_row, cudaStream_t st)
 {
     for (int v = 0; v < n_vec; ++v) {
-        const double2* xv = reinterpret_cast<const double2*>(x) + (int64_t)v * rows;
-        double2* yv = reinterpret_cast<double2*>(y) + (int64_t)v * rows;
-        cudaError_t err;
-        if (mean_row <= 6.0) err = launch_complex<8, false>(rows, row_ptr, col_idx, values, xv, yv, st);
-        else if (mean_row <= 12.0) err = launch_complex<16, false>(rows, row_ptr, col_idx, values, xv, yv, st);
-        else if (mean_row >= 128.0) err = launch_complex<32, true>(rows, row_ptr, col_idx, values, xv, yv, st);
-        else err = launch_complex<32, false>(rows, row_ptr, col_idx, values, xv, yv, st);
+        const double2* xv = reinterpret_cast<const double2*>(x) + (int64_t)v * rows * (n_inter / 2);
+        double2* yv = reinterpret_cast<double2*>(y) + (int64_t)v * rows * (n_inter / 2);
+        cudaError_t err = n_inter == 4 ? dispatch_interleaved<4>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st)
+                                       : dispatch_interleaved<2>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;

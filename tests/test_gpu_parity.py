@@ -479,6 +479,73 @@ def test_handle_state_between_count_and_build(wpcd):
         assert np.all(np.abs(out[name][2] - v) <= tol)
 
 
+def test_apply_interleaved(wpcd):
+    """Four (and two) real vectors stored interleaved [rows][n_inter]: one gather per entry; short-row and long-row matrices."""
+    torch = _torch()
+    cases = []
+    p = wi.tan2_grid(24, 1.0, 0.1, seed=8)
+    cases.append(wpcd.build_perm(wpcd.wpcd_grid_create(p, p), wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5), 8))
+    p2 = wi.tan2_grid(10, 1.0, 0.1, seed=61)
+    cases.append(wpcd.build_perm(wpcd.wpcd_grid_create(p2, p2),
+                                 wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=1, two_T=1, j_pair_max=2), 6))
+    for m in cases:
+        rows = m.rows
+        rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+        for n_inter in (2, 4):
+            xh = np.stack([wi.normal_vector(rows, k=500 + k) for k in range(n_inter)], axis=1).copy()    # [rows, n_inter]
+            x = torch.from_numpy(xh).cuda().contiguous()
+            y = torch.empty_like(x)
+            wpcd.wpcd_perm_apply_interleaved(rows, m.row_ptr, m.col_idx, m.values, x, y)
+            yh = y.cpu().numpy()
+            for k in range(n_inter):
+                ref = operm.spmv(rp, ci, v, np.ascontiguousarray(xh[:, k]))
+                scale = operm.spmv(rp, ci, np.abs(v), np.abs(np.ascontiguousarray(xh[:, k])))
+                assert np.all(np.abs(yh[:, k] - ref) <= 1e-12 * scale + 1e-300)
+
+
+def test_apply_row_length_sweep(wpcd):
+    """Foreign CSR arrays with controlled row lengths (empty rows, one batch, batch boundaries +-1, several batches,
+    pipelined long rows): every lane-count variant of the plain, multi-vector, complex and interleaved products
+    against the oracle's row-by-row product."""
+    torch = _torch()
+    rng = np.random.default_rng(77)
+    for rows, short, long_ in ((500, 4, 4), (500, 4, 33), (500, 9, 64), (500, 9, 65), (500, 0, 129), (500, 20, 257),
+                              (700, 40, 300), (1200, 150, 600)):
+        lens = np.full(rows, short, dtype=np.int64)
+        lens[::7] = long_
+        rp = np.zeros(rows + 1, dtype=np.int64)
+        rp[1:] = np.cumsum(lens)
+        nnz = int(rp[-1])
+        ci = rng.integers(0, rows, nnz).astype(np.int32)
+        v = rng.standard_normal(nnz)
+        rpd, cid, vd = torch.from_numpy(rp).cuda(), torch.from_numpy(ci).cuda(), torch.from_numpy(v).cuda()
+        xs = np.stack([wi.normal_vector(rows, k=700 + k) for k in range(4)])                 # [4, rows]
+        refs = [operm.spmv(rp, ci, v, xs[k]) for k in range(4)]
+        scales = [operm.spmv(rp, ci, np.abs(v), np.abs(xs[k])) for k in range(4)]
+
+        def check(got, k):
+            assert np.all(np.abs(got - refs[k]) <= 1e-12 * scales[k] + 1e-300), (rows, short, long_, k)
+
+        for n_vec in (1, 2, 3, 4):
+            x = torch.from_numpy(xs[:n_vec].copy()).cuda()
+            y = torch.full_like(x, np.nan)
+            wpcd.wpcd_perm_apply(rows, rpd, cid, vd, x, y, n_vec)
+            for k in range(n_vec):
+                check(y[k].cpu().numpy(), k)
+        xc = torch.from_numpy((xs[0] + 1j * xs[1])[None, :].copy()).cuda()
+        yc = torch.full_like(xc, np.nan)
+        wpcd.wpcd_perm_apply_complex(rows, rpd, cid, vd, xc, yc, 1)
+        check(yc[0].real.cpu().numpy(), 0)
+        check(yc[0].imag.cpu().numpy(), 1)
+        for n_inter in (2, 4):
+            xi = torch.from_numpy(np.ascontiguousarray(xs[:n_inter].T)).cuda()              # [rows, n_inter]
+            yi = torch.full_like(xi, np.nan)
+            wpcd.wpcd_perm_apply_interleaved(rows, rpd, cid, vd, xi, yi)
+            yh = yi.cpu().numpy()
+            for k in range(n_inter):
+                check(yh[:, k], k)
+
+
 def test_block_apply_and_kernel_apply(wpcd):
     """batched dense blocks (FP64 MMA) and the factored kernel K = O P0 O^T V1 G1 against
     the numpy oracle, on a lattice whose block sizes are not multiples of the 32 x 32 tile."""

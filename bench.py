@@ -393,6 +393,19 @@ def run_ours(args):
         spmm["kernel_apply_ms"] = a.elapsed_time(b) / reps
         spmm["kernel_apply_dense_gflop"] = 3 * 2.0 * n_ch * grid.n_p ** 2 * (2 * grid.n_q) / 1e9
 
+        # the dependent products of the iteration in one call (wpcd_perm_apply_chain): small matrices only
+        if wl.model == "swave":
+            n_it = 50
+            ych = torch.empty(n_it, job.rows, dtype=torch.float64, device="cuda")
+            for _ in range(3):
+                wpcd.wpcd_perm_apply_chain(job.rows, job.row_ptr, job.col_idx, job.values, x4[0], ych, n_it)
+            a.record()
+            for _ in range(5):
+                wpcd.wpcd_perm_apply_chain(job.rows, job.row_ptr, job.col_idx, job.values, x4[0], ych, n_it)
+            b.record()
+            torch.cuda.synchronize()
+            spmm["chain50_us_per_product"] = a.elapsed_time(b) / 5 / n_it * 1e3
+
     # ---- end to end through the C-ABI with HOST buffers (handles, tables and vectors from the host)
     def e2e_step():
         g2 = wpcd.wpcd_grid_create(p, p)

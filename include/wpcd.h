@@ -168,6 +168,18 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
                                         const double* values_dev, const double* x_dev, double* y_dev, int n_inter,
                                         void* cuda_stream);
 
+/* The dependent products of the simple iteration (paper step 5; Neumann terms):
+ * y_k = P0 y_{k-1}, k = 1 .. n_iter, y_0 = x.  y_dev holds all iterates, y_dev[(k-1)*rows + r] = (P0^k x)[r], dev;
+ * x_dev [rows], dev, must not overlap y_dev.  A matrix in the size window where it pays (about 1.6e4 <= nnz <=
+ * 1.6e5 on a B200, measured: spmv_chain.cu) runs the whole chain in ONE cooperative launch -- row slices resident
+ * in shared memory, a grid-wide barrier between products; any other matrix takes n_iter ordinary products on the
+ * stream.  Either way a row is summed in a fixed lane order (deterministic), but the two orders differ, so results
+ * agree to rounding, not bit for bit, across the two paths.  Asynchronous.  At most 64 fused chains in flight per
+ * device (the barrier counters are a ring). */
+wpcd_status wpcd_perm_apply_chain(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
+                                  const double* values_dev, const double* x_dev, double* y_dev, int n_iter,
+                                  void* cuda_stream);
+
 /* Next step of SURVEY.md section 8(f): the kernel of eq. (12) in factored form.
  * wpcd_block_apply: for every channel gamma, Y_gamma = A_gamma X_gamma (transpose = 0) or A_gamma^T X_gamma
  * (transpose != 0), where X_gamma is the n_p x n_q block x_dev[(gamma*n_p + i)*n_q + j] of the vector and

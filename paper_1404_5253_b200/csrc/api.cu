@@ -674,6 +674,32 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
     return WPCD_OK;
 }
 
+wpcd_status wpcd_perm_apply_chain(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                  const double* x_dev, double* y_dev, int n_iter, void* cuda_stream)
+{
+    if (rows < 0 || n_iter < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: negative size");
+    if (rows == 0 || n_iter == 0) return WPCD_OK;
+    if (!row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: null pointer");
+    if (x_dev + rows > y_dev && y_dev + (int64_t)n_iter * rows > x_dev)
+        return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: x overlaps y");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
+    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: null matrix arrays");
+    int fused = 0;
+    cudaError_t err = launch_spmv_chain(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_iter, mean_row, st, &fused);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_chain");
+    if (!fused) {
+        const double* xin = x_dev;
+        for (int k = 0; k < n_iter; ++k) {
+            double* yk = y_dev + (int64_t)k * rows;
+            err = launch_spmv(rows, row_ptr_dev, col_idx_dev, values_dev, xin, yk, 1, mean_row, st);
+            if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_chain");
+            xin = yk;
+        }
+    }
+    return WPCD_OK;
+}
+
 wpcd_status wpcd_block_apply(int n_channels, int n_p, int n_q, const double* a_dev, int transpose, const double* x_dev,
                              double* y_dev, int complex_vectors, void* cuda_stream)
 {

@@ -546,6 +546,66 @@ def test_apply_row_length_sweep(wpcd):
                 check(yh[:, k], k)
 
 
+def _chain_check(wpcd, torch, rows, rp, ci, v, rpd, cid, vd, n_iter, tag):
+    xh = wi.normal_vector(rows, k=900)
+    x = torch.from_numpy(xh).cuda()
+    y = torch.full((n_iter, rows), np.nan, dtype=torch.float64, device="cuda")
+    wpcd.wpcd_perm_apply_chain(rows, rpd, cid, vd, x, y, n_iter)
+    yh = y.cpu().numpy()
+    ref, scale = xh, np.abs(xh)
+    av = np.abs(v)
+    for k in range(n_iter):
+        ref = operm.spmv(rp, ci, v, ref)
+        scale = operm.spmv(rp, ci, av, scale)                   # |P0|^k |x|: what rounding errors are relative to
+        assert np.all(np.abs(yh[k] - ref) <= (k + 1) * 2e-12 * scale + 1e-300), (tag, k)
+
+
+def test_apply_chain(wpcd):
+    """The dependent products y_k = P0 y_{k-1} in one cooperative launch (matrix slices resident in shared memory, grid
+    barrier between products) against the oracle's product applied n_iter times; also the slices that do not fit
+    (one very long row), empty rows, and a matrix too large for the scheme (ordinary products)."""
+    torch = _torch()
+    for n_bins, n_iter in ((24, 7), (50, 20), (100, 50)):      # N = 50 lies in the window where the fused launch is the default
+        p = wi.tan2_grid(n_bins, 1.0, 0.1, seed=8)
+        m = wpcd.build_perm(wpcd.wpcd_grid_create(p, p), wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5), 8)
+        rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+        _chain_check(wpcd, torch, m.rows, rp, ci, v, m.row_ptr, m.col_idx, m.values, n_iter, ("swave", n_bins))
+    p2 = wi.tan2_grid(10, 1.0, 0.1, seed=61)
+    m = wpcd.build_perm(wpcd.wpcd_grid_create(p2, p2), wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=1, two_T=1, j_pair_max=2), 6)
+    rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    _chain_check(wpcd, torch, m.rows, rp, ci, v, m.row_ptr, m.col_idx, m.values, 5, "coupled")
+    rng = np.random.default_rng(78)
+    for rows, short, long_, every, n_iter, tag in ((3000, 6, 40000, 2999, 4, "one long row"), (5000, 0, 60, 3, 6, "empty rows"),
+                                                  (40000, 90, 90, 1, 3, "too large: ordinary products"), (37, 3, 3, 1, 1, "n_iter 1")):
+        lens = np.full(rows, short, dtype=np.int64)
+        lens[::every] = long_
+        rp = np.zeros(rows + 1, dtype=np.int64)
+        rp[1:] = np.cumsum(lens)
+        nnz = int(rp[-1])
+        ci = rng.integers(0, rows, nnz).astype(np.int32)
+        v = rng.standard_normal(nnz) / np.sqrt(max(short, 1) + long_ / every)
+        _chain_check(wpcd, torch, rows, rp, ci, v, torch.from_numpy(rp).cuda(), torch.from_numpy(ci).cuda(), torch.from_numpy(v).cuda(),
+                     n_iter, tag)
+
+
+def test_apply_chain_fused_everywhere():
+    """The same chain cases with the fused cooperative launch forced on for every matrix that fits on chip
+    (WPCD_FORCE_CHAIN=1 is read once per process, hence the child process)."""
+    import os
+    import subprocess
+    import sys
+
+    if os.environ.get("WPCD_FORCE_CHAIN") == "1":
+        pytest.skip("already inside the forced run")
+    env = dict(os.environ, WPCD_FORCE_CHAIN="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-m", "gpu", "-x", "-q",
+                        "-k", "test_apply_chain and not fused_everywhere", "-p", "no:cacheprovider"],
+                       env=env, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert "1 passed" in r.stdout
+
+
 def test_block_apply_and_kernel_apply(wpcd):
     """batched dense blocks (FP64 MMA) and the factored kernel K = O P0 O^T V1 G1 against
     the numpy oracle, on a lattice whose block sizes are not multiples of the 32 x 32 tile."""

@@ -40,6 +40,8 @@ def lib():
         L.wpo_geo_fill.argtypes = [i32, i32, _D, _D, _I64, _I32]
         L.wpo_elements.argtypes = [i32, i32, _D, _D, i64, _I32, _I32, _I32, _I32, i32, _D, _D,
                                    i32, _I32, _I32, _I64, _I32, _I32, _I32, _D, _D, _D]
+        L.wpo_elements_rule.argtypes = [i32, i32, _D, _D, i64, _I32, _I32, _I32, _I32, i32, _D, _D, i32,
+                                        i32, _I32, _I32, _I64, _I32, _I32, _I32, _D, _D, _D]
         L.wpo_spmv.argtypes = [i64, _I64, _I32, _D, _D, _D]
         L.wpo_num_threads.restype = ctypes.c_int
         _lib = L
@@ -101,9 +103,9 @@ def gauss_legendre(n):
     return np.ascontiguousarray(xi), np.ascontiguousarray(w)
 
 
-def element_values(p, q, ei, ej, eip, ejp, n_quad, table):
-    """Values (A15) by rule R(n_quad) of the listed geometric elements, all pairs.
-    Returns (val, absval), each [n_elem, n_pairs]."""
+def element_values(p, q, ei, ej, eip, ejp, n_quad, table, split=False):
+    """Values (A15) by rule R(n_quad) -- or the kink-split rule RS(n_quad) if split -- of the listed
+    geometric elements, all pairs.  Returns (val, absval), each [n_elem, n_pairs]."""
     p = np.ascontiguousarray(p, np.float64)
     q = np.ascontiguousarray(q, np.float64)
     ei, ej, eip, ejp = (np.ascontiguousarray(v, np.int32) for v in (ei, ej, eip, ejp))
@@ -111,7 +113,7 @@ def element_values(p, q, ei, ej, eip, ejp, n_quad, table):
     ne = len(ei)
     val = np.zeros((ne, table.n_pairs))
     absval = np.zeros((ne, table.n_pairs))
-    lib().wpo_elements(len(p) - 1, len(q) - 1, p, q, ne, ei, ej, eip, ejp, n_quad, xi, w,
+    lib().wpo_elements_rule(len(p) - 1, len(q) - 1, p, q, ne, ei, ej, eip, ejp, n_quad, xi, w, 1 if split else 0,
                        table.n_pairs, table.pair_l, table.pair_lp, table.term_ptr, table.term_k,
                        table.term_l1, table.term_l1p, table.term_g, val, absval)
     return val, absval
@@ -128,7 +130,7 @@ def full_row_ptr(geo_ptr, table, n_p, n_q):
     return ptr
 
 
-def build_csr(p, q, n_quad, table, geo=None, geo_rows=None):
+def build_csr(p, q, n_quad, table, geo=None, geo_rows=None, split=False):
     """Full CSR (row_ptr, col_idx, values, absvalues) of P0.
 
     If geo_rows is given, values are computed only for those geometric rows (all
@@ -164,7 +166,7 @@ def build_csr(p, q, n_quad, table, geo=None, geo_rows=None):
         erow = np.repeat(rows, cnts)
         eidx = np.concatenate([np.arange(geo_ptr[r], geo_ptr[r + 1]) for r in rows]) if len(rows) else np.zeros(0, np.int64)
         ecol = geo_col[eidx]
-        val, absval = element_values(p, q, erow // n_q, erow % n_q, ecol // n_q, ecol % n_q, n_quad, table)
+        val, absval = element_values(p, q, erow // n_q, erow % n_q, ecol // n_q, ecol % n_q, n_quad, table, split=split)
         pos_in_row = eidx - geo_ptr[erow]
         for g in range(table.n_ch):
             coupled = np.nonzero(table.mask[g])[0]

@@ -16,6 +16,7 @@
  *   wpo_geo_count/fill geometric CSR pattern (rows (i,j), columns (i',j') ascending)
  *   wpo_elements       values of listed geometric elements for all coupled channel
  *                      pairs by the rule R(n) (R7) applied to (A15)
+ *   wpo_elements_rule  the same with the kink-split rule RS(n) (R14) when split != 0
  *   wpo_spmv           sequential CSR y = P0 x
  *
  * Pins: tests/test_oracle_*.py (Cartesian (A7) brute force, single-cell constant,
@@ -177,7 +178,7 @@ void wpo_geo_fill(int n_p, int n_q, const double* p, const double* q,
 #define WPO_MAXPOW 24
 static void element_values(double a, double b, double c, double d,
                            double L1, double U1, double L2, double U2,
-                           int n, const double* xi, const double* w,
+                           int n, const double* xi, const double* w, int split,
                            int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
                            const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
                            const int32_t* term_l1p, const double* term_g,
@@ -197,7 +198,23 @@ static void element_values(double a, double b, double c, double d,
     }
     if (!(phi_a < phi_b)) return;
     double norm = 1.0 / sqrt((U2 - L2) * (b - a) * (U1 - L1) * (d - c)); /* (d_i dbar_j d_i' dbar_j')^{-1/2}, A5/A9 */
-    double half_phi = 0.5 * (phi_b - phi_a), mid_phi = 0.5 * (phi_a + phi_b);
+    /* Rule R(n): one piece in phi, one piece in u.  Rule RS(n) (split != 0, R14): the phi-range is
+     * cut at the rectangle-corner angles where the active member of Lq = max(a/C, c/S) or Uq = min(b/C, d/S)
+     * switches (tan phi = c/a, tan phi = d/b), and at every phi-node the u-range is cut at the abscissae where two
+     * members of Qmax = min(Uq, U1/zeta1, U2/zeta2) or of Qmin = max(Lq, L1/zeta1, L2/zeta2) of (A14) cross
+     * (zeta^2 is linear in u, so each crossing is a closed form); n-point Gauss-Legendre on every piece. */
+    double phi_cut[4];
+    int n_phi_piece = 1;
+    phi_cut[0] = phi_a;
+    if (split) {
+        double c1 = atan2(c, a), c2 = atan2(d, b);
+        double lo = fmin(c1, c2), hi = fmax(c1, c2);
+        if (lo > phi_a && lo < phi_b) phi_cut[n_phi_piece++] = lo;
+        if (hi > phi_cut[n_phi_piece - 1] && hi < phi_b) phi_cut[n_phi_piece++] = hi;
+    }
+    phi_cut[n_phi_piece] = phi_b;
+    for (int piece = 0; piece < n_phi_piece; ++piece) {
+    double half_phi = 0.5 * (phi_cut[piece + 1] - phi_cut[piece]), mid_phi = 0.5 * (phi_cut[piece] + phi_cut[piece + 1]);
     for (int m = 0; m < n; ++m) {
         double phi = mid_phi + half_phi * xi[m];
         double wphi = half_phi * w[m];
@@ -231,11 +248,36 @@ static void element_values(double a, double b, double c, double d,
             else if (!(0.0 < R)) continue;
         }
         if (!(u_lo < u_hi)) continue;
-        double half_u = 0.5 * (u_hi - u_lo), mid_u = 0.5 * (u_lo + u_hi);
+        double u_cut[8];
+        int n_u_piece = 1;
+        u_cut[0] = u_lo;
+        if (split) {
+            double cand[6];
+            int nc = 0;
+            cand[nc++] = ((U1 / Uq) * (U1 / Uq) - b1) / beta;                         /* Uq = U1/zeta1 */
+            cand[nc++] = ((U2 / Uq) * (U2 / Uq) - b2) / beta;                         /* Uq = U2/zeta2 */
+            if (U1 != U2) cand[nc++] = (U2 * U2 * b1 - U1 * U1 * b2) / (beta * (U1 * U1 - U2 * U2)); /* U1/zeta1 = U2/zeta2 */
+            if (Lq > 0.0) {
+                cand[nc++] = ((L1 / Lq) * (L1 / Lq) - b1) / beta;                     /* Lq = L1/zeta1 */
+                cand[nc++] = ((L2 / Lq) * (L2 / Lq) - b2) / beta;                     /* Lq = L2/zeta2 */
+            }
+            if (L1 != L2) cand[nc++] = (L2 * L2 * b1 - L1 * L1 * b2) / (beta * (L1 * L1 - L2 * L2)); /* L1/zeta1 = L2/zeta2 */
+            for (int i1 = 1; i1 < nc; ++i1) {                                         /* ascending */
+                double key = cand[i1];
+                int i0 = i1 - 1;
+                while (i0 >= 0 && cand[i0] > key) { cand[i0 + 1] = cand[i0]; --i0; }
+                cand[i0 + 1] = key;
+            }
+            for (int i1 = 0; i1 < nc; ++i1)
+                if (cand[i1] > u_cut[n_u_piece - 1] && cand[i1] < u_hi) u_cut[n_u_piece++] = cand[i1];
+        }
+        u_cut[n_u_piece] = u_hi;
         /* powers of cos, sin */
         double cp[WPO_MAXPOW], sp[WPO_MAXPOW];
         cp[0] = 1.0; sp[0] = 1.0;
         for (int e = 1; e < WPO_MAXPOW; ++e) { cp[e] = cp[e - 1] * C; sp[e] = sp[e - 1] * S; }
+        for (int upiece = 0; upiece < n_u_piece; ++upiece) {
+        double half_u = 0.5 * (u_cut[upiece + 1] - u_cut[upiece]), mid_u = 0.5 * (u_cut[upiece] + u_cut[upiece + 1]);
         for (int r = 0; r < n; ++r) {
             double u = mid_u + half_u * xi[r];
             double x = u - 1.0;
@@ -270,12 +312,33 @@ static void element_values(double a, double b, double c, double d,
                 absval[cidx] += wF * asum / denom;
             }
         }
+        } /* u pieces */
     }
+    } /* phi pieces */
     for (int cidx = 0; cidx < n_pairs; ++cidx) { val[cidx] *= norm; absval[cidx] *= norm; }
 }
 
 /* Values of n_elem listed geometric elements (row cell (ei,ej), column cell (eip,ejp),
  * all 0-based bin indices).  val/absval are [n_elem][n_pairs], row-major. */
+void wpo_elements_rule(int n_p, int n_q, const double* p, const double* q,
+                       int64_t n_elem, const int32_t* ei, const int32_t* ej, const int32_t* eip, const int32_t* ejp,
+                       int n, const double* xi, const double* w, int split,
+                       int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
+                       const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
+                       const int32_t* term_l1p, const double* term_g,
+                       double* val, double* absval)
+{
+    (void)n_p; (void)n_q;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t e = 0; e < n_elem; ++e) {
+        int i = ei[e], j = ej[e], ip = eip[e], jp = ejp[e];
+        element_values(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1],
+                       n, xi, w, split, n_pairs, pair_l, pair_lp, term_ptr, term_k, term_l1, term_l1p, term_g,
+                       val + e * n_pairs, absval + e * n_pairs);
+    }
+}
+
+/* rule R(n) */
 void wpo_elements(int n_p, int n_q, const double* p, const double* q,
                   int64_t n_elem, const int32_t* ei, const int32_t* ej, const int32_t* eip, const int32_t* ejp,
                   int n, const double* xi, const double* w,
@@ -284,14 +347,8 @@ void wpo_elements(int n_p, int n_q, const double* p, const double* q,
                   const int32_t* term_l1p, const double* term_g,
                   double* val, double* absval)
 {
-    (void)n_p; (void)n_q;
-#pragma omp parallel for schedule(dynamic, 16)
-    for (int64_t e = 0; e < n_elem; ++e) {
-        int i = ei[e], j = ej[e], ip = eip[e], jp = ejp[e];
-        element_values(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1],
-                       n, xi, w, n_pairs, pair_l, pair_lp, term_ptr, term_k, term_l1, term_l1p, term_g,
-                       val + e * n_pairs, absval + e * n_pairs);
-    }
+    wpo_elements_rule(n_p, n_q, p, q, n_elem, ei, ej, eip, ejp, n, xi, w, 0, n_pairs, pair_l, pair_lp, term_ptr, term_k, term_l1,
+                      term_l1p, term_g, val, absval);
 }
 
 /* y = P0 x, CSR, each row summed sequentially in column order. */

@@ -277,3 +277,84 @@ def test_rule_converges_with_order(swave_table):
     assert 1e-2 < errs[8] < 4e-2 and errs[32] < 2e-3
     rate = np.log(errs[8] / errs[32]) / np.log(4.0)
     assert 1.0 < rate < 3.0
+
+
+# ---- kink-split rule RS(n) (R14; SURVEY.md section 8(c) item 7 "optional refinements", 8(f) item 4) ----
+def test_split_rule_converges_faster(swave_table):
+    """RS(n) cuts phi at the rectangle-corner angles and u at the crossings of the members of (A14)'s min/max.
+    Pins: (1) it converges to the SAME limit as R(n) (a wrong cut or a dropped piece would converge elsewhere);
+    (2) the survey's probe figure for this lattice: RS(8) reaches 1.9e-3 where R(8) has 2.1e-2; (3) monotone."""
+    p = wi.tan2_grid(12, 1.0, 0.1, seed=3)
+    geo = perm.geo_pattern(p, p)
+    ref_split = perm.build_csr(p, p, 64, swave_table, geo=geo, split=True)[2]
+    ref_plain = perm.build_csr(p, p, 64, swave_table, geo=geo)[2]
+    nrm = np.linalg.norm(ref_split)
+    assert np.linalg.norm(ref_plain - ref_split) / nrm < 5e-4          # R(64) itself is only good to ~3e-4
+    errs, errs_plain = {}, {}
+    for n in (4, 8, 16, 32):
+        errs[n] = np.linalg.norm(perm.build_csr(p, p, n, swave_table, geo=geo, split=True)[2] - ref_split) / nrm
+        errs_plain[n] = np.linalg.norm(perm.build_csr(p, p, n, swave_table, geo=geo)[2] - ref_split) / nrm
+    assert errs[4] > errs[8] > errs[16] > errs[32]
+    assert 1.5e-3 < errs[8] < 2.3e-3                                    # SURVEY: "with both, n=8 reaches 1.9e-3"
+    for n in (4, 8, 16, 32):
+        assert errs[n] < errs_plain[n] / 5.0
+
+
+def test_split_rule_against_cartesian_A7(swave_table, nd_half_plus_j1):
+    """The split rule against the unreduced (q,q',x) brute force: s-wave elements of a lattice with different p and q
+    grids, and multichannel pairs with l != l' (catches a cut placed with the wrong cell's bounds: such a rule still
+    converges, but a piece dropped or counted twice does not)."""
+    p = wi.tan2_grid(5, 1.0, 0.1, seed=3)
+    q = wi.tan2_grid(4, 0.7, 0.1, seed=4)
+    ptr, col = perm.geo_pattern(p, q)
+    n_q = len(q) - 1
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    v, _ = perm.element_values(p, q, rows // n_q, rows % n_q, col // n_q, col % n_q, 16, swave_table, split=True)
+    v_ref, _ = perm.element_values(p, q, rows // n_q, rows % n_q, col // n_q, col % n_q, 64, swave_table)
+    assert np.abs(v - v_ref).max() < 2e-3 * np.abs(v_ref).max()
+    worst = 0.0
+    for e in range(0, len(col), 3):
+        i, j, ip, jp = rows[e] // n_q, rows[e] % n_q, col[e] // n_q, col[e] % n_q
+        ref = brute.element(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1], 0, 0, [(0, 0, 0, 1.0)], m=160)
+        worst = max(worst, abs(v[e, 0] - ref))
+    assert worst < 4e-3 * np.abs(v).max()
+    tab = nd_half_plus_j1
+    p3 = wi.tan2_grid(3, 1.0, 0.1, seed=5)
+    q3 = wi.tan2_grid(3, 0.8, 0.1, seed=6)
+    ptr, col = perm.geo_pattern(p3, q3)
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    sel = [e for e in range(len(col)) if min(rows[e] // 3, col[e] // 3) >= 1][:6]
+    vs, avs = perm.element_values(p3, q3, rows[sel] // 3, rows[sel] % 3, col[sel] // 3, col[sel] % 3, 32, tab, split=True)
+    vp, _ = perm.element_values(p3, q3, rows[sel] // 3, rows[sel] % 3, col[sel] // 3, col[sel] % 3, 64, tab)
+    assert np.all(np.abs(vs - vp) <= 1.5e-3 * np.maximum(avs, 1e-3))     # same limit as R(n): R(64) is good to ~1e-3 here
+    pick = [c for c in range(tab.n_pairs) if tab.pair_l[c] != tab.pair_lp[c] and min(tab.pair_l[c], tab.pair_lp[c]) >= 1][:3]
+    for c in pick:
+        terms = [(tab.term_k[t], tab.term_l1[t], tab.term_l1p[t], tab.term_g[t]) for t in range(tab.term_ptr[c], tab.term_ptr[c + 1])]
+        for n_e, e in enumerate(sel[:3]):
+            i, j, ip, jp = rows[e] // 3, rows[e] % 3, col[e] // 3, col[e] % 3
+            ref = brute.element(q3[j], q3[j + 1], q3[jp], q3[jp + 1], p3[ip], p3[ip + 1], p3[i], p3[i + 1],
+                                int(tab.pair_l[c]), int(tab.pair_lp[c]), terms, m=120)
+            assert abs(vs[n_e, c] - ref) < 1e-2 * max(avs[n_e, c], 1e-3), (c, e)
+
+
+def test_split_rule_single_cell(swave_table):
+    """Single cell [0,1]^4 (golden constant C1 = 1.5056 +- 1e-4 of SURVEY.md section 8(c)): RS(n) is closer than R(n)
+    at every order and reaches the constant; the 1/zeta corner keeps even RS algebraic."""
+    gold = dict(line.split() for line in open(GOLD) if line.strip() and not line.startswith("#"))
+    c1 = float(gold["C1"])
+    p = np.array([0.0, 1.0])
+    for n in (8, 32, 128):
+        vs, _ = perm.element_values(p, p, [0], [0], [0], [0], n, swave_table, split=True)
+        vp, _ = perm.element_values(p, p, [0], [0], [0], [0], n, swave_table)
+        assert abs(vs[0, 0] - c1) < abs(vp[0, 0] - c1) + 1e-4
+    assert abs(vs[0, 0] - c1) < 1.5e-4
+
+
+def test_split_rule_symmetric_matrix(swave_table):
+    """P0 is symmetric (same integral with the two Jacobi sets exchanged).  On a q == p lattice the
+    exchange maps phi -> pi/2 - phi and every cut of RS(n) onto a cut of the transposed element, so the rule's matrix
+    is symmetric to rounding -- a cut taken from the wrong cell's bounds breaks this at the 1e-3 level."""
+    p = wi.tan2_grid(10, 1.0, 0.1, seed=11)
+    rp, ci, v, _ = perm.build_csr(p, p, 8, swave_table, split=True)
+    m = _dense(rp, ci, v)
+    assert np.abs(m - m.T).max() < 1e-12 * np.abs(m).max()

@@ -406,6 +406,23 @@ def run_ours(args):
             torch.cuda.synchronize()
             spmm["chain50_us_per_product"] = a.elapsed_time(b) / 5 / n_it * 1e3
 
+    # ---- extra: the kink-split rule RS(n) (R14): cost of the build against R(n)
+    rule_split = {}
+    job = jobs[-1]
+    for name, nq in (("plain", wl.n_quad), ("split", wl.n_quad | wpcd.WPCD_RULE_KINK_SPLIT)):
+        reps = 3 if wl.model == "swave" else 1
+        for _ in range(1):
+            wpcd.wpcd_perm_build(grid, job.channels, nq, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            wpcd.wpcd_perm_build(grid, job.channels, nq, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+        b.record()
+        torch.cuda.synchronize()
+        rule_split["build_ms_" + name] = a.elapsed_time(b) / reps
+    wpcd.wpcd_perm_build(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+    torch.cuda.synchronize()
+
     # ---- end to end through the C-ABI with HOST buffers (handles, tables and vectors from the host)
     def e2e_step():
         g2 = wpcd.wpcd_grid_create(p, p)
@@ -511,7 +528,7 @@ def run_ours(args):
         "stage_ms_per_step": share,
         "build_nnz_per_s": nnz1 / max(1e-12, (ms_per_step - spmv_ms / steps) * 1e-3),
         "fp64_peak_tflops_measured": fp64_peak / 1e12,
-        "spmm_nvec4": spmm,
+        "spmm_nvec4": spmm, "rule_split": rule_split,
         "cpu_baseline": cpu_baseline,
     }
     print(json.dumps(line))

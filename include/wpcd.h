@@ -53,6 +53,7 @@ typedef int wpcd_status;
 #define WPCD_ERR_UNSUPPORTED (-6)   /* n_quad, l or k beyond WPCD_MAX_* */
 
 #define WPCD_MAX_QUAD 64            /* Gauss-Legendre points per dimension (paper: 48, l.334) */
+#define WPCD_RULE_KINK_SPLIT 0x100   /* OR into n_quad: the kink-split rule RS(n) of DESIGN.md R14 */
 #define WPCD_MAX_L 7                /* largest pair orbital momentum l */
 #define WPCD_MAX_K 23               /* largest Legendre order k in (A3) */
 
@@ -136,6 +137,9 @@ size_t wpcd_perm_workspace_bytes(const wpcd_channels* channels, int64_t nnz_geo)
  * channel-pair sum (A3), by the rule R(n_quad) of DESIGN.md R7: n_quad-point Gauss-Legendre
  * in phi over the angular extent of the overlap polygon, and at every phi-node n_quad-point
  * Gauss-Legendre in x over the closed-form support of F.  1 <= n_quad <= WPCD_MAX_QUAD.
+ * n_quad | WPCD_RULE_KINK_SPLIT selects the kink-split rule RS(n_quad) of DESIGN.md R14 instead (the phi-range cut at
+ * the rectangle-corner angles, the x-range at the crossings of the members of (A14)'s min / max; about ten times
+ * the accuracy and ten times the cost of R(n_quad)); the pattern (wpcd_perm_count) does not depend on the rule.
  * Coupled channels: a channel pair may use any number of (k, l1+l1') monomials (more than 32 are
  * handled in several passes); WPCD_ERR_CUDA "invalid argument" if the tables exceed shared memory.
  * Asynchronous on the stream. */

@@ -23,6 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libwpcd.so")
 
 WPCD_SPINLESS_SWAVE = 0
 WPCD_ND = 1
+WPCD_RULE_KINK_SPLIT = 0x100   # OR into n_quad: kink-split rule RS(n) (R14)
 WPCD_MAX_QUAD = 64
 
 EXPORTS = [

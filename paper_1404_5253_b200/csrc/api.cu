@@ -538,6 +538,7 @@ wpcd_status wpcd_perm_count(const wpcd_grid* g_in, const wpcd_channels* c, int n
 {
     if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_count: null pointer");
+    n_quad &= ~WPCD_RULE_KINK_SPLIT;       // the pattern does not depend on the rule
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_count: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_count: channel tables are not on a device (no CUDA device?)");
     wpcd_grid* g = const_cast<wpcd_grid*>(g_in);   // the staging scratch inside the handle is mutable state
@@ -568,6 +569,8 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
                             double* values_dev)
 {
     if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
+    const bool split = (n_quad & WPCD_RULE_KINK_SPLIT) != 0;
+    n_quad &= ~WPCD_RULE_KINK_SPLIT;
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_build: channel tables are not on a device (no CUDA device?)");
     wpcd_grid* g = const_cast<wpcd_grid*>(g_in);
@@ -605,8 +608,8 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
         std::memcpy(xi, tab.data(), sizeof(double) * n_quad);
         std::memcpy(w, tab.data() + n_quad, sizeof(double) * n_quad);
     }
-    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
-    else err = launch_fill_coupled(g, c, n_quad, xi, w, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
+    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, split, xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
+    else err = launch_fill_coupled(g, c, n_quad, split, xi, w, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(fill)");
     return WPCD_OK;
 }

@@ -71,11 +71,85 @@ fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, in
     }
 }
 
+// ------------------------------------------------------------------ s-wave, kink-split rule RS(n) (R14)
+// The work items of an element are its (phi-piece, phi-node) pairs, dealt to the LPE lanes; each item integrates its
+// u-pieces one after the other (sorted candidate cuts in registers, no arrays).
+template <int LPE, int NQ>
+__global__ void __launch_bounds__(256)
+fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n_rt, double g0,
+                        int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
+                        const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t e = t / LPE;
+    const int sub = (int)(t - e * LPE);
+    const bool valid = e < nnz_geo;
+    const int n = NQ > 0 ? NQ : n_rt;
+    double acc = 0.0;
+    double norm = 0.0;
+    int col = 0;
+    if (valid) {
+        col = geo_col[e];
+        const int row = geo_row[e];
+        const double2 ph = geo_phi[e];
+        const Cell z = load_cell(p, q, n_q, row, col);
+        const CellSq zs = square_cell(z);
+        norm = cell_norm(z);
+        if (ph.x < ph.y) {
+            double pc[SPLIT_MAX_PHI + 1];
+            const int n_piece = split_phi(z, ph.x, ph.y, pc);
+#pragma unroll 1
+            for (int item = sub; item < n_piece * n; item += LPE) {
+                const int piece = item / n, m = item - piece * n;
+                const double pa = piece == 0 ? pc[0] : (piece == 1 ? pc[1] : pc[2]);
+                const double pb = piece == 0 ? pc[1] : (piece == 1 ? pc[2] : pc[3]);
+                const double half_phi = 0.5 * (pb - pa), mid_phi = 0.5 * (pa + pb);
+                PhiNodeSq s;
+                if (!phi_node_sq(z, zs, mid_phi + half_phi * c_xi[m], s)) continue;
+                double cand[6];
+                split_u_candidates(z, zs, s, cand);
+                auto piece_sum = [&](double lo, double hi) {
+                    const double half_u = 0.5 * (hi - lo), mid_u = 0.5 * (lo + hi);
+                    double inner = 0.0;
+#pragma unroll
+                    for (int r = 0; r < n; ++r) {
+                        const double u = mid_u + half_u * c_xi[r];
+                        const double z1 = s.b1 + s.beta * u, z2 = s.b2 + s.beta * u;    // zeta1^2, zeta2^2 (A11)
+                        const double t = rsqrt(z1 * z2);                                // 1/(zeta1 zeta2)
+                        const double t2 = t * t;
+                        inner += c_w[r] * twoF_A14_sq(zs, s, t2 * z2, t2 * z1) * t;
+                    }
+                    return half_u * inner;
+                };
+                // cut list in local memory (8 doubles, L1-resident): one copy of the inner rule instead of seven
+                double cut[SPLIT_MAX_U + 1];
+                int np = 1;
+                cut[0] = s.u_lo;
+#pragma unroll
+                for (int i = 0; i < 6; ++i) {
+                    if (cand[i] > cut[np - 1] && cand[i] < s.u_hi) cut[np++] = cand[i];
+                }
+                cut[np] = s.u_hi;
+                double node = 0.0;
+#pragma unroll 1
+                for (int k = 0; k < np; ++k) node += piece_sum(cut[k], cut[k + 1]);
+                acc += half_phi * c_w[m] * s.beta * node;    // cos*sin = beta
+            }
+        }
+    }
+#pragma unroll
+    for (int o = LPE / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (valid && sub == 0) {
+        values[e] = 0.5 * g0 * norm * acc;    // the 1/2 of (A14)
+        col_idx[e] = col;
+    }
+}
+
 }  // namespace
 
 namespace wpcd_detail {
 
-cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, const double* xi, const double* w,
+cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
                               int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st)
 {
     // the rule's nodes and weights live in constant memory; they are uploaded again only when the
@@ -102,6 +176,16 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     StageTimer timer(WPCD_STAGE_FILL_SWAVE, st);
 #define WPCD_LAUNCH_SW(L, Q) fill_swave_kernel<L, Q><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
                                                                             ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
+    if (split) {
+        // the rule has up to 3 n work items per element: eight lanes each
+        lpe = 8; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256);
+        if (n_quad == 8) fill_swave_split_kernel<8, 8><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,
+                                                                                ws.geo_row, ws.geo_phi, col_idx, values);
+        else fill_swave_split_kernel<8, 0><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,
+                                                                    ws.geo_row, ws.geo_phi, col_idx, values);
+        ++g_launches;
+        return cudaGetLastError();
+    }
     // order 8: two lanes per element once there are enough elements to fill the chip (the per-element
     // prologue -- cell loads, normalisation -- is then paid twice instead of eight times), eight lanes otherwise
     if (n_quad == 8 && nnz_geo >= 65536) { lpe = 2; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256); WPCD_LAUNCH_SW(2, 8); }

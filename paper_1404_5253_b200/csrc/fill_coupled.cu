@@ -44,6 +44,7 @@ __constant__ double k_invk[WPCD_MAX_K + 2];   // 1/k for the Legendre recurrence
 
 struct MomentShape {
     int n;        // quadrature order
+    int NS;       // phi-node slots staged per warp: n, or max(n, 28) for the kink-split rule (7 u-pieces x 4 items)
     int G;        // phi-nodes handled together by the node set-up
     int K1;       // k_max + 1
     int SP;       // row stride of the P_k table:  8 ceil(K1 / 8) + 4   (conflict-free fragment loads)
@@ -58,7 +59,7 @@ struct MomentShape {
 __host__ __device__ inline int moment_smem_doubles(const MomentShape& s)
 {
     const int rows = s.G * s.n;
-    return (s.n * NODE_F + rows * (s.SP + s.ST) + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;   // even: 16-byte pieces
+    return (s.NS * NODE_F + rows * (s.SP + s.ST) + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;   // even: 16-byte pieces
 }
 
 // D (8x8) += A (8x4, row) * B (4x8, col), FP64 tensor-core MMA.  Fragment layout: a = A[lane/4][lane%4],
@@ -101,7 +102,7 @@ __device__ __forceinline__ double ipow_small(double b, int e)   // e < 64
 
 // Moment layout: [tile of 32 elements][mu][element in tile] (the contraction reads 32 elements of
 // one monomial as one 256-byte line).
-template <int MAXS>
+template <int MAXS, bool SPLIT>
 __global__ void __launch_bounds__(MOM_WARPS * 32)
 moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
@@ -124,8 +125,8 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     const int64_t e = e_begin + (int64_t)blockIdx.x * MOM_WARPS + warp;
     if (e >= e_end) return;
     const bool full_ll = n_ll == LM1 * LM1;                           // every (l, l') present: ll = l * LM1 + l'
-    double* nodeS = wbase + (size_t)warp * moment_smem_doubles(sh);   // [n][NODE_F]
-    double* Pk = nodeS + n * NODE_F;                                  // [G*n][SP]    P_k(x_r)
+    double* nodeS = wbase + (size_t)warp * moment_smem_doubles(sh);   // [NS][NODE_F]
+    double* Pk = nodeS + sh.NS * NODE_F;                                  // [G*n][SP]    P_k(x_r)
     double* T = Pk + G * n * SP;                                      // [G*n][ST]    T_r[l,l']
     double* Ib = T + G * n * ST;                                      // [K1][IS]     I[k][l,l'] of one phi-node
     double* cs = Ib + K1 * IS;                                        // [G][2][CP]   powers of cos, sin
@@ -151,18 +152,11 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     const double norm = cell_norm(z);
     const double half_phi = 0.5 * (ph.y - ph.x), mid_phi = 0.5 * (ph.x + ph.y);
     const int MT = (SP - 4) >> 3, NT = (ST - 4) >> 3, KT = (n + 3) >> 2;
-    if (ph.x < ph.y) {
-        // ---- step 1: everything that depends on phi only, one lane per phi-node
-        for (int m = lane; m < n; m += 32) {
-            PhiNodeSq s;
-            const bool ok = phi_node_sq(z, zs, mid_phi + half_phi * k_xi[m], s);
-            double* o = nodeS + m * NODE_F;
-            o[0] = ok ? 1.0 : 0.0; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
-            o[5] = s.b1; o[6] = s.b2; o[7] = s.beta; o[8] = s.u_lo; o[9] = s.u_hi;
-        }
-        __syncwarp();
-        for (int m0 = 0; m0 < n; m0 += G) {
-            const int cnt = min(G, n - m0);
+    // steps 2-4 for the V phi-node slots staged in nodeS (slot: weight in phi (0 = skip), C, S, Lq^2, Uq^2, b1, b2, beta,
+    // and the u-interval the inner rule runs on)
+    auto process = [&](const int V) {
+        for (int m0 = 0; m0 < V; m0 += G) {
+            const int cnt = min(G, V - m0);
             // ---- step 2: node set-up, lane = (phi-node g, x-node r)
             for (int idx = lane; idx < cnt * n; idx += 32) {
                 const int g = idx / n, r = idx - g * n;
@@ -175,7 +169,7 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                 const double u = mid_u + half_u * k_xi[r];
                 const double x = u - 1.0;
                 const double iz1 = rsqrt(b1 + beta * u), iz2 = rsqrt(b2 + beta * u);
-                const double wF = (half_phi * k_w[m0 + g] * norm) * (half_u * k_w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
+                const double wF = (o[0] * norm) * (half_u * k_w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
                 double* Pr = Pk + (g * n + r) * SP;
                 double p0 = 1.0, p1 = x;
                 Pr[0] = 1.0;
@@ -247,6 +241,71 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                     if (v >= 0) acc[s] = fma(csp[v >> 16], Ib[v & 0xffff], acc[s]);
                 }
                 __syncwarp();
+            }
+        }
+    };
+    if (ph.x < ph.y) {
+        if (!SPLIT) {
+            // ---- step 1: everything that depends on phi only, one lane per phi-node
+            for (int m = lane; m < n; m += 32) {
+                PhiNodeSq s;
+                const bool ok = phi_node_sq(z, zs, mid_phi + half_phi * k_xi[m], s);
+                double* o = nodeS + m * NODE_F;
+                o[0] = ok ? half_phi * k_w[m] : 0.0; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
+                o[5] = s.b1; o[6] = s.b2; o[7] = s.beta; o[8] = s.u_lo; o[9] = s.u_hi;
+            }
+            __syncwarp();
+            process(n);
+        } else {
+            // ---- kink-split rule RS(n) (R14): items = (phi-piece, phi-node); an item stages one slot per
+            // u-piece (at most 7), IPR items per round so that a round always fits the NS slots
+            double pc[SPLIT_MAX_PHI + 1];
+            const int n_items = split_phi(z, ph.x, ph.y, pc) * n;
+            const int IPR = sh.NS / SPLIT_MAX_U;
+            for (int i0 = 0; i0 < n_items; i0 += IPR) {
+                const int item = i0 + lane;
+                int np = 0;
+                PhiNodeSq s;
+                double cand[6];
+                double wphi = 0.0;
+                if (lane < IPR && item < n_items) {
+                    const int piece = item / n, m = item - piece * n;
+                    const double pa = piece == 0 ? pc[0] : (piece == 1 ? pc[1] : pc[2]);
+                    const double pb = piece == 0 ? pc[1] : (piece == 1 ? pc[2] : pc[3]);
+                    const double hp = 0.5 * (pb - pa);
+                    if (phi_node_sq(z, zs, 0.5 * (pa + pb) + hp * k_xi[m], s)) {
+                        split_u_candidates(z, zs, s, cand);
+                        wphi = hp * k_w[m];
+                        double lower = s.u_lo;
+                        np = 1;
+#pragma unroll
+                        for (int i = 0; i < 6; ++i)
+                            if (cand[i] > lower && cand[i] < s.u_hi) { ++np; lower = cand[i]; }
+                    }
+                }
+                int off = np;                                    // inclusive scan over the lanes
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int t = __shfl_up_sync(0xffffffffu, off, d);
+                    if (lane >= d) off += t;
+                }
+                const int V = __shfl_sync(0xffffffffu, off, 31);
+                off -= np;
+                if (np > 0) {
+                    double lower = s.u_lo;
+                    auto put = [&](double lo, double hi) {
+                        double* o = nodeS + off * NODE_F;
+                        o[0] = wphi; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
+                        o[5] = s.b1; o[6] = s.b2; o[7] = s.beta; o[8] = lo; o[9] = hi;
+                        ++off;
+                    };
+#pragma unroll
+                    for (int i = 0; i < 6; ++i)
+                        if (cand[i] > lower && cand[i] < s.u_hi) { put(lower, cand[i]); lower = cand[i]; }
+                    put(lower, s.u_hi);
+                }
+                __syncwarp();
+                process(V);
             }
         }
     }
@@ -427,7 +486,7 @@ contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, cons
 
 namespace wpcd_detail {
 
-cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, const double* xi, const double* w,
+cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
                                 int64_t nnz_geo, const Workspace& ws, const int64_t* /*row_ptr*/, const int32_t* geo_row_ptr,
                                 int32_t* col_idx, double* values, cudaStream_t st)
 {
@@ -450,7 +509,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
     static const int g_forced = [] { const char* e = getenv("WPCD_MOM_G"); return e ? atoi(e) : 0; }();   // tuning knob
-    sh.n = n_quad; sh.G = std::max(1, std::min(32 / n_quad, g_forced > 0 ? g_forced : 2));
+    sh.n = n_quad; sh.NS = split ? std::max(n_quad, 4 * SPLIT_MAX_U) : n_quad; sh.G = std::max(1, std::min(32 / n_quad, g_forced > 0 ? g_forced : 2));
     sh.K1 = ch->k_max + 1; sh.SP = 8 * ((sh.K1 + 7) / 8) + 4;
     sh.ST = 8 * ((ch->n_ll + 7) / 8) + 4; sh.IS = 8 * ((ch->n_ll + 7) / 8) + 2;
     sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.n_ab = ch->n_ab;
@@ -496,14 +555,15 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if (err != cudaSuccess) return err;
     const int n_geo = g->n_p * g->n_q;
     const int maxs = (ch->n_mu + 31) / 32;
-#define WPCD_MOM(MS)                                                                                                          \
+#define WPCD_MOM2(MS, SPL)                                                                                                        \
     do {                                                                                                                      \
-        err = cudaFuncSetAttribute(moments_kernel<MS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
+        err = cudaFuncSetAttribute(moments_kernel<MS, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
         if (err != cudaSuccess) return err;                                                                                   \
-        moments_kernel<MS><<<blocks, MOM_WARPS * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
+        moments_kernel<MS, SPL><<<blocks, MOM_WARPS * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
                                                                      ws.geo_row, ws.geo_phi, ch->ll_pack_dev,                 \
                                                                      ch->trip_pack_dev, ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);         \
     } while (0)
+#define WPCD_MOM(MS) do { if (split) WPCD_MOM2(MS, true); else WPCD_MOM2(MS, false); } while (0)
     err = cudaFuncSetAttribute(contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem);
     if (err != cudaSuccess) return err;
     for (int64_t e0 = 0; e0 < nnz_geo; e0 += ws.chunk) {
@@ -533,6 +593,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         }
     }
 #undef WPCD_MOM
+#undef WPCD_MOM2
     return cudaSuccess;
 }
 

@@ -80,6 +80,7 @@ struct PhiNodeSq {
     double Lq2, Uq2;      // squares of the Q-limits of (A12)
     double b1, b2, beta;
     double u_lo, u_hi;
+    double ibeta;         // 1/beta
 };
 
 __device__ __forceinline__ bool phi_node_sq(const Cell& z, const CellSq& zs, double phi, PhiNodeSq& s)
@@ -121,7 +122,7 @@ __device__ __forceinline__ bool phi_node_sq(const Cell& z, const CellSq& zs, dou
         else if (D < 0.0) u_lo = fmax(u_lo, R * ibeta / D);
         else if (!(0.0 < R)) return false;
     }
-    s.u_lo = u_lo; s.u_hi = u_hi;
+    s.u_lo = u_lo; s.u_hi = u_hi; s.ibeta = ibeta;
     return u_lo < u_hi;
 }
 
@@ -136,6 +137,56 @@ __device__ __forceinline__ double twoF_A14_sq(const CellSq& zs, const PhiNodeSq&
     Qmin2 = pL2 > Qmin2 ? pL2 : Qmin2;
     const double F2 = Qmax2 - Qmin2;
     return F2 > 0.0 ? F2 : 0.0;
+}
+
+// ---- kink-split rule RS(n) (R14): cuts of the phi-range and of the u-range.
+constexpr int SPLIT_MAX_PHI = 3;   // pieces in phi
+constexpr int SPLIT_MAX_U = 7;     // pieces in u
+
+// cut[0 .. n_piece]: the range (phi_a, phi_b) cut at the rectangle-corner angles atan2(c, a), atan2(d, b) inside it
+// (static indexing only: the array stays in registers).
+__device__ __forceinline__ int split_phi(const Cell& z, double phi_a, double phi_b, double (&cut)[SPLIT_MAX_PHI + 1])
+{
+    const double c1 = atan2(z.c, z.a), c2 = atan2(z.d, z.b);
+    const double lo = fmin(c1, c2), hi = fmax(c1, c2);
+    const bool lo_in = lo > phi_a && lo < phi_b;
+    const double last = lo_in ? lo : phi_a;
+    const bool hi_in = hi > last && hi < phi_b;
+    cut[0] = phi_a;
+    cut[1] = lo_in ? lo : (hi_in ? hi : phi_b);
+    cut[2] = (lo_in && hi_in) ? hi : phi_b;
+    cut[3] = phi_b;
+    return 1 + (lo_in ? 1 : 0) + (hi_in ? 1 : 0);
+}
+
+// The six candidate cuts of the u-range, ascending (+inf where a crossing does not exist): crossings of the members of
+// Qmax = min(Uq, U1/zeta1, U2/zeta2) and of Qmin = max(Lq, L1/zeta1, L2/zeta2) (zeta^2 linear in u: closed forms).
+// The pieces are (u_lo, c_1), (c_1, c_2), ..., (c_k, u_hi) over the candidates strictly inside, taken in order:
+//   lower = u_lo;  for each c: if (c > lower && c < u_hi) { piece(lower, c); lower = c; }  piece(lower, u_hi).
+__device__ __forceinline__ void split_u_candidates(const Cell& z, const CellSq& zs, const PhiNodeSq& s, double (&cand)[6])
+{
+    const double inf = __longlong_as_double(0x7ff0000000000000ll);
+    const double iUq2 = __drcp_rn(s.Uq2);
+    cand[0] = (zs.U1s * iUq2 - s.b1) * s.ibeta;                                                      // Uq = U1/zeta1
+    cand[1] = (zs.U2s * iUq2 - s.b2) * s.ibeta;                                                      // Uq = U2/zeta2
+    cand[2] = z.U1 != z.U2 ? (zs.U2s * s.b1 - zs.U1s * s.b2) * s.ibeta / (zs.U1s - zs.U2s) : inf;     // U1/zeta1 = U2/zeta2
+    if (s.Lq2 > 0.0) {
+        const double iLq2 = __drcp_rn(s.Lq2);
+        cand[3] = (zs.L1s * iLq2 - s.b1) * s.ibeta;                                                  // Lq = L1/zeta1
+        cand[4] = (zs.L2s * iLq2 - s.b2) * s.ibeta;                                                  // Lq = L2/zeta2
+    } else {
+        cand[3] = inf; cand[4] = inf;
+    }
+    cand[5] = z.L1 != z.L2 ? (zs.L2s * s.b1 - zs.L1s * s.b2) * s.ibeta / (zs.L1s - zs.L2s) : inf;     // L1/zeta1 = L2/zeta2
+    // ascending: odd-even transposition network on six registers
+#pragma unroll
+    for (int pass = 0; pass < 6; ++pass) {
+#pragma unroll
+        for (int i = pass & 1; i + 1 < 6; i += 2) {
+            const double lo = fmin(cand[i], cand[i + 1]), hi = fmax(cand[i], cand[i + 1]);
+            cand[i] = lo; cand[i + 1] = hi;
+        }
+    }
 }
 
 __device__ __forceinline__ Cell load_cell(const double* __restrict__ p, const double* __restrict__ q, int n_q, int row, int col)

@@ -40,12 +40,12 @@ def _gpu_channels(wpcd, wl, two_J=None, parity=None):
     return wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=wl.j_pair_max)
 
 
-def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None):
+def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None, split=False):
     grid = wpcd.wpcd_grid_create(p, q)
-    m = wpcd.build_perm(grid, gch, n_quad)
+    m = wpcd.build_perm(grid, gch, n_quad | (wpcd.WPCD_RULE_KINK_SPLIT if split else 0))
     _torch().cuda.synchronize()
     geo = operm.geo_pattern(p, q)
-    rp, ci, v, av = operm.build_csr(p, q, n_quad, tab, geo=geo, geo_rows=geo_rows)
+    rp, ci, v, av = operm.build_csr(p, q, n_quad, tab, geo=geo, geo_rows=geo_rows, split=split)
     assert m.nnz == rp[-1] and m.nnz_geo == geo[0][-1]
     assert np.array_equal(m.geo_row_ptr.cpu().numpy().astype(np.int64), geo[0])
     assert np.array_equal(m.row_ptr.cpu().numpy(), rp)
@@ -477,6 +477,50 @@ def test_handle_state_between_count_and_build(wpcd):
         assert np.array_equal(out[name][0], rp) and np.array_equal(out[name][1], ci)
         tol = VALUE_RTOL * np.maximum(np.abs(v), av) + VALUE_FLOOR * np.abs(v).max()
         assert np.all(np.abs(out[name][2] - v) <= tol)
+
+
+@pytest.mark.parametrize("n_quad", [2, 5, 8, 16, 33])
+def test_split_rule_swave(wpcd, n_quad):
+    """the kink-split rule RS(n) (R14), s-wave kernel, same pattern, values 1e-11 against the
+    oracle at the same rule: jittered lattices with p != q, first-bin cells, a single cell, grids away from zero."""
+    ch, pairs = och.spinless_swave_table(0.5)
+    tab = operm.PairTable(ch, pairs)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    cases = [(wi.tan2_grid(9, 1.0, 0.1, seed=21), wi.tan2_grid(7, 0.6, 0.1, seed=22)),
+             (np.array([0.0, 0.37]), np.array([0.0, 0.37])),
+             (np.array([0.3, 0.5, 2.0]), np.array([0.1, 0.2, 0.9, 4.0]))]
+    if n_quad == 8:
+        wl = wi.WORKLOADS["cfg1"]
+        cases.append((wl.grid(), wl.grid()))
+    for p, q in cases:
+        _compare_full(wpcd, p, q, n_quad, gch, tab, split=True)
+
+
+@pytest.mark.parametrize("two_J,parity,jmax,nb,nq", [(1, 1, 1, 6, 6), (1, -1, 2, 5, 4), (3, 1, 2, 4, 8), (5, -1, 3, 3, 10), (1, 1, 2, 4, 33)])
+def test_split_rule_coupled(wpcd, two_J, parity, jmax, nb, nq):
+    """The kink-split rule through the coupled path (moments on the FP64 tensor cores + contraction): the u-pieces of a
+    phi-node are staged as extra node slots, several rounds per element."""
+    chs = och.enumerate_channels(two_J, parity, jmax)
+    tab = operm.PairTable(chs, och.g_table(chs, two_J, 1))
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=jmax)
+    p = wi.tan2_grid(nb, 1.0, 0.1, seed=31)
+    q = wi.tan2_grid(nb + 1, 0.8, 0.1, seed=32)
+    _compare_full(wpcd, p, q, nq, gch, tab, split=True)
+
+
+def test_split_rule_is_more_accurate(wpcd):
+    """RS(8) on the device against the oracle's RS(64): ten times closer than R(8) (the accuracy claim of DESIGN.md R14)."""
+    ch, pairs = och.spinless_swave_table(1.0)
+    tab = operm.PairTable(ch, pairs)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=1.0)
+    p = wi.tan2_grid(12, 1.0, 0.1, seed=3)
+    ref = operm.build_csr(p, p, 64, tab, split=True)[2]
+    grid = wpcd.wpcd_grid_create(p, p)
+    plain = wpcd.build_perm(grid, gch, 8).values.cpu().numpy()
+    split = wpcd.build_perm(grid, gch, 8 | wpcd.WPCD_RULE_KINK_SPLIT).values.cpu().numpy()
+    e_plain = np.linalg.norm(plain - ref) / np.linalg.norm(ref)
+    e_split = np.linalg.norm(split - ref) / np.linalg.norm(ref)
+    assert 1.5e-3 < e_split < 2.3e-3 and e_plain > 8 * e_split
 
 
 def test_apply_interleaved(wpcd):

@@ -172,6 +172,17 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
                                         const double* values_dev, const double* x_dev, double* y_dev, int n_inter,
                                         void* cuda_stream);
 
+/* y = P0 x for a matrix built by wpcd_perm_build on (grid, channels), using its block structure: row (gamma,i,j)
+ * holds, for every gamma' coupled to gamma, the same geometric columns shifted by gamma' * n_p * n_q, so only the
+ * first block's column indices of each row are read: the matrix streams at 8 bytes per nonzero instead of the 12
+ * of the general CSR product (the SpMV is HBM-bound).  row_ptr_dev, geo_row_ptr_dev as written
+ * by wpcd_perm_count, col_idx_dev / values_dev by wpcd_perm_build, for THESE handles (not checked); x_dev, y_dev
+ * [n_vec][rows], dev.  Each row is summed by one warp in a fixed order (deterministic; agrees with wpcd_perm_apply to
+ * rounding).  Asynchronous; the first apply on arrays not built through this library synchronises the stream once. */
+wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* grid, const wpcd_channels* channels, const int64_t* row_ptr_dev,
+                                    const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                    const double* x_dev, double* y_dev, int n_vec, void* cuda_stream);
+
 /* The dependent products of the simple iteration (paper step 5; Neumann terms):
  * y_k = P0 y_{k-1}, k = 1 .. n_iter, y_0 = x.  y_dev holds all iterates, y_dev[(k-1)*rows + r] = (P0^k x)[r], dev;
  * x_dev [rows], dev, must not overlap y_dev.  A matrix in the size window where it pays (about 1.6e4 <= nnz <=

@@ -31,7 +31,7 @@ EXPORTS = [
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
+    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
     "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
@@ -80,6 +80,7 @@ def load():
     L.wpcd_perm_apply_host.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp, vp, vp]
     L.wpcd_perm_apply_complex.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_interleaved.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
+    L.wpcd_perm_apply_blocked.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_chain.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_block_apply.argtypes = [i32, i32, i32, vp, i32, vp, vp, i32, vp]
     L.wpcd_kernel_apply.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -243,6 +244,15 @@ def wpcd_perm_apply_interleaved(rows, row_ptr, col_idx, values, x, y, stream=Non
     _check(load().wpcd_perm_apply_interleaved(rows, _dev_ptr(row_ptr, torch.int64), _dev_ptr(col_idx, torch.int32),
                                               _dev_ptr(values, torch.float64), _dev_ptr(x), _dev_ptr(y), int(x.shape[1]),
                                               _stream_ptr(stream)))
+
+
+def wpcd_perm_apply_blocked(grid, channels, row_ptr, geo_row_ptr, col_idx, values, x, y, n_vec=1, stream=None):
+    """y = P0 x through the block structure of the matrix built on (grid, channels); x, y: float64 [n_vec, rows] (CUDA)."""
+    import torch
+
+    _check(load().wpcd_perm_apply_blocked(grid.handle, channels.handle, _dev_ptr(row_ptr, torch.int64), _dev_ptr(geo_row_ptr, torch.int32),
+                                          _dev_ptr(col_idx, torch.int32), _dev_ptr(values, torch.float64), _dev_ptr(x, torch.float64),
+                                          _dev_ptr(y, torch.float64), n_vec, _stream_ptr(stream)))
 
 
 def wpcd_perm_apply_chain(rows, row_ptr, col_idx, values, x, y, n_iter, stream=None):

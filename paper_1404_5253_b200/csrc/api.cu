@@ -145,7 +145,7 @@ static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_p
 static void free_channels_device(wpcd_channels* c)
 {
     if (c->ncoupled_dev) cudaDeviceSynchronize();   // the tables go back to the buffer cache: no kernel may still read them
-    pool_free(c->ncoupled_dev); pool_free(c->chan_off_dev); pool_free(c->ll_pack_dev); pool_free(c->trip_pack_dev);
+    pool_free(c->ncoupled_dev); pool_free(c->chan_off_dev); pool_free(c->coupled_gp_dev); pool_free(c->ll_pack_dev); pool_free(c->trip_pack_dev);
     pool_free(c->mu_pack_dev); pool_free(c->ab_pack_dev); pool_free(c->slab_blob_dev);
 }
 
@@ -199,6 +199,8 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     std::vector<int64_t> chan_off(c->n_ch + 1, 0);
     for (int a = 0; a < c->n_ch; ++a) chan_off[a + 1] = chan_off[a] + c->ncoupled[a];
     c->total_coupled = chan_off[c->n_ch];
+    c->coupled_gp.assign(c->n_pairs, 0);      // gamma' of block t of channel gamma, at chan_off[gamma] + t
+    for (int pidx = 0; pidx < c->n_pairs; ++pidx) c->coupled_gp[chan_off[c->pair_gamma[pidx]] + pair_ci[pidx]] = c->pair_gammap[pidx];
     // ---- moment row: one block per (l, l') with its distinct monomials; (l,l') list; (k,l,l') triples
     std::map<std::pair<int, int>, int> ll_index;
     c->ll_pack.clear();
@@ -331,6 +333,7 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     cudaError_t err;
     if ((err = upload(&c->ncoupled_dev, c->ncoupled)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->chan_off_dev, chan_off)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    if ((err = upload(&c->coupled_gp_dev, c->coupled_gp)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->ll_pack_dev, c->ll_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->trip_pack_dev, c->trip_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     if ((err = upload(&c->mu_pack_dev, c->mu_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
@@ -674,6 +677,28 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
     if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: null matrix arrays");
     cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, 1, n_inter, mean_row, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_interleaved");
+    return WPCD_OK;
+}
+
+wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* g, const wpcd_channels* c, const int64_t* row_ptr_dev,
+                                    const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                    const double* x_dev, double* y_dev, int n_vec, void* cuda_stream)
+{
+    if (!g || !c) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null handle");
+    if (n_vec < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: negative size");
+    const int64_t rows = wpcd_rows(g, c);
+    if (rows == 0 || n_vec == 0) return WPCD_OK;
+    if (!row_ptr_dev || !geo_row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int n_geo = g->n_p * g->n_q;
+    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
+    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null matrix arrays");
+    // mean geometric entries per row = nnz / (coupled pairs per geometric row summed over gamma) = nnz / total_coupled / n_geo
+    const double mean_cnt = c->total_coupled > 0 ? mean_row * (double)rows / ((double)c->total_coupled * n_geo) : 0.0;
+    (void)mean_cnt;
+    cudaError_t err = launch_spmv_blocked(rows, n_geo, c->chan_off_dev, c->coupled_gp_dev, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev,
+                                          x_dev, y_dev, n_vec, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_blocked");
     return WPCD_OK;
 }
 

@@ -70,6 +70,8 @@ struct wpcd_channels {
     // device tables
     int32_t* ncoupled_dev = nullptr;          // [n_ch]   number of gamma' coupled to gamma
     int64_t* chan_off_dev = nullptr;          // [n_ch+1] prefix of ncoupled
+    int32_t* coupled_gp_dev = nullptr;        // [n_pairs] gamma' of block t of channel gamma at chan_off[gamma] + t
+    std::vector<int32_t> coupled_gp;
     int32_t* ll_pack_dev = nullptr;
     int32_t* trip_pack_dev = nullptr;
     int32_t* mu_pack_dev = nullptr;
@@ -128,6 +130,9 @@ cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col
                         const double* x, double* y, int n_vec, double mean_row, cudaStream_t st);
 cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                                     const double* x, double* y, int n_vec, int n_inter, double mean_row, cudaStream_t st);
+cudaError_t launch_spmv_blocked(int64_t rows, int n_geo, const int64_t* chan_off, const int32_t* coupled_gp, const int64_t* row_ptr,
+                                const int32_t* geo_row_ptr, const int32_t* col_idx, const double* values, const double* x, double* y,
+                                int n_vec, cudaStream_t st);
 cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                               const double* x, double* y, int n_iter, double mean_row, cudaStream_t st, int* fused);
 cudaError_t run_fp64_peak(cudaStream_t st, double* flops_out);

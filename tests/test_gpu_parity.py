@@ -590,6 +590,53 @@ def test_apply_row_length_sweep(wpcd):
                 check(yh[:, k], k)
 
 
+def test_apply_blocked(wpcd):
+    """The product through the block structure of P0 (only the first block's column indices of a row are read): against
+    the oracle's row-by-row product on coupled matrices (several J^pi, p != q, few and many geometric entries per row, more
+    than 32 coupled channels), the s-wave matrix (one block per row) and a lattice with empty rows."""
+    torch = _torch()
+    cases = []
+    for two_J, parity, jmax, nb in ((1, 1, 1, 6), (3, 1, 2, 9), (5, -1, 3, 4), (1, -1, 2, 14)):
+        gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=jmax)
+        cases.append((gch, wi.tan2_grid(nb, 1.0, 0.1, seed=41), wi.tan2_grid(nb + 2, 0.8, 0.1, seed=42), 4))
+    sw = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    cases.append((sw, wi.tan2_grid(40, 1.0, 0.1, seed=8), wi.tan2_grid(40, 1.0, 0.1, seed=8), 8))
+    cases.append((sw, np.array([0.0, 0.1, 0.2, 5.0, 5.1]), np.array([0.0, 0.05, 3.0]), 8))
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=1)
+    cases.append((gch, np.array([0.0, 0.1, 0.2, 5.0, 5.1]), np.array([0.0, 0.05, 3.0]), 4))
+    for gch, p, q, n_quad in cases:
+        grid = wpcd.wpcd_grid_create(p, q)
+        m = wpcd.build_perm(grid, gch, n_quad)
+        rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+        xs = np.stack([wi.normal_vector(m.rows, k=800 + k) for k in range(3)])
+        x = torch.from_numpy(xs).cuda()
+        y = torch.full_like(x, np.nan)
+        wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y, n_vec=3)
+        yh = y.cpu().numpy()
+        for k in range(3):
+            ref = operm.spmv(rp, ci, v, xs[k])
+            scale = operm.spmv(rp, ci, np.abs(v), np.abs(xs[k]))
+            assert np.all(np.abs(yh[k] - ref) <= 1e-12 * scale + 1e-300), (gch.count, len(p), k)
+
+
+def test_apply_blocked_unstaged_rows():
+    """The same cases through the path for rows too long for the shared-memory staging area (forced by
+    WPCD_SPMV_BLOCKED_UNSTAGED=1, read once per process, hence the child process)."""
+    import os
+    import subprocess
+    import sys
+
+    if os.environ.get("WPCD_SPMV_BLOCKED_UNSTAGED") == "1":
+        pytest.skip("already inside the forced run")
+    env = dict(os.environ, WPCD_SPMV_BLOCKED_UNSTAGED="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-m", "gpu", "-x", "-q",
+                        "-k", "test_apply_blocked and not unstaged", "-p", "no:cacheprovider"],
+                       env=env, cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert "1 passed" in r.stdout
+
+
 def _chain_check(wpcd, torch, rows, rp, ci, v, rpd, cid, vd, n_iter, tag):
     xh = wi.normal_vector(rows, k=900)
     x = torch.from_numpy(xh).cuda()

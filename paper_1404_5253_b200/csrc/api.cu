@@ -693,9 +693,6 @@ wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* g, const wpcd_channels* c, 
     const int n_geo = g->n_p * g->n_q;
     double mean_row = mean_row_hint(rows, row_ptr_dev, st);
     if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null matrix arrays");
-    // mean geometric entries per row = nnz / (coupled pairs per geometric row summed over gamma) = nnz / total_coupled / n_geo
-    const double mean_cnt = c->total_coupled > 0 ? mean_row * (double)rows / ((double)c->total_coupled * n_geo) : 0.0;
-    (void)mean_cnt;
     cudaError_t err = launch_spmv_blocked(rows, n_geo, c->chan_off_dev, c->coupled_gp_dev, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev,
                                           x_dev, y_dev, n_vec, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_blocked");

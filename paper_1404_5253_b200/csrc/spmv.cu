@@ -8,6 +8,9 @@
 // Launched with programmatic dependent launch (back-to-back products overlap launch latency).
 #include <stdlib.h>
 
+#include <algorithm>
+#include <mutex>
+
 #include "wpcd_internal.h"
 
 namespace wpcd_detail { bool use_pdl(); }

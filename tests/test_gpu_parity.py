@@ -619,19 +619,20 @@ def test_apply_blocked(wpcd):
             assert np.all(np.abs(yh[k] - ref) <= 1e-12 * scale + 1e-300), (gch.count, len(p), k)
 
 
-def test_apply_blocked_unstaged_rows():
-    """The same cases through the path for rows too long for the shared-memory staging area (forced by
-    WPCD_SPMV_BLOCKED_UNSTAGED=1, read once per process, hence the child process)."""
+@pytest.mark.parametrize("knobs", [{"WPCD_SPMV_BLOCKED_UNSTAGED": "1"}])
+def test_apply_blocked_other_paths(knobs):
+    """The same cases through the path for rows too long for the shared-memory staging area (the knob is read once per
+    process, hence the child process)."""
     import os
     import subprocess
     import sys
 
-    if os.environ.get("WPCD_SPMV_BLOCKED_UNSTAGED") == "1":
+    if os.environ.get("WPCD_BLOCKED_CHILD") == "1":
         pytest.skip("already inside the forced run")
-    env = dict(os.environ, WPCD_SPMV_BLOCKED_UNSTAGED="1")
+    env = dict(os.environ, WPCD_BLOCKED_CHILD="1", **knobs)
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-m", "gpu", "-x", "-q",
-                        "-k", "test_apply_blocked and not unstaged", "-p", "no:cacheprovider"],
+                        "-k", "test_apply_blocked and not other_paths", "-p", "no:cacheprovider"],
                        env=env, cwd=root, capture_output=True, text=True, timeout=600)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
     assert "1 passed" in r.stdout

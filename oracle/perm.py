@@ -104,8 +104,12 @@ def gauss_legendre(n):
 
 
 def element_values(p, q, ei, ej, eip, ejp, n_quad, table, split=False):
-    """Values (A15) by rule R(n_quad) -- or the kink-split rule RS(n_quad) if split -- of the listed
-    geometric elements, all pairs.  Returns (val, absval), each [n_elem, n_pairs]."""
+    """Values (A15) by rule R(n_quad) -- the kink-split rule RS(n_quad) if split is True / 1, the rule RA(n_quad) with the
+    exact u-integral (s-wave term only) if split == 2 -- of the listed geometric elements, all pairs.
+    Returns (val, absval), each [n_elem, n_pairs]."""
+    if int(split) == 2:
+        one = np.diff(table.term_ptr) == 1
+        assert one.all() and not table.pair_l.any() and not table.pair_lp.any() and not table.term_k.any(), "RA(n): s-wave term only"
     p = np.ascontiguousarray(p, np.float64)
     q = np.ascontiguousarray(q, np.float64)
     ei, ej, eip, ejp = (np.ascontiguousarray(v, np.int32) for v in (ei, ej, eip, ejp))
@@ -113,7 +117,7 @@ def element_values(p, q, ei, ej, eip, ejp, n_quad, table, split=False):
     ne = len(ei)
     val = np.zeros((ne, table.n_pairs))
     absval = np.zeros((ne, table.n_pairs))
-    lib().wpo_elements_rule(len(p) - 1, len(q) - 1, p, q, ne, ei, ej, eip, ejp, n_quad, xi, w, 1 if split else 0,
+    lib().wpo_elements_rule(len(p) - 1, len(q) - 1, p, q, ne, ei, ej, eip, ejp, n_quad, xi, w, int(split),
                        table.n_pairs, table.pair_l, table.pair_lp, table.term_ptr, table.term_k,
                        table.term_l1, table.term_l1p, table.term_g, val, absval)
     return val, absval

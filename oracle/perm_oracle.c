@@ -16,7 +16,8 @@
  *   wpo_geo_count/fill geometric CSR pattern (rows (i,j), columns (i',j') ascending)
  *   wpo_elements       values of listed geometric elements for all coupled channel
  *                      pairs by the rule R(n) (R7) applied to (A15)
- *   wpo_elements_rule  the same with the kink-split rule RS(n) (R14) when split != 0
+ *   wpo_elements_rule  the same with the kink-split rule RS(n) (R14) when split == 1, with the rule RA(n)
+ *                      (kink-split in phi and u, exact u-integral; s-wave term only; R15) when split == 2
  *   wpo_spmv           sequential CSR y = P0 x
  *
  * Pins: tests/test_oracle_*.py (Cartesian (A7) brute force, single-cell constant,
@@ -278,6 +279,46 @@ static void element_values(double a, double b, double c, double d,
         for (int e = 1; e < WPO_MAXPOW; ++e) { cp[e] = cp[e - 1] * C; sp[e] = sp[e - 1] * S; }
         for (int upiece = 0; upiece < n_u_piece; ++upiece) {
         double half_u = 0.5 * (u_cut[upiece + 1] - u_cut[upiece]), mid_u = 0.5 * (u_cut[upiece] + u_cut[upiece + 1]);
+        if (split == 2) {
+            /* Rule RA(n) (R15), s-wave term only (k = l1 = l1' = 0, l = l' = 0): on a piece between two
+             * cuts the active members of (A14)'s min and max do not change, each is a constant or a constant over
+             * zeta^2, so with F = 1/2 (Qmax^2 - Qmin^2) = 1/2 (dA + dB / zeta1^2 + dC / zeta2^2) the u-integral of
+             * F / (zeta1 zeta2) is elementary:
+             *   I0 = int du / (zeta1 zeta2)     = (2/beta) ln[(zeta1h + zeta2h) / (zeta1l + zeta2l)]
+             *   I1 = int du / (zeta1^3 zeta2)   = (2/beta) (1/zeta1l^2 - 1/zeta1h^2) / (zeta2h/zeta1h + zeta2l/zeta1l)
+             *   I2 = int du / (zeta1 zeta2^3)   = (2/beta) (1/zeta2l^2 - 1/zeta2h^2) / (zeta1h/zeta2h + zeta1l/zeta2l)
+             * (l, h = lower, upper end of the piece; the forms for I1, I2 have no cancellation when b1 -> b2).
+             * The active members are read off at the midpoint of the piece. */
+            double ul = u_cut[upiece], uh = u_cut[upiece + 1];
+            double z1m = sqrt(b1 + beta * mid_u), z2m = sqrt(b2 + beta * mid_u);
+            double dA = 0.0, dB = 0.0, dC = 0.0;
+            {   /* Qmax^2 = min(Uq^2, U1^2/zeta1^2, U2^2/zeta2^2) */
+                double m0 = Uq, m1 = U1 / z1m, m2 = U2 / z2m;
+                if (m0 <= m1 && m0 <= m2) dA += Uq * Uq; else if (m1 <= m2) dB += U1 * U1; else dC += U2 * U2;
+            }
+            {   /* Qmin^2 = max(Lq^2, L1^2/zeta1^2, L2^2/zeta2^2) */
+                double m0 = Lq, m1 = L1 / z1m, m2 = L2 / z2m;
+                if (m0 >= m1 && m0 >= m2) dA -= Lq * Lq; else if (m1 >= m2) dB -= L1 * L1; else dC -= L2 * L2;
+            }
+            double z1l = sqrt(b1 + beta * ul), z2l = sqrt(b2 + beta * ul);
+            double z1h = sqrt(b1 + beta * uh), z2h = sqrt(b2 + beta * uh);
+            /* differences of the ends written without cancellation: zeta_h - zeta_l = beta du / (zeta_h + zeta_l),
+             * 1/zeta_l^2 - 1/zeta_h^2 = beta du / (zeta_l^2 zeta_h^2) */
+            double du = uh - ul;
+            double integral = 0.0;
+            if (dA != 0.0)
+                integral += dA * (2.0 / beta) * log1p((beta * du / (z1h + z1l) + beta * du / (z2h + z2l)) / (z1l + z2l));
+            if (dB != 0.0) integral += dB * 2.0 * du / (z1l * z1l * z1h * z1h) / (z2h / z1h + z2l / z1l);
+            if (dC != 0.0) integral += dC * 2.0 * du / (z2l * z2l * z2h * z2h) / (z1h / z2h + z1l / z2l);
+            if (integral > 0.0) {
+                for (int cidx = 0; cidx < n_pairs; ++cidx) {
+                    double g = term_g[term_ptr[cidx]];
+                    val[cidx] += wphi * 0.5 * integral * g * C * S;
+                    absval[cidx] += wphi * 0.5 * integral * fabs(g) * C * S;
+                }
+            }
+            continue;
+        }
         for (int r = 0; r < n; ++r) {
             double u = mid_u + half_u * xi[r];
             double x = u - 1.0;

@@ -358,3 +358,52 @@ def test_split_rule_symmetric_matrix(swave_table):
     rp, ci, v, _ = perm.build_csr(p, p, 8, swave_table, split=True)
     m = _dense(rp, ci, v)
     assert np.abs(m - m.T).max() < 1e-12 * np.abs(m).max()
+
+
+# ---- rule RA(n): kink-split in phi and u, exact u-integral for the s-wave term (R15) ----
+def test_analytic_u_rule_against_quadrature(swave_table):
+    """The closed-form u-integrals of RA(n) against 64-point Gauss-Legendre on the same pieces (RS(64) in u, same phi-nodes):
+    a wrong antiderivative, a wrong active member or a swapped zeta shows at once.  At equal n the two rules differ only by
+    the u-quadrature error of RS(n), so RA(n) -> RS(n) as the u-order grows: compare at n = 64 (1e-5) and check that the
+    phi-convergence is the same (RA(8) within 2x of RS(8)'s error, both against RS(64))."""
+    p = wi.tan2_grid(12, 1.0, 0.1, seed=3)
+    geo = perm.geo_pattern(p, p)
+    rs64 = perm.build_csr(p, p, 64, swave_table, geo=geo, split=1)[2]
+    ra64 = perm.build_csr(p, p, 64, swave_table, geo=geo, split=2)[2]
+    nrm = np.linalg.norm(rs64)
+    assert np.linalg.norm(ra64 - rs64) / nrm < 3e-5
+    errs = {n: np.linalg.norm(perm.build_csr(p, p, n, swave_table, geo=geo, split=2)[2] - ra64) / nrm for n in (4, 8, 16, 32)}
+    assert errs[4] > errs[8] > errs[16] > errs[32]
+    assert errs[8] < 4e-3 and errs[32] < 1.5e-4
+    # p != q lattice, element by element against RS(64)
+    p5, q4 = wi.tan2_grid(5, 1.0, 0.1, seed=3), wi.tan2_grid(4, 0.7, 0.1, seed=4)
+    ptr, col = perm.geo_pattern(p5, q4)
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    va, _ = perm.element_values(p5, q4, rows // 4, rows % 4, col // 4, col % 4, 64, swave_table, split=2)
+    vs, _ = perm.element_values(p5, q4, rows // 4, rows % 4, col // 4, col % 4, 64, swave_table, split=1)
+    assert np.abs(va - vs).max() < 5e-5 * np.abs(vs).max()
+
+
+def test_analytic_u_rule_single_cell_and_cartesian(swave_table):
+    """Single cell (C1 = 1.5056 +- 1e-4) and the Cartesian (A7) brute force on a p != q lattice."""
+    gold = dict(line.split() for line in open(GOLD) if line.strip() and not line.startswith("#"))
+    p1 = np.array([0.0, 1.0])
+    v, av = perm.element_values(p1, p1, [0], [0], [0], [0], 128, swave_table, split=2)
+    assert abs(v[0, 0] - float(gold["C1"])) < 1e-4 and av[0, 0] == pytest.approx(v[0, 0])
+    p = wi.tan2_grid(5, 1.0, 0.1, seed=3)
+    q = wi.tan2_grid(4, 0.7, 0.1, seed=4)
+    ptr, col = perm.geo_pattern(p, q)
+    n_q = len(q) - 1
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    v, _ = perm.element_values(p, q, rows // n_q, rows % n_q, col // n_q, col % n_q, 32, swave_table, split=2)
+    worst = 0.0
+    for e in range(0, len(col), 3):
+        i, j, ip, jp = rows[e] // n_q, rows[e] % n_q, col[e] // n_q, col[e] % n_q
+        ref = brute.element(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1], 0, 0, [(0, 0, 0, 1.0)], m=160)
+        worst = max(worst, abs(v[e, 0] - ref))
+    assert worst < 4e-3 * np.abs(v).max()
+    # symmetric to rounding on a q == p lattice (exchange symmetry of the cuts and of the closed forms, zeta1 <-> zeta2)
+    pp = wi.tan2_grid(10, 1.0, 0.1, seed=11)
+    rp, ci, vv, _ = perm.build_csr(pp, pp, 8, swave_table, split=2)
+    m = _dense(rp, ci, vv)
+    assert np.abs(m - m.T).max() < 1e-12 * np.abs(m).max()

@@ -420,7 +420,10 @@ def run_ours(args):
     # ---- extra: the kink-split rule RS(n) (R14): cost of the build against R(n)
     rule_split = {}
     job = jobs[-1]
-    for name, nq in (("plain", wl.n_quad), ("split", wl.n_quad | wpcd.WPCD_RULE_KINK_SPLIT)):
+    rules = [("plain", wl.n_quad), ("split", wl.n_quad | wpcd.WPCD_RULE_KINK_SPLIT)]
+    if wl.model == "swave":
+        rules += [("analytic_u", wl.n_quad | wpcd.WPCD_RULE_ANALYTIC_U), ("analytic_u_n32", 32 | wpcd.WPCD_RULE_ANALYTIC_U), ("plain_n32", 32)]
+    for name, nq in rules:
         reps = 3 if wl.model == "swave" else 1
         for _ in range(1):
             wpcd.wpcd_perm_build(grid, job.channels, nq, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)

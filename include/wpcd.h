@@ -54,6 +54,7 @@ typedef int wpcd_status;
 
 #define WPCD_MAX_QUAD 64            /* Gauss-Legendre points per dimension (paper: 48, l.334) */
 #define WPCD_RULE_KINK_SPLIT 0x100   /* OR into n_quad: the kink-split rule RS(n) of DESIGN.md R14 */
+#define WPCD_RULE_ANALYTIC_U 0x200   /* OR into n_quad: rule RA(n) of DESIGN.md R15, exact x-integral; s-wave term only */
 #define WPCD_MAX_L 7                /* largest pair orbital momentum l */
 #define WPCD_MAX_K 23               /* largest Legendre order k in (A3) */
 
@@ -139,7 +140,9 @@ size_t wpcd_perm_workspace_bytes(const wpcd_channels* channels, int64_t nnz_geo)
  * Gauss-Legendre in x over the closed-form support of F.  1 <= n_quad <= WPCD_MAX_QUAD.
  * n_quad | WPCD_RULE_KINK_SPLIT selects the kink-split rule RS(n_quad) of DESIGN.md R14 instead (the phi-range cut at
  * the rectangle-corner angles, the x-range at the crossings of the members of (A14)'s min / max; about ten times
- * the accuracy and ten times the cost of R(n_quad)); the pattern (wpcd_perm_count) does not depend on the rule.
+ * the accuracy and ten times the cost of R(n_quad)); n_quad | WPCD_RULE_ANALYTIC_U the rule RA(n_quad) of R15 (the
+ * same cuts, the x-integral of every piece in closed form; only for the s-wave channel set, WPCD_ERR_UNSUPPORTED
+ * otherwise).  The pattern (wpcd_perm_count) does not depend on the rule.
  * Coupled channels: a channel pair may use any number of (k, l1+l1') monomials (more than 32 are
  * handled in several passes); WPCD_ERR_CUDA "invalid argument" if the tables exceed shared memory.
  * Asynchronous on the stream. */

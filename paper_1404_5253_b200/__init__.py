@@ -24,6 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libwpcd.so")
 WPCD_SPINLESS_SWAVE = 0
 WPCD_ND = 1
 WPCD_RULE_KINK_SPLIT = 0x100   # OR into n_quad: kink-split rule RS(n) (R14)
+WPCD_RULE_ANALYTIC_U = 0x200   # OR into n_quad: rule RA(n), exact x-integral, s-wave only (R15)
 WPCD_MAX_QUAD = 64
 
 EXPORTS = [

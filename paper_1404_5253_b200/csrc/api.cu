@@ -541,7 +541,7 @@ wpcd_status wpcd_perm_count(const wpcd_grid* g_in, const wpcd_channels* c, int n
 {
     if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_count: null pointer");
-    n_quad &= ~WPCD_RULE_KINK_SPLIT;       // the pattern does not depend on the rule
+    n_quad &= ~(WPCD_RULE_KINK_SPLIT | WPCD_RULE_ANALYTIC_U);       // the pattern does not depend on the rule
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_count: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_count: channel tables are not on a device (no CUDA device?)");
     wpcd_grid* g = const_cast<wpcd_grid*>(g_in);   // the staging scratch inside the handle is mutable state
@@ -572,8 +572,11 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
                             double* values_dev)
 {
     if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
-    const bool split = (n_quad & WPCD_RULE_KINK_SPLIT) != 0;
-    n_quad &= ~WPCD_RULE_KINK_SPLIT;
+    const bool analytic = (n_quad & WPCD_RULE_ANALYTIC_U) != 0;
+    const bool split = (n_quad & WPCD_RULE_KINK_SPLIT) != 0 || analytic;
+    n_quad &= ~(WPCD_RULE_KINK_SPLIT | WPCD_RULE_ANALYTIC_U);
+    if (analytic && !c->swave_single)
+        return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: WPCD_RULE_ANALYTIC_U is for the s-wave term (k = l = l' = 0) only");
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_build: channel tables are not on a device (no CUDA device?)");
     wpcd_grid* g = const_cast<wpcd_grid*>(g_in);
@@ -611,7 +614,7 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
         std::memcpy(xi, tab.data(), sizeof(double) * n_quad);
         std::memcpy(w, tab.data() + n_quad, sizeof(double) * n_quad);
     }
-    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, split, xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
+    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, analytic ? 2 : (split ? 1 : 0), xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
     else err = launch_fill_coupled(g, c, n_quad, split, xi, w, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(fill)");
     return WPCD_OK;

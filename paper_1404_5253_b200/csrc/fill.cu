@@ -145,11 +145,95 @@ fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__
     }
 }
 
+// ------------------------------------------------------------------ s-wave, rule RA(n): exact u-integral (R15)
+// Same work items and cuts as the kink-split kernel; on a piece the active members of (A14)'s min / max are fixed, so
+// int 2F / (zeta1 zeta2) du = dA I0 + dB I1 + dC I2 in closed form (squared variables, one division per term,
+// end-point square roots carried from piece to piece).
+template <int LPE>
+__global__ void __launch_bounds__(256)
+fill_swave_analytic_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n, double g0,
+                           int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
+                           const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t e = t / LPE;
+    const int sub = (int)(t - e * LPE);
+    const bool valid = e < nnz_geo;
+    double acc = 0.0;
+    double norm = 0.0;
+    int col = 0;
+    if (valid) {
+        col = geo_col[e];
+        const int row = geo_row[e];
+        const double2 ph = geo_phi[e];
+        const Cell z = load_cell(p, q, n_q, row, col);
+        const CellSq zs = square_cell(z);
+        norm = cell_norm(z);
+        if (ph.x < ph.y) {
+            double pc[SPLIT_MAX_PHI + 1];
+            const int n_piece = split_phi(z, ph.x, ph.y, pc);
+#pragma unroll 1
+            for (int item = sub; item < n_piece * n; item += LPE) {
+                const int piece = item / n, m = item - piece * n;
+                const double pa = piece == 0 ? pc[0] : (piece == 1 ? pc[1] : pc[2]);
+                const double pb = piece == 0 ? pc[1] : (piece == 1 ? pc[2] : pc[3]);
+                const double half_phi = 0.5 * (pb - pa), mid_phi = 0.5 * (pa + pb);
+                PhiNodeSq s;
+                if (!phi_node_sq(z, zs, mid_phi + half_phi * c_xi[m], s)) continue;
+                double cand[6];
+                split_u_candidates(z, zs, s, cand);
+                double cut[SPLIT_MAX_U + 1];
+                int np = 1;
+                cut[0] = s.u_lo;
+#pragma unroll
+                for (int i = 0; i < 6; ++i) {
+                    if (cand[i] > cut[np - 1] && cand[i] < s.u_hi) cut[np++] = cand[i];
+                }
+                cut[np] = s.u_hi;
+                double node = 0.0;
+                double z1l = sqrt(s.b1 + s.beta * cut[0]), z2l = sqrt(s.b2 + s.beta * cut[0]);
+#pragma unroll 1
+                for (int k = 0; k < np; ++k) {
+                    const double ul = cut[k], uh = cut[k + 1], du = uh - ul;
+                    const double um = 0.5 * (ul + uh);
+                    const double z1m2 = s.b1 + s.beta * um, z2m2 = s.b2 + s.beta * um;     // zeta^2 at the midpoint
+                    const double z1h = sqrt(s.b1 + s.beta * uh), z2h = sqrt(s.b2 + s.beta * uh);
+                    // active member of Qmax^2 = min(Uq^2, U1^2/zeta1^2, U2^2/zeta2^2) and of Qmin^2 = max(Lq^2, L1^2/.., L2^2/..)
+                    double dA = 0.0, dB = 0.0, dC = 0.0;
+                    if (s.Uq2 * z1m2 <= zs.U1s && s.Uq2 * z2m2 <= zs.U2s) dA = s.Uq2;
+                    else if (zs.U1s * z2m2 <= zs.U2s * z1m2) dB = zs.U1s;
+                    else dC = zs.U2s;
+                    if (s.Lq2 * z1m2 >= zs.L1s && s.Lq2 * z2m2 >= zs.L2s) dA -= s.Lq2;
+                    else if (zs.L1s * z2m2 >= zs.L2s * z1m2) dB -= zs.L1s;
+                    else dC -= zs.L2s;
+                    double integral = 0.0;
+                    const double bdu = s.beta * du;
+                    if (dA != 0.0) {
+                        const double s1 = z1h + z1l, s2 = z2h + z2l;
+                        integral += dA * 2.0 * s.ibeta * log1p(bdu * (s1 + s2) / (s1 * s2 * (z1l + z2l)));
+                    }
+                    if (dB != 0.0) integral += dB * 2.0 * du / (z1l * z1h * (z2h * z1l + z2l * z1h));
+                    if (dC != 0.0) integral += dC * 2.0 * du / (z2l * z2h * (z1h * z2l + z1l * z2h));
+                    if (integral > 0.0) node += integral;
+                    z1l = z1h; z2l = z2h;
+                }
+                acc += half_phi * c_w[m] * s.beta * node;    // cos*sin = beta
+            }
+        }
+    }
+#pragma unroll
+    for (int o = LPE / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (valid && sub == 0) {
+        values[e] = 0.5 * g0 * norm * acc;    // the 1/2 of (A14)
+        col_idx[e] = col;
+    }
+}
+
 }  // namespace
 
 namespace wpcd_detail {
 
-cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
+cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, int rule, const double* xi, const double* w,
                               int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st)
 {
     // the rule's nodes and weights live in constant memory; they are uploaded again only when the
@@ -176,7 +260,14 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     StageTimer timer(WPCD_STAGE_FILL_SWAVE, st);
 #define WPCD_LAUNCH_SW(L, Q) fill_swave_kernel<L, Q><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
                                                                             ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
-    if (split) {
+    if (rule == 2) {
+        lpe = 8; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256);
+        fill_swave_analytic_kernel<8><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col, ws.geo_row,
+                                                              ws.geo_phi, col_idx, values);
+        ++g_launches;
+        return cudaGetLastError();
+    }
+    if (rule == 1) {
         // the rule has up to 3 n work items per element: eight lanes each
         lpe = 8; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256);
         if (n_quad == 8) fill_swave_split_kernel<8, 8><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,

@@ -119,7 +119,7 @@ cudaError_t launch_geo_gather(const wpcd_grid* g, const int32_t* geo_row_ptr_dev
                               double2* geo_phi, cudaStream_t st);
 
 // fill.cu
-cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
+cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, int rule, const double* xi, const double* w,
                               int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st);
 cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
                                 int64_t nnz_geo, const Workspace& ws, const int64_t* row_ptr, const int32_t* geo_row_ptr,

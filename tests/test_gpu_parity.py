@@ -42,7 +42,8 @@ def _gpu_channels(wpcd, wl, two_J=None, parity=None):
 
 def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None, split=False):
     grid = wpcd.wpcd_grid_create(p, q)
-    m = wpcd.build_perm(grid, gch, n_quad | (wpcd.WPCD_RULE_KINK_SPLIT if split else 0))
+    flag = {0: 0, 1: wpcd.WPCD_RULE_KINK_SPLIT, 2: wpcd.WPCD_RULE_ANALYTIC_U}[int(split)]
+    m = wpcd.build_perm(grid, gch, n_quad | flag)
     _torch().cuda.synchronize()
     geo = operm.geo_pattern(p, q)
     rp, ci, v, av = operm.build_csr(p, q, n_quad, tab, geo=geo, geo_rows=geo_rows, split=split)
@@ -506,6 +507,32 @@ def test_split_rule_coupled(wpcd, two_J, parity, jmax, nb, nq):
     p = wi.tan2_grid(nb, 1.0, 0.1, seed=31)
     q = wi.tan2_grid(nb + 1, 0.8, 0.1, seed=32)
     _compare_full(wpcd, p, q, nq, gch, tab, split=True)
+
+
+@pytest.mark.parametrize("n_quad", [1, 4, 8, 9, 32])
+def test_analytic_u_rule_swave(wpcd, n_quad):
+    """rule RA(n) (R15), the u-integral of every kink-split piece in closed form; values 1e-11
+    against the oracle at the same rule; odd orders put a phi-node on pi/4 (b1 = b2) on the symmetric cells."""
+    ch, pairs = och.spinless_swave_table(0.5)
+    tab = operm.PairTable(ch, pairs)
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    cases = [(wi.tan2_grid(9, 1.0, 0.1, seed=21), wi.tan2_grid(7, 0.6, 0.1, seed=22)),
+             (np.array([0.0, 0.37]), np.array([0.0, 0.37])),
+             (np.array([0.3, 0.5, 2.0]), np.array([0.1, 0.2, 0.9, 4.0])),
+             (wi.tan2_grid(12, 1.0, 0.0), wi.tan2_grid(12, 1.0, 0.0))]
+    if n_quad == 8:
+        wl = wi.WORKLOADS["cfg1"]
+        cases.append((wl.grid(), wl.grid()))
+    for p, q in cases:
+        _compare_full(wpcd, p, q, n_quad, gch, tab, split=2)
+
+
+def test_analytic_u_rule_needs_swave(wpcd):
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=1)
+    p = wi.tan2_grid(4, 1.0, 0.1, seed=1)
+    grid = wpcd.wpcd_grid_create(p, p)
+    with pytest.raises(wpcd.WpcdError, match="s-wave"):
+        wpcd.build_perm(grid, gch, 8 | wpcd.WPCD_RULE_ANALYTIC_U)
 
 
 def test_split_rule_is_more_accurate(wpcd):

@@ -26,13 +26,15 @@ import wpcd_inputs as wi  # noqa: E402
 # DRAM bytes per launch of the dominant kernel from one `ncu --set full` capture (dram__bytes_read.sum +
 # dram__bytes_write.sum), profiles/r01h_ncu_full.md; null where no capture of that workload exists.
 NCU_TRAFFIC = {
-    ("cfg2", "spmv"): 3.59e6,            # spmv_kernel<32,1>, 3.4 MB matrix (L2-resident after the first product)
+    ("cfg2", "spmv"): 3.84e6,            # spmv_kernel<32,4>, one pass of 4 right-hand sides over the 3.4 MB matrix (cold L2 under ncu)
+    ("cfg2", "selection"): 6.38e6,       # geo_select_kernel: staged verdicts written, node tables read
     ("cfg2", "fill_swave"): 6.88e6,
     ("cfg4", "spmv"): 6.19e9,            # J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
 }
 
 METRIC = "P-matrix nonzeros/sec (FP64 build + the workload's P*vector SpMVs per step)"
 UNIT = "nnz/s"
+SELECT_FLOPS_PER_GEO_NNZ = 562.0   # FP64 flops of the selection pass per structural geometric nonzero (ncu op counts, cfg2)
 FLOPS_PER_NODE = 70.0          # algorithmic FP64 flops per (phi,x) quadrature node, s-wave
 L2_FLUSH_BYTES = 256 << 20     # > 126 MB L2
 
@@ -259,8 +261,24 @@ def run_ours(args):
     n_spmv = wl.n_spmv
 
     def spmv_sweep(job):
+        if job.x_all is not None:
+            # all right-hand sides of the workload are resident (s-wave workloads; P is reused for many energies, PAPER.md:270):
+            # one call, the library shares each pass over the matrix among 4 of them
+            wpcd.wpcd_perm_apply(job.rows, job.row_ptr, job.col_idx, job.values, job.x_all, job.y_all, n_vec=n_spmv)
+            return
         for k in range(n_spmv):
             wpcd.wpcd_perm_apply(job.rows, job.row_ptr, job.col_idx, job.values, job.x[k % job.n_x], job.y)
+
+    def sweep_passes(job):
+        """[right-hand sides per launch] of one sweep (mirrors the library: passes of 4, then 2, then 1)."""
+        if job.x_all is None:
+            return [1] * n_spmv
+        out, v = [], 0
+        while v < n_spmv:
+            step_v = 4 if n_spmv - v >= 4 else 2 if n_spmv - v >= 2 else 1
+            out.append(step_v)
+            v += step_v
+        return out
 
     def step(job_list):
         for job in job_list:
@@ -322,7 +340,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
-    graph_launches = sum(n_spmv for job in jobs if job.graph is not None) * args.steps
+    graph_launches = sum(len(sweep_passes(job)) for job in jobs if job.graph is not None) * args.steps
     launches = wpcd.wpcd_launch_count() - launches0 + graph_launches
     stages = wpcd.wpcd_trace_read()
     wpcd.wpcd_trace_enable(False)
@@ -495,17 +513,31 @@ def run_ours(args):
                                  "frac": ach / peaks["hbm_gbs"], "traffic": None,
                                  "ms_per_step": {"moments": stage_ms["moments"], "contract": stage_ms["contract"]},
                                  "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})"}
+    if stage_ms["geo_count"] > 0:
+        # selection (a1): FP64 compare / clip arithmetic, latency- and divergence-bound; per-unit figure of DESIGN.md section 7
+        flops = SELECT_FLOPS_PER_GEO_NNZ * nnz_geo1
+        ach = flops / (stage_ms["geo_count"] * 1e-3) / 1e12
+        roofs["selection"] = {"bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
+                              "frac": ach / (fp64_peak / 1e12), "traffic": None,
+                              "ms_per_launch": stage_ms["geo_count"] / len(jobs),
+                              "peak_source": "in-run DFMA microbenchmark (wpcd_fp64_peak)",
+                              "note": "divergent polygon tests and dependent interval searches: latency-bound, FP64 pipe 24 % active (ncu)"}
     if n_spmv:
-        per_launch_ms = spmv_ms / (steps * n_spmv * len(jobs))
-        sbytes = (12.0 * nnz1 + 16.0 * rows1 + 8.0 * rows1) / len(jobs)
-        ach = sbytes / (per_launch_ms * 1e-3) / 1e9
+        # algorithmic bytes of a launch with v right-hand sides: the matrix once (12 B per nonzero + row_ptr) + v vectors in and out
+        n_launch = sum(len(sweep_passes(j)) for j in jobs)
+        sbytes = sum(sum(12.0 * j.nnz + 8.0 * j.rows + v * 16.0 * j.rows for v in sweep_passes(j)) for j in jobs)
+        per_launch_ms = spmv_ms / (steps * n_launch)
+        ach = sbytes / (spmv_ms / steps * 1e-3) / 1e9
         roofs["spmv"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
-                         "traffic": None, "ms_per_launch": per_launch_ms, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})",
+                         "traffic": None, "ms_per_launch": per_launch_ms, "launches_per_step": n_launch,
+                         "rhs_per_launch": max(max(sweep_passes(j)) for j in jobs),
+                         "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})",
                          "note": "matrix is L2-resident (3 MB)" if wl.model == "swave" else "streams from HBM"}
     share = dict(stage_ms)
     share["spmv_sweep"] = spmv_ms / steps
     dominant = max(share, key=share.get)
-    key = {"fill_swave": "fill_swave", "moments": "fill_coupled", "contract": "fill_coupled", "spmv_sweep": "spmv"}.get(dominant)
+    key = {"fill_swave": "fill_swave", "moments": "fill_coupled", "contract": "fill_coupled", "spmv_sweep": "spmv",
+           "geo_count": "selection"}.get(dominant)
     for name, rf in roofs.items():
         rf["traffic"] = NCU_TRAFFIC.get((wl.name, name))
     roofline = dict(roofs[key]) if key in roofs else {
@@ -530,7 +562,8 @@ def run_ours(args):
         "config": {"workload": wl.name, "n_bins": wl.n_bins, "n_quad": wl.n_quad, "model": wl.model, "jitter": wl.jitter,
                    "jpis": jobs_of(wl) if wl.model == "nd" else None, "n_spmv_per_matrix": n_spmv,
                    "nnz": nnz1, "nnz_geo": nnz_geo1, "rows": rows1, "l2": "flushed between timed steps (256 MiB fill)",
-                   "spmv_launch": "CUDA graph" if jobs[0].graph is not None else "direct"},
+                   "spmv_launch": ("CUDA graph" if jobs[0].graph is not None else "direct")
+                   + (", one call for all right-hand sides (passes of 4)" if jobs[0].x_all is not None and n_spmv else "")},
         "clocks": sampler.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps, "includes": "grid/channel handle creation (host g-table), count, build, the products with pinned-host x and y"

@@ -148,7 +148,7 @@ constexpr int CTRL_OVERFLOW = 1;   // set when the staging capacity was too smal
 constexpr int CTRL_TICKET = 2;     // CTAs finished (the last one runs the scan)
 constexpr int CTRL_RESULT = 4;     // [4] cursor, [5] overflow, [6] nnz_geo of the finished pass (read back by the host)
 
-__global__ void __launch_bounds__(TPB)
+__global__ void __launch_bounds__(TPB, 4)
 geo_select_kernel(const double* __restrict__ p_g, const double* __restrict__ q_g, int n_p, int n_q, int cap,
                   int32_t* __restrict__ geo_counts, int32_t* __restrict__ stage_off, int32_t* __restrict__ stage_len,
                   int32_t* __restrict__ stage_col, double4* __restrict__ stage_ext, int32_t* __restrict__ ctrl)

@@ -597,6 +597,13 @@ def test_apply_row_length_sweep(wpcd):
         def check(got, k):
             assert np.all(np.abs(got - refs[k]) <= 1e-12 * scales[k] + 1e-300), (rows, short, long_, k)
 
+        xs11 = np.stack([xs[k % 4] * (1.0 + 0.25 * (k // 4)) for k in range(11)])          # 11 right-hand sides: passes of 4, 4, 2, 1
+        x11 = torch.from_numpy(xs11).cuda()
+        y11 = torch.full_like(x11, np.nan)
+        wpcd.wpcd_perm_apply(rows, rpd, cid, vd, x11, y11, 11)
+        for k in range(11):
+            got = y11[k].cpu().numpy() / (1.0 + 0.25 * (k // 4))
+            assert np.all(np.abs(got - refs[k % 4]) <= 2e-12 * scales[k % 4] + 1e-300), (rows, short, long_, k)
         for n_vec in (1, 2, 3, 4):
             x = torch.from_numpy(xs[:n_vec].copy()).cuda()
             y = torch.full_like(x, np.nan)

@@ -395,6 +395,7 @@ void wpcd_grid_destroy(wpcd_grid* g)
     if (!g) return;
     if (g->select_ready) cudaDeviceSynchronize();   // scratch goes back to the cache: no kernel may still use it
     pool_free(g->block_dev); pool_free(g->stage_col); pool_free(g->stage_ext); pool_free(g->ctrl_pinned);
+    if (g->count_event) cudaEventDestroy(g->count_event);
     delete g;
 }
 
@@ -520,10 +521,17 @@ static wpcd_status run_selection(wpcd_grid* g, const wpcd_channels* c, int32_t* 
         cudaError_t err = ensure_stage(g, want);
         if (err != cudaSuccess) return cuda_fail(err, who);
         g->stage_valid = false;
+        // the host waits for the selection pass only (an event behind the read-back of its result); the expansion to the
+        // full row pointer is queued behind it and runs while the call returns
+        if (!g->count_event) {
+            err = cudaEventCreateWithFlags(&g->count_event, cudaEventDisableTiming);
+            if (err != cudaSuccess) return cuda_fail(err, who);
+        }
         err = launch_geo_select(g, geo_row_ptr_dev, st);
-        if (err == cudaSuccess && c) err = launch_rowptr(g, c, geo_row_ptr_dev, row_ptr_dev, st);
         if (err == cudaSuccess) err = cudaMemcpyAsync(g->ctrl_pinned, g->ctrl + 4, sizeof(int32_t) * 4, cudaMemcpyDeviceToHost, st);
-        if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+        if (err == cudaSuccess) err = cudaEventRecord(g->count_event, st);
+        if (err == cudaSuccess && c) err = launch_rowptr(g, c, geo_row_ptr_dev, row_ptr_dev, st);
+        if (err == cudaSuccess) err = cudaEventSynchronize(g->count_event);
         if (err != cudaSuccess) return cuda_fail(err, who);
         if (g->ctrl_pinned[1] == 0) {
             g->stage_valid = true;

@@ -22,6 +22,7 @@ struct wpcd_grid {
     int32_t* stage_len = nullptr;       // [n_p*n_q]    number of candidates of a geometric row
     int32_t* ctrl = nullptr;            // [4] device: slot cursor, overflow flag, nnz_geo
     int32_t* ctrl_pinned = nullptr;     // [4] pinned host copy
+    cudaEvent_t count_event = nullptr;  // behind the read-back of the selection result
     int64_t stage_cap = 0;
     bool stage_valid = false;
     bool select_ready = false;          // kernel attributes set

@@ -118,7 +118,8 @@ int64_t wpcd_geo_rows(const wpcd_grid* grid);
  * scratch memory owned by the GRID handle, for the wpcd_perm_build that follows; the handle grows that
  * scratch on demand (a first call on a large lattice may run the pass twice).
  * Waits once, for the selection pass and the read-back of the two counts; the expansion to row_ptr_dev is queued on
- * the stream behind it and may still be running when the call returns (stream order covers every later use). */
+ * the stream behind it and may still be running when the call returns (stream order covers every later use; a
+ * wpcd_perm_build on another stream is ordered behind it by the library). */
 wpcd_status wpcd_perm_count(const wpcd_grid* grid, const wpcd_channels* channels, int n_quad, void* cuda_stream,
                             int64_t* row_ptr_dev, int32_t* geo_row_ptr_dev, int64_t* nnz_out, int64_t* nnz_geo_out);
 

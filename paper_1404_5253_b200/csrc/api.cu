@@ -396,6 +396,7 @@ void wpcd_grid_destroy(wpcd_grid* g)
     if (g->select_ready) cudaDeviceSynchronize();   // scratch goes back to the cache: no kernel may still use it
     pool_free(g->block_dev); pool_free(g->stage_col); pool_free(g->stage_ext); pool_free(g->ctrl_pinned);
     if (g->count_event) cudaEventDestroy(g->count_event);
+    if (g->rowptr_event) cudaEventDestroy(g->rowptr_event);
     delete g;
 }
 
@@ -525,12 +526,15 @@ static wpcd_status run_selection(wpcd_grid* g, const wpcd_channels* c, int32_t* 
         // full row pointer is queued behind it and runs while the call returns
         if (!g->count_event) {
             err = cudaEventCreateWithFlags(&g->count_event, cudaEventDisableTiming);
+            if (err == cudaSuccess) err = cudaEventCreateWithFlags(&g->rowptr_event, cudaEventDisableTiming);
             if (err != cudaSuccess) return cuda_fail(err, who);
         }
         err = launch_geo_select(g, geo_row_ptr_dev, st);
         if (err == cudaSuccess) err = cudaMemcpyAsync(g->ctrl_pinned, g->ctrl + 4, sizeof(int32_t) * 4, cudaMemcpyDeviceToHost, st);
         if (err == cudaSuccess) err = cudaEventRecord(g->count_event, st);
         if (err == cudaSuccess && c) err = launch_rowptr(g, c, geo_row_ptr_dev, row_ptr_dev, st);
+        if (err == cudaSuccess && c) err = cudaEventRecord(g->rowptr_event, st);     // for a build on another stream
+        g->count_stream = st;
         if (err == cudaSuccess) err = cudaEventSynchronize(g->count_event);
         if (err != cudaSuccess) return cuda_fail(err, who);
         if (g->ctrl_pinned[1] == 0) {
@@ -602,6 +606,10 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
     }
     const int64_t nnz_geo = g->stage_nnz_geo;
     if (nnz_geo == 0 || c->total_coupled == 0) return WPCD_OK;
+    if (g->rowptr_event && st != g->count_stream) {      // the count's row-pointer expansion may still run on its own stream
+        cudaError_t werr = cudaStreamWaitEvent(st, g->rowptr_event, 0);
+        if (werr != cudaSuccess) return cuda_fail(werr, "wpcd_perm_build");
+    }
     if (!workspace_dev || !col_idx_dev || !values_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null output or workspace");
     if ((reinterpret_cast<uintptr_t>(workspace_dev) & 255) != 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: workspace must be 256-byte aligned");
     Workspace ws = carve_workspace(c, nnz_geo, workspace_dev);

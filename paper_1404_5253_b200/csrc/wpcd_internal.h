@@ -23,6 +23,8 @@ struct wpcd_grid {
     int32_t* ctrl = nullptr;            // [4] device: slot cursor, overflow flag, nnz_geo
     int32_t* ctrl_pinned = nullptr;     // [4] pinned host copy
     cudaEvent_t count_event = nullptr;  // behind the read-back of the selection result
+    cudaEvent_t rowptr_event = nullptr; // behind the row-pointer expansion of the last count
+    cudaStream_t count_stream = nullptr;
     int64_t stage_cap = 0;
     bool stage_valid = false;
     bool select_ready = false;          // kernel attributes set

@@ -550,6 +550,32 @@ def test_split_rule_is_more_accurate(wpcd):
     assert 1.5e-3 < e_split < 2.3e-3 and e_plain > 8 * e_split
 
 
+def test_count_and_build_on_different_streams(wpcd):
+    """wpcd_perm_count returns once the selection is read back, its row-pointer expansion still queued on the count's stream;
+    a build issued on ANOTHER stream is ordered behind it by the library (coupled channels: the contraction reads row_ptr)."""
+    torch = _torch()
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=2)
+    p = wi.tan2_grid(24, 1.0, 0.1, seed=77)
+    grid = wpcd.wpcd_grid_create(p, p)
+    ref = wpcd.build_perm(grid, gch, 6)
+    torch.cuda.synchronize()
+    s_count, s_build = torch.cuda.Stream(), torch.cuda.Stream()
+    rows = ref.rows
+    for _ in range(5):
+        row_ptr = torch.zeros(rows + 1, dtype=torch.int64, device="cuda")
+        geo_row_ptr = torch.zeros(24 * 24 + 1, dtype=torch.int32, device="cuda")
+        col_idx = torch.zeros(ref.nnz, dtype=torch.int32, device="cuda")
+        values = torch.zeros(ref.nnz, dtype=torch.float64, device="cuda")
+        workspace = torch.empty(max(wpcd.wpcd_perm_workspace_bytes(gch, ref.nnz_geo), 256), dtype=torch.uint8, device="cuda")
+        torch.cuda.synchronize()
+        nnz, nnz_geo = wpcd.wpcd_perm_count(grid, gch, 6, row_ptr, geo_row_ptr, s_count)
+        assert (nnz, nnz_geo) == (ref.nnz, ref.nnz_geo)
+        wpcd.wpcd_perm_build(grid, gch, 6, row_ptr, geo_row_ptr, workspace, col_idx, values, s_build)
+        s_build.synchronize()
+        s_count.synchronize()
+        assert torch.equal(row_ptr, ref.row_ptr) and torch.equal(col_idx, ref.col_idx) and torch.equal(values, ref.values)
+
+
 def test_apply_interleaved(wpcd):
     """Four (and two) real vectors stored interleaved [rows][n_inter]: one gather per entry; short-row and long-row matrices."""
     torch = _torch()

@@ -844,14 +844,63 @@ wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const
     if (rows == 0 || n_vec == 0) return WPCD_OK;
     if (!x_host || !y_host || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_host: null pointer");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    size_t bytes = sizeof(double) * (size_t)rows * (size_t)n_vec;
-    cudaError_t err = cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(H2D)");
-    wpcd_status s = wpcd_perm_apply(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, cuda_stream);
-    if (s != WPCD_OK) return s;
-    err = cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, st);
+    constexpr int CHUNK = 8;       // right-hand sides per pipeline stage (two passes of 4)
+    if (n_vec <= CHUNK) {
+        size_t bytes = sizeof(double) * (size_t)rows * (size_t)n_vec;
+        cudaError_t err = cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(H2D)");
+        wpcd_status s = wpcd_perm_apply(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, cuda_stream);
+        if (s != WPCD_OK) return s;
+        err = cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, st);
+        if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(D2H)");
+        return WPCD_OK;
+    }
+    // Many right-hand sides: three-stage pipeline over chunks of CHUNK vectors -- upload of chunk k+1 (copy stream "up"),
+    // products of chunk k (the caller's stream) and download of chunk k-1 (copy stream "down") run together, so the call
+    // costs about the larger of the two copy directions instead of upload + products + download.
+    struct HostPipe { cudaStream_t up = nullptr, down = nullptr; std::vector<cudaEvent_t> ev; };
+    static std::mutex pipe_mutex;
+    static std::map<int, HostPipe> pipes;
+    std::lock_guard<std::mutex> lock(pipe_mutex);      // the call is synchronous; one pipelined host apply at a time
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host");
+    HostPipe& hp = pipes[dev];
+    if (!hp.up) {
+        err = cudaStreamCreateWithFlags(&hp.up, cudaStreamNonBlocking);
+        if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&hp.down, cudaStreamNonBlocking);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(streams)");
+    }
+    const int n_chunk = (n_vec + CHUNK - 1) / CHUNK;
+    while ((int)hp.ev.size() < 2 * n_chunk + 1) {
+        cudaEvent_t e;
+        err = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(events)");
+        hp.ev.push_back(e);
+    }
+    // the copy streams start behind whatever the caller's stream holds (the matrix, earlier users of the scratch vectors)
+    err = cudaEventRecord(hp.ev[2 * n_chunk], st);
+    if (err == cudaSuccess) err = cudaStreamWaitEvent(hp.up, hp.ev[2 * n_chunk], 0);
+    if (err == cudaSuccess) err = cudaStreamWaitEvent(hp.down, hp.ev[2 * n_chunk], 0);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host");
+    for (int k = 0; k < n_chunk; ++k) {
+        const int v0 = k * CHUNK, nv = std::min(CHUNK, n_vec - v0);
+        const size_t off = (size_t)v0 * (size_t)rows, bytes = sizeof(double) * (size_t)rows * (size_t)nv;
+        err = cudaMemcpyAsync(x_dev + off, x_host + off, bytes, cudaMemcpyHostToDevice, hp.up);
+        if (err == cudaSuccess) err = cudaEventRecord(hp.ev[2 * k], hp.up);
+        if (err == cudaSuccess) err = cudaStreamWaitEvent(st, hp.ev[2 * k], 0);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(H2D)");
+        wpcd_status s = wpcd_perm_apply(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev + off, y_dev + off, nv, cuda_stream);
+        if (s != WPCD_OK) return s;
+        err = cudaEventRecord(hp.ev[2 * k + 1], st);
+        if (err == cudaSuccess) err = cudaStreamWaitEvent(hp.down, hp.ev[2 * k + 1], 0);
+        if (err == cudaSuccess) err = cudaMemcpyAsync(y_host + off, y_dev + off, bytes, cudaMemcpyDeviceToHost, hp.down);
+        if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(D2H)");
+    }
+    err = cudaStreamSynchronize(hp.down);
     if (err == cudaSuccess) err = cudaStreamSynchronize(st);
-    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(D2H)");
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(sync)");
     return WPCD_OK;
 }
 

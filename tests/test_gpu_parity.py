@@ -147,16 +147,19 @@ def test_apply_multi_vector_and_host(wpcd):
     wpcd.wpcd_perm_apply_host(rows, m.row_ptr, m.col_idx, m.values, xh, yh, xd, yd)
     ref = operm.spmv(rp, ci, v, xh.numpy())
     assert np.all(np.abs(yh.numpy() - ref) <= 1e-12 * operm.spmv(rp, ci, np.abs(v), np.abs(xh.numpy())))
-    # several vectors in one host call (bench.py's end-to-end leg)
-    n_vec = 7
-    xh7 = torch.from_numpy(np.stack([wi.normal_vector(rows, k=120 + k) for k in range(n_vec)])).pin_memory()
-    yh7 = torch.empty(n_vec, rows, dtype=torch.float64).pin_memory()
-    xd7 = torch.empty(n_vec, rows, dtype=torch.float64, device="cuda")
-    yd7 = torch.empty_like(xd7)
-    wpcd.wpcd_perm_apply_host(rows, m.row_ptr, m.col_idx, m.values, xh7, yh7, xd7, yd7, n_vec=n_vec)
-    for k in range(n_vec):
-        ref = operm.spmv(rp, ci, v, xh7[k].numpy())
-        assert np.all(np.abs(yh7[k].numpy() - ref) <= 1e-12 * operm.spmv(rp, ci, np.abs(v), np.abs(xh7[k].numpy())))
+    # several vectors in one host call (bench.py's end-to-end leg): 7 go in one piece, 21 through the pipeline over the copy
+    # streams (chunks of 8, 8, 5), twice in a row with the same scratch
+    for n_vec, reps in ((7, 1), (21, 2)):
+        xh7 = torch.from_numpy(np.stack([wi.normal_vector(rows, k=120 + k) for k in range(n_vec)])).pin_memory()
+        yh7 = torch.empty(n_vec, rows, dtype=torch.float64).pin_memory()
+        xd7 = torch.empty(n_vec, rows, dtype=torch.float64, device="cuda")
+        yd7 = torch.empty_like(xd7)
+        for _ in range(reps):
+            yh7.fill_(float("nan"))
+            wpcd.wpcd_perm_apply_host(rows, m.row_ptr, m.col_idx, m.values, xh7, yh7, xd7, yd7, n_vec=n_vec)
+            for k in range(n_vec):
+                ref = operm.spmv(rp, ci, v, xh7[k].numpy())
+                assert np.all(np.abs(yh7[k].numpy() - ref) <= 1e-12 * operm.spmv(rp, ci, np.abs(v), np.abs(xh7[k].numpy())))
 
 
 def test_errors_on_device_path(wpcd):

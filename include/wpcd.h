@@ -237,7 +237,8 @@ wpcd_status wpcd_pade_sum(const double* terms_host, int n_terms, double* sum_out
 /* Same product with HOST vectors: copies x_host -> x_dev (scratch, dev, n_vec*rows doubles),
  * applies, copies y_dev (scratch) -> y_host, then synchronises.  With more than 8 vectors the call pipelines chunks of 8
  * over two internal copy streams (upload of the next chunk, products of this one on the caller's stream and download of the
- * previous one overlap); one such call at a time per process.  Pinned host memory makes the copies asynchronous. */
+ * previous one overlap; the uploads start at once, without waiting for work queued earlier on the stream, so x_dev / y_dev
+ * must not be in use by such work); one such call at a time per process.  Pinned host memory makes the copies asynchronous. */
 wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
                                  const double* values_dev, const double* x_host, double* y_host, int n_vec,
                                  double* x_dev, double* y_dev, void* cuda_stream);

@@ -145,8 +145,8 @@ static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_p
 static void free_channels_device(wpcd_channels* c)
 {
     if (c->ncoupled_dev) cudaDeviceSynchronize();   // the tables go back to the buffer cache: no kernel may still read them
-    pool_free(c->ncoupled_dev); pool_free(c->chan_off_dev); pool_free(c->coupled_gp_dev); pool_free(c->ll_pack_dev); pool_free(c->trip_pack_dev);
-    pool_free(c->mu_pack_dev); pool_free(c->ab_pack_dev); pool_free(c->slab_blob_dev);
+    pool_free(c->tables_dev);
+    c->tables_dev = nullptr;
 }
 
 template <class T>
@@ -330,15 +330,31 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     // inspectable, every compute call then fails with WPCD_ERR_CUDA)
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return WPCD_OK; }
-    cudaError_t err;
-    if ((err = upload(&c->ncoupled_dev, c->ncoupled)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->chan_off_dev, chan_off)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->coupled_gp_dev, c->coupled_gp)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->ll_pack_dev, c->ll_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->trip_pack_dev, c->trip_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->mu_pack_dev, c->mu_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->ab_pack_dev, c->ab_pack)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
-    if ((err = upload(&c->slab_blob_dev, c->slab_blob)) != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    // all device tables in ONE allocation and ONE copy (eight separate synchronous copies cost ~55 us per handle)
+    auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t sz[8] = {sizeof(int32_t) * c->ncoupled.size(), sizeof(int64_t) * chan_off.size(), sizeof(int32_t) * c->coupled_gp.size(),
+                          sizeof(int32_t) * c->ll_pack.size(),  sizeof(int32_t) * c->trip_pack.size(), sizeof(int32_t) * c->mu_pack.size(),
+                          sizeof(int32_t) * c->ab_pack.size(),  c->slab_blob.size()};
+    const void* src[8] = {c->ncoupled.data(), chan_off.data(), c->coupled_gp.data(), c->ll_pack.data(), c->trip_pack.data(),
+                          c->mu_pack.data(), c->ab_pack.data(), c->slab_blob.data()};
+    size_t off[9];
+    off[0] = 0;
+    for (int k = 0; k < 8; ++k) off[k + 1] = off[k] + pad(std::max<size_t>(sz[k], 1));
+    std::vector<unsigned char> blob(off[8], 0);
+    for (int k = 0; k < 8; ++k)
+        if (sz[k]) std::memcpy(blob.data() + off[k], src[k], sz[k]);
+    cudaError_t err = cudaSuccess;
+    c->tables_dev = static_cast<unsigned char*>(pool_alloc(off[8], false, &err));
+    if (err == cudaSuccess) err = cudaMemcpy(c->tables_dev, blob.data(), off[8], cudaMemcpyHostToDevice);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
+    c->ncoupled_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[0]);
+    c->chan_off_dev = reinterpret_cast<int64_t*>(c->tables_dev + off[1]);
+    c->coupled_gp_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[2]);
+    c->ll_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[3]);
+    c->trip_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[4]);
+    c->mu_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[5]);
+    c->ab_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[6]);
+    c->slab_blob_dev = c->tables_dev + off[7];
     return WPCD_OK;
 }
 
@@ -873,17 +889,14 @@ wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const
         if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(streams)");
     }
     const int n_chunk = (n_vec + CHUNK - 1) / CHUNK;
-    while ((int)hp.ev.size() < 2 * n_chunk + 1) {
+    while ((int)hp.ev.size() < 2 * n_chunk) {
         cudaEvent_t e;
         err = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
         if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host(events)");
         hp.ev.push_back(e);
     }
-    // the copy streams start behind whatever the caller's stream holds (the matrix, earlier users of the scratch vectors)
-    err = cudaEventRecord(hp.ev[2 * n_chunk], st);
-    if (err == cudaSuccess) err = cudaStreamWaitEvent(hp.up, hp.ev[2 * n_chunk], 0);
-    if (err == cudaSuccess) err = cudaStreamWaitEvent(hp.down, hp.ev[2 * n_chunk], 0);
-    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_host");
+    // The uploads start at once -- they do not wait for what the caller's stream still holds (typically the build of the
+    // matrix), only the products do; the scratch vectors must therefore not be in use by earlier asynchronous work.
     for (int k = 0; k < n_chunk; ++k) {
         const int v0 = k * CHUNK, nv = std::min(CHUNK, n_vec - v0);
         const size_t off = (size_t)v0 * (size_t)rows, bytes = sizeof(double) * (size_t)rows * (size_t)nv;

@@ -70,7 +70,8 @@ struct wpcd_channels {
     // contraction slabs
     std::vector<wpcd_slab> slabs;
     std::vector<unsigned char> slab_blob;
-    // device tables
+    // device tables (one allocation, tables_dev; the typed pointers below point into it)
+    unsigned char* tables_dev = nullptr;
     int32_t* ncoupled_dev = nullptr;          // [n_ch]   number of gamma' coupled to gamma
     int64_t* chan_off_dev = nullptr;          // [n_ch+1] prefix of ncoupled
     int32_t* coupled_gp_dev = nullptr;        // [n_pairs] gamma' of block t of channel gamma at chan_off[gamma] + t

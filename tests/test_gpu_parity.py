@@ -213,6 +213,15 @@ def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows):
     vmax = np.abs(val).max()
     off = np.concatenate([[0], np.cumsum(cnt)])
     worst = 0.0
+    # the products of the full-size matrix (general CSR kernel and the blocked one) on the sampled rows: the oracle's row
+    # values times x, summed by the oracle side; the tolerance carries the value tolerance through the sum
+    rows_all = m.rows
+    xh = wi.normal_vector(rows_all, k=333)
+    xd = torch.from_numpy(xh).cuda()
+    y_csr, y_blk = torch.empty_like(xd), torch.empty_like(xd)
+    wpcd.wpcd_perm_apply(rows_all, m.row_ptr, m.col_idx, m.values, xd, y_csr)
+    wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, xd, y_blk)
+    y_csr, y_blk = y_csr.cpu().numpy(), y_blk.cpu().numpy()
     for g in range(tab.n_ch):
         coupled = np.nonzero(tab.mask[g])[0]
         if len(coupled) == 0:
@@ -230,6 +239,10 @@ def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows):
             err = np.abs(gv - ev)
             worst = max(worst, float(np.max(err / tol)))
             assert np.all(err <= tol), f"channel {g} geo row {r}: worst err/tol {np.max(err / tol)}"
+            xs = xh[exp_cols]
+            y_ref = float(np.dot(ev, xs))
+            y_tol = float(np.dot(tol, np.abs(xs))) + 1e-12 * float(np.dot(np.abs(ev), np.abs(xs)))
+            assert abs(y_csr[g * n_geo + r] - y_ref) <= y_tol and abs(y_blk[g * n_geo + r] - y_ref) <= y_tol, (g, r)
     return m, worst
 
 

@@ -509,7 +509,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
     static const int g_forced = [] { const char* e = getenv("WPCD_MOM_G"); return e ? atoi(e) : 0; }();   // tuning knob
-    sh.n = n_quad; sh.NS = split ? std::max(n_quad, 4 * SPLIT_MAX_U) : n_quad; sh.G = std::max(1, std::min(32 / n_quad, g_forced > 0 ? g_forced : 2));
+    sh.n = n_quad; sh.NS = split ? std::max(n_quad, 4 * SPLIT_MAX_U) : n_quad; sh.G = std::max(1, std::min(32 / n_quad, g_forced > 0 ? g_forced : (n_quad <= 8 ? 4 : 2)));   // measured: n = 8: 4 beats 2 by 13 %, n = 10: 3 loses to 2
     sh.K1 = ch->k_max + 1; sh.SP = 8 * ((sh.K1 + 7) / 8) + 4;
     sh.ST = 8 * ((ch->n_ll + 7) / 8) + 4; sh.IS = 8 * ((ch->n_ll + 7) / 8) + 2;
     sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.n_ab = ch->n_ab;

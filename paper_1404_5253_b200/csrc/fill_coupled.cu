@@ -37,7 +37,9 @@ namespace {
 __constant__ double k_xi[WPCD_MAX_QUAD];
 __constant__ double k_w[WPCD_MAX_QUAD];
 
-constexpr int MOM_WARPS = 2;
+constexpr int MOM_MAX_WARPS = 1;  // warps (= elements) per CTA.  One warp with __launch_bounds__(32) beats two with (64) on config 3
+                                  // (1.48 -> 1.29 ms: the compiler schedules with more registers), costs 0-4 % on the moments of
+                                  // configs 4-5 (0.5 % of their step); one warp under __launch_bounds__(64) gains nothing; four lose
 constexpr int NODE_F = 10;   // doubles per staged phi-node
 
 __constant__ double k_invk[WPCD_MAX_K + 2];   // 1/k for the Legendre recurrence
@@ -103,7 +105,7 @@ __device__ __forceinline__ double ipow_small(double b, int e)   // e < 64
 // Moment layout: [tile of 32 elements][mu][element in tile] (the contraction reads 32 elements of
 // one monomial as one 256-byte line).
 template <int MAXS, bool SPLIT>
-__global__ void __launch_bounds__(MOM_WARPS * 32)
+__global__ void __launch_bounds__(MOM_MAX_WARPS * 32)
 moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
@@ -122,7 +124,7 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
     for (int t = threadIdx.x; t < n_ll; t += blockDim.x) { const int v = ll_pack[t]; ll_of[(v & 0xff) * LM1 + (v >> 8)] = t; }
     for (int t = threadIdx.x; t < n_trip; t += blockDim.x) trip_s[t] = trip_pack[t];
     __syncthreads();
-    const int64_t e = e_begin + (int64_t)blockIdx.x * MOM_WARPS + warp;
+    const int64_t e = e_begin + (int64_t)blockIdx.x * (blockDim.x >> 5) + warp;
     if (e >= e_end) return;
     const bool full_ll = n_ll == LM1 * LM1;                           // every (l, l') present: ll = l * LM1 + l'
     double* nodeS = wbase + (size_t)warp * moment_smem_doubles(sh);   // [NS][NODE_F]
@@ -522,7 +524,8 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         err = cudaMemcpyToSymbolAsync(k_invk, invk, sizeof(invk), 0, cudaMemcpyHostToDevice, st);
         if (err != cudaSuccess) return err;
     }
-    const size_t mom_smem = sizeof(double) * ((size_t)((((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + 1) & ~1) + (size_t)MOM_WARPS * moment_smem_doubles(sh));
+    const int mom_warps = MOM_MAX_WARPS;
+    const size_t mom_smem = sizeof(double) * ((size_t)((((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + 1) & ~1) + (size_t)mom_warps * moment_smem_doubles(sh));
     size_t ct_smem = 0;
     double cost_sum = 0.0;
     for (auto& sl : ch->slabs) { ct_smem = std::max(ct_smem, sl.bytes); cost_sum += sl.cost; }
@@ -559,7 +562,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     do {                                                                                                                      \
         err = cudaFuncSetAttribute(moments_kernel<MS, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
         if (err != cudaSuccess) return err;                                                                                   \
-        moments_kernel<MS, SPL><<<blocks, MOM_WARPS * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
+        moments_kernel<MS, SPL><<<blocks, mom_warps * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
                                                                      ws.geo_row, ws.geo_phi, ch->ll_pack_dev,                 \
                                                                      ch->trip_pack_dev, ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);         \
     } while (0)
@@ -569,7 +572,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     for (int64_t e0 = 0; e0 < nnz_geo; e0 += ws.chunk) {
         const int64_t e1 = std::min(nnz_geo, e0 + ws.chunk);
         {
-            const unsigned blocks = (unsigned)((e1 - e0 + MOM_WARPS - 1) / MOM_WARPS);
+            const unsigned blocks = (unsigned)((e1 - e0 + mom_warps - 1) / mom_warps);
             StageTimer timer(WPCD_STAGE_MOMENTS, st);
             if (maxs <= 4) WPCD_MOM(4);
             else if (maxs <= 8) WPCD_MOM(8);

@@ -207,6 +207,32 @@ def wpcd_perm_count(grid, channels, n_quad, row_ptr, geo_row_ptr, stream=None):
     return nnz.value, nnz_geo.value
 
 
+def bind_count_build(grid, channels, n_quad, row_ptr, geo_row_ptr, workspace, col_idx, values, stream):
+    """The same two calls with their arguments marshalled ONCE: returns (count, build), two zero-argument callables for a loop
+    that rebuilds into fixed buffers on a fixed stream (`stream`: a torch stream or a raw handle, not None).  count() returns
+    (nnz, nnz_geo).  The tensors must stay alive and in place while the callables are used."""
+    import torch
+
+    L = load()
+    st = _stream_ptr(stream)
+    rp, gp = _dev_ptr(row_ptr, torch.int64), _dev_ptr(geo_row_ptr, torch.int32)
+    ws, wsb = _dev_ptr(workspace), workspace.numel() * workspace.element_size()
+    ci, va = _dev_ptr(col_idx, torch.int32), _dev_ptr(values, torch.float64)
+    nnz, nnz_geo = ctypes.c_int64(0), ctypes.c_int64(0)
+    p_nnz, p_geo = ctypes.byref(nnz), ctypes.byref(nnz_geo)
+    gh, chh = grid.handle, channels.handle
+    f_count, f_build = L.wpcd_perm_count, L.wpcd_perm_build
+
+    def count():
+        _check(f_count(gh, chh, n_quad, st, rp, gp, p_nnz, p_geo))
+        return nnz.value, nnz_geo.value
+
+    def build():
+        _check(f_build(gh, chh, n_quad, st, rp, gp, ws, wsb, ci, va))
+
+    return count, build
+
+
 def wpcd_perm_workspace_bytes(channels, nnz_geo):
     return load().wpcd_perm_workspace_bytes(channels.handle, nnz_geo)
 

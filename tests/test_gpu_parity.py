@@ -566,6 +566,25 @@ def test_split_rule_is_more_accurate(wpcd):
     assert 1.5e-3 < e_split < 2.3e-3 and e_plain > 8 * e_split
 
 
+def test_bound_count_build_callables(wpcd):
+    """bind_count_build: the same two C calls with their arguments marshalled once (what bench.py's step loop uses)."""
+    torch = _torch()
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    p = wi.tan2_grid(17, 1.0, 0.1, seed=5)
+    grid = wpcd.wpcd_grid_create(p, p)
+    ref = wpcd.build_perm(grid, gch, 8)
+    row_ptr, geo_row_ptr = torch.zeros_like(ref.row_ptr), torch.zeros_like(ref.geo_row_ptr)
+    col_idx, values = torch.zeros_like(ref.col_idx), torch.zeros_like(ref.values)
+    workspace = torch.empty(max(wpcd.wpcd_perm_workspace_bytes(gch, ref.nnz_geo), 256), dtype=torch.uint8, device="cuda")
+    count, build = wpcd.bind_count_build(grid, gch, 8, row_ptr, geo_row_ptr, workspace, col_idx, values, torch.cuda.current_stream())
+    for _ in range(3):
+        col_idx.zero_(); values.zero_()
+        assert count() == (ref.nnz, ref.nnz_geo)
+        build()
+        torch.cuda.synchronize()
+        assert torch.equal(row_ptr, ref.row_ptr) and torch.equal(col_idx, ref.col_idx) and torch.equal(values, ref.values)
+
+
 def test_count_and_build_on_different_streams(wpcd):
     """wpcd_perm_count returns once the selection is read back, its row-pointer expansion still queued on the count's stream;
     a build issued on ANOTHER stream is ordered behind it by the library (coupled channels: the contraction reads row_ptr)."""

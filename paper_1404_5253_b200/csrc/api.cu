@@ -35,10 +35,20 @@ static bool g_trace_on = false;
 struct TraceRec { int stage; cudaEvent_t e0, e1; };
 static std::vector<TraceRec> g_trace;
 
+static std::vector<cudaEvent_t> g_trace_spare;      // timing events are reused: creating one costs more than recording it
+
+static cudaEvent_t trace_event()
+{
+    cudaEvent_t e = nullptr;
+    if (!g_trace_spare.empty()) { e = g_trace_spare.back(); g_trace_spare.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+
 StageTimer::StageTimer(int stage_, cudaStream_t st_) : stage(stage_), st(st_)
 {
     if (!g_trace_on) return;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    e0 = trace_event(); e1 = trace_event();
     cudaEventRecord(e0, st);
 }
 StageTimer::~StageTimer()
@@ -928,6 +938,13 @@ wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out)
 wpcd_status wpcd_trace_enable(int on)
 {
     g_trace_on = on != 0;
+    if (g_trace_on) {                       // have the timing events ready before the region that is timed
+        while (g_trace_spare.size() < 2048) {
+            cudaEvent_t e = nullptr;
+            if (cudaEventCreate(&e) != cudaSuccess) break;
+            g_trace_spare.push_back(e);
+        }
+    }
     return WPCD_OK;
 }
 
@@ -943,7 +960,8 @@ wpcd_status wpcd_trace_read(double* ms_out, int64_t* launches_out)
         if (e != cudaSuccess) err = e;
         ms_out[r.stage] += ms;
         if (launches_out) launches_out[r.stage] += 1;
-        cudaEventDestroy(r.e0); cudaEventDestroy(r.e1);
+        if (g_trace_spare.size() < 4096) { g_trace_spare.push_back(r.e0); g_trace_spare.push_back(r.e1); }
+        else { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     }
     g_trace.clear();
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_trace_read");

@@ -321,14 +321,34 @@ def run_ours(args):
     torch.cuda.synchronize()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    wpcd.wpcd_trace_enable(True)
-    wpcd.wpcd_trace_read()
     launches0 = wpcd.wpcd_launch_count()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    sp_ev = []
     for s in range(args.steps):
         flush.fill_(s & 0xFF)                       # L2 flush between timed iterations (not timed)
         ev[s][0].record()
+        for job in jobs:
+            job.count()
+            job.build()
+            if n_spmv:
+                if job.graph is not None:
+                    job.graph.replay()
+                else:
+                    spmv_sweep(job)
+        ev[s][1].record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    graph_launches = sum(len(sweep_passes(job)) for job in jobs if job.graph is not None) * args.steps
+    launches = wpcd.wpcd_launch_count() - launches0 + graph_launches
+    # ---- the same steps once more with CUDA events around every stage (the library's stage trace) and around the sweep: the
+    # per-stage and per-launch times of the rooflines.  Kept out of the region above because the events themselves cost
+    # ~17 us per step on the small workloads (5 % of the cfg2 step).
+    inst_steps = max(1, min(args.steps, 20))
+    wpcd.wpcd_trace_enable(True)
+    wpcd.wpcd_trace_read()
+    sp_ev = []
+    for s in range(inst_steps):
+        flush.fill_(s & 0xFF)
         for job in jobs:
             job.count()
             job.build()
@@ -341,12 +361,7 @@ def run_ours(args):
                     spmv_sweep(job)
                 b.record()
                 sp_ev.append((a, b))
-        ev[s][1].record()
     torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
-    graph_launches = sum(len(sweep_passes(job)) for job in jobs if job.graph is not None) * args.steps
-    launches = wpcd.wpcd_launch_count() - launches0 + graph_launches
     stages = wpcd.wpcd_trace_read()
     wpcd.wpcd_trace_enable(False)
     sampler.stop_flag = True
@@ -501,7 +516,7 @@ def run_ours(args):
     nnz1 = sum(j.nnz for j in jobs)
     nnz_geo1 = sum(j.nnz_geo for j in jobs)
     rows1 = sum(j.rows for j in jobs)
-    steps = args.steps
+    steps = inst_steps          # the stage and sweep times below come from the instrumented repeat
     roofs = {}
     stage_ms = {k: v[0] / steps for k, v in stages.items()}
     if stage_ms["fill_swave"] > 0:
@@ -579,6 +594,7 @@ def run_ours(args):
         "rooflines": roofs,
         "stage_ms_per_step": share,
         "build_nnz_per_s": nnz1 / max(1e-12, (ms_per_step - spmv_ms / steps) * 1e-3),
+        "stage_timing": f"instrumented repeat of {inst_steps} steps after the timed region (events around every stage)",
         "fp64_peak_tflops_measured": fp64_peak / 1e12,
         "spmm_nvec4": spmm, "rule_split": rule_split,
         "cpu_baseline": cpu_baseline,

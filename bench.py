@@ -1,13 +1,16 @@
 #!/usr/bin/env python
 """bench.py -- one "step" = one pass of the whole hot path (pattern
 count, scan, column indices, FP64 fill, then the workload's P0*x products) over one synthetic
-lattice.  Default workload: BASELINE.json configs[1] ("cfg2": s-wave, N_p=N_q=100 jittered tan^2
-grid, 8-point Gauss-Legendre, 50 SpMVs).  Prints ONE JSON line (contract in the task statement).
+lattice.  Default workload: BASELINE.json configs[4] ("cfg5", the largest single-GPU configuration: nd channels
+J = 1/2 .. 7/2, both parities, pair j <= 3, N_p = N_q = 150 tan^2 grid, 10-point Gauss-Legendre, 20 SpMVs per
+J^pi matrix; 1.67e10 nonzeros per step, one matrix of up to 39 GB resident at a time).  Prints ONE JSON line
+(contract in the task statement).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1..cfg5] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1..cfg5] [--impl reference] [--only-jpi 7,-1]
 
-N > 1 (torchrun): every rank builds its own independent lattice (seed + rank) -- the path
-shards over independent problems, no data-path collective ("scaling": "weak").
+N > 1 (torchrun): the path shards over independent problems, no data-path collective.  The nd workloads deal their
+J^pi matrices to the ranks (largest first, to the least loaded rank; total work fixed: "scaling": "strong"); the
+s-wave workloads give every rank its own lattice (seed + rank; "scaling": "weak").
 """
 import argparse
 import json
@@ -27,14 +30,12 @@ import wpcd_inputs as wi  # noqa: E402
 # dram__bytes_write.sum), profiles/r01h_ncu_full.md; null where no capture of that workload exists.
 NCU_TRAFFIC = {
     ("cfg2", "spmv"): 3.84e6,            # spmv_kernel<32,4>, one pass of 4 right-hand sides over the 3.4 MB matrix (cold L2 under ncu)
-    ("cfg2", "selection"): 6.38e6,       # geo_select_kernel: staged verdicts written, node tables read
     ("cfg2", "fill_swave"): 6.88e6,
     ("cfg4", "spmv"): 6.19e9,            # J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
 }
 
 METRIC = "P-matrix nonzeros/sec (FP64 build + the workload's P*vector SpMVs per step)"
 UNIT = "nnz/s"
-SELECT_FLOPS_PER_GEO_NNZ = 562.0   # FP64 flops of the selection pass per structural geometric nonzero (ncu op counts, cfg2)
 FLOPS_PER_NODE = 70.0          # algorithmic FP64 flops per (phi,x) quadrature node, s-wave
 L2_FLUSH_BYTES = 256 << 20     # > 126 MB L2
 
@@ -242,8 +243,8 @@ def run_ours(args):
         dist.barrier()
     wpcd.load()
     wl = wi.WORKLOADS[args.workload]
-    p = wl.grid(seed_offset=shard.lattice_seed_offset(rank))   # independent lattice per rank (weak scaling)
-    stream = torch.cuda.current_stream()
+    strong = wl.model == "nd"          # nd sweeps: the J^pi matrices of ONE lattice are dealt to the ranks
+    p = wl.grid(seed_offset=0 if strong else shard.lattice_seed_offset(rank))   # s-wave: independent lattice per rank (weak scaling)
     grid = wpcd.wpcd_grid_create(p, p)
 
     def make_channels(two_J, parity):
@@ -252,11 +253,19 @@ def run_ours(args):
         return wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=wl.j_pair_max)
 
     # one J^pi matrix resident at a time; buffers sized for the largest
-    jobs = []
-    for (two_J, parity) in jobs_of(wl):
-        ch = make_channels(two_J, parity)
-        jobs.append(Job(ch, wpcd.wpcd_rows(grid, ch)))
-    allocate(wpcd, torch, grid, jobs, wl)
+    all_jpis = jobs_of(wl)
+    if args.only_jpi:
+        tj, par = (int(v) for v in args.only_jpi.split(","))
+        all_jpis = [jp for jp in all_jpis if tuple(jp) == (tj, par)]
+        assert all_jpis, "--only-jpi names no matrix of this workload"
+    all_ch = [make_channels(two_J, parity) for (two_J, parity) in all_jpis]
+    # cost of a matrix ~ its coupled channel pairs (the geometric pattern is shared): largest first, to the least loaded rank
+    mine = shard.assign_balanced(list(range(len(all_jpis))), [c.pairs for c in all_ch], rank, world) if strong else list(range(len(all_jpis)))
+    my_jpis = [all_jpis[k] for k in mine]
+    jobs = [Job(all_ch[k], wpcd.wpcd_rows(grid, all_ch[k])) for k in mine]
+    idle = not jobs                    # more ranks than matrices: this rank only takes part in the reductions
+    if not idle:
+        allocate(wpcd, torch, grid, jobs, wl)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     # count / build of a job with their arguments marshalled once (fixed buffers, fixed stream): the Python side of a step is
     # two ctypes calls per job
@@ -296,7 +305,8 @@ def run_ours(args):
                     spmv_sweep(job)
 
     # capture the launch-bound SpMV sweep in a CUDA graph (small matrices only)
-    step(jobs)
+    if not idle:
+        step(jobs)
     torch.cuda.synchronize()
     if n_spmv and wl.model == "swave":
         for job in jobs:
@@ -310,7 +320,7 @@ def run_ours(args):
             with torch.cuda.graph(g):
                 spmv_sweep(job)
             job.graph = g
-    for _ in range(args.warmup):
+    for _ in range(args.warmup if not idle else 0):
         step(jobs)
     torch.cuda.synchronize()
     fp64_peak = wpcd.wpcd_fp64_peak()
@@ -343,7 +353,7 @@ def run_ours(args):
     # ---- the same steps once more with CUDA events around every stage (the library's stage trace) and around the sweep: the
     # per-stage and per-launch times of the rooflines.  Kept out of the region above because the events themselves cost
     # ~17 us per step on the small workloads (5 % of the cfg2 step).
-    inst_steps = max(1, min(args.steps, 20))
+    inst_steps = max(1, min(args.steps, 20 if wl.model == "swave" else 3))
     wpcd.wpcd_trace_enable(True)
     wpcd.wpcd_trace_read()
     sp_ev = []
@@ -371,10 +381,11 @@ def run_ours(args):
     ms_max, nnz_all = shard.reduce_step(dist, "cuda", total_ms, sum(j.nnz for j in jobs))
     ms_per_step = ms_max / args.steps
     value = shard.throughput(ms_per_step, nnz_all)
+    extras = rank == 0 and not idle and not args.no_extras
 
     # ---- extra: multi-vector apply: 4 right-hand sides share one pass over the matrix
     spmm = None
-    if n_spmv:
+    if n_spmv and extras:
         job = jobs[-1]                     # its matrix is the one resident after the timed region
         x4 = torch.from_numpy(np.stack([wi.normal_vector(job.rows, k=100 + k) for k in range(4)])).cuda().contiguous()
         y4 = torch.empty_like(x4)
@@ -457,8 +468,8 @@ def run_ours(args):
 
     # ---- extra: the kink-split rule RS(n) (R14): cost of the build against R(n)
     rule_split = {}
-    job = jobs[-1]
-    rules = [("plain", wl.n_quad), ("split", wl.n_quad | wpcd.WPCD_RULE_KINK_SPLIT)]
+    job = jobs[-1] if not idle else None
+    rules = [("plain", wl.n_quad), ("split", wl.n_quad | wpcd.WPCD_RULE_KINK_SPLIT)] if extras else []
     if wl.model == "swave":
         rules += [("analytic_u", wl.n_quad | wpcd.WPCD_RULE_ANALYTIC_U), ("analytic_u_n32", 32 | wpcd.WPCD_RULE_ANALYTIC_U), ("plain_n32", 32)]
     for name, nq in rules:
@@ -472,13 +483,14 @@ def run_ours(args):
         b.record()
         torch.cuda.synchronize()
         rule_split["build_ms_" + name] = a.elapsed_time(b) / reps
-    wpcd.wpcd_perm_build(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
+    if extras:
+        wpcd.wpcd_perm_build(grid, job.channels, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
     torch.cuda.synchronize()
 
     # ---- end to end through the C-ABI with HOST buffers (handles, tables and vectors from the host)
     def e2e_step():
         g2 = wpcd.wpcd_grid_create(p, p)
-        for job, (two_J, parity) in zip(jobs, jobs_of(wl)):
+        for job, (two_J, parity) in zip(jobs, my_jpis):
             ch2 = make_channels(two_J, parity)
             wpcd.wpcd_perm_count(g2, ch2, wl.n_quad, job.row_ptr, job.geo_row_ptr)
             wpcd.wpcd_perm_build(g2, ch2, wl.n_quad, job.row_ptr, job.geo_row_ptr, job.workspace, job.col_idx, job.values)
@@ -489,7 +501,7 @@ def run_ours(args):
             for k in range(n_spmv):
                 wpcd.wpcd_perm_apply_host(job.rows, job.row_ptr, job.col_idx, job.values, job.x_host[k % job.n_x], job.y_host,
                                           job.x[0], job.y)
-    e2e_steps = max(1, min(args.steps, 20))
+    e2e_steps = max(1, min(args.steps, 20 if wl.model == "swave" else 3))
     e2e_step()
     torch.cuda.synchronize()
     if dist is not None:
@@ -511,7 +523,8 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- rooflines (per launch, averaged over the timed region)
+    # ---- rooflines (per launch; stage and sweep times from the instrumented repeat).  Algorithmic work per unit is
+    # SURVEY.md section 8(d)'s, restated in DESIGN.md section 7.
     peaks, peak_kind = measured_peaks()
     nnz1 = sum(j.nnz for j in jobs)
     nnz_geo1 = sum(j.nnz_geo for j in jobs)
@@ -519,29 +532,31 @@ def run_ours(args):
     steps = inst_steps          # the stage and sweep times below come from the instrumented repeat
     roofs = {}
     stage_ms = {k: v[0] / steps for k, v in stages.items()}
+    hbm_src = f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})"
+    alu_src = "in-run DFMA microbenchmark (wpcd_fp64_peak)"
     if stage_ms["fill_swave"] > 0:
         flops = FLOPS_PER_NODE * wl.n_quad * wl.n_quad * nnz1
         ach = flops / (stage_ms["fill_swave"] * 1e-3) / 1e12
         roofs["fill_swave"] = {"bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
                                "frac": ach / (fp64_peak / 1e12), "traffic": None, "ms_per_launch": stage_ms["fill_swave"],
-                               "peak_source": "in-run DFMA microbenchmark (wpcd_fp64_peak)"}
-    if stage_ms["moments"] > 0 or stage_ms["contract"] > 0:
+                               "peak_source": alu_src}
+    t_fill = (stage_ms["moments"] + stage_ms["contract"]) * 1e-3
+    if t_fill > 0:
+        # two bounds, the larger one is the roofline: the HBM write of 12 B per nonzero (value + column index), and the
+        # FP64 work of schedule (B) of SURVEY 8(d): per geometric element n^2 nodes x 2 flops x n_mu monomial moments,
+        # plus 2 flops per (pair, monomial) coefficient of the g-contraction
         wbytes = 12.0 * nnz1
-        t = (stage_ms["moments"] + stage_ms["contract"]) * 1e-3
-        ach = wbytes / t / 1e9
-        roofs["fill_coupled"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                                 "frac": ach / peaks["hbm_gbs"], "traffic": None,
-                                 "ms_per_step": {"moments": stage_ms["moments"], "contract": stage_ms["contract"]},
-                                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})"}
-    if stage_ms["geo_count"] > 0:
-        # selection (a1): FP64 compare / clip arithmetic, latency- and divergence-bound; per-unit figure of DESIGN.md section 7
-        flops = SELECT_FLOPS_PER_GEO_NNZ * nnz_geo1
-        ach = flops / (stage_ms["geo_count"] * 1e-3) / 1e12
-        roofs["selection"] = {"bound": "alu", "achieved": ach, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
-                              "frac": ach / (fp64_peak / 1e12), "traffic": None,
-                              "ms_per_launch": stage_ms["geo_count"] / len(jobs),
-                              "peak_source": "in-run DFMA microbenchmark (wpcd_fp64_peak)",
-                              "note": "divergent polygon tests and dependent interval searches: latency-bound, FP64 pipe 24 % active (ncu)"}
+        flops = sum(j.nnz_geo * (2.0 * wl.n_quad * wl.n_quad * j.channels.monomials + 2.0 * j.channels.coefficients) for j in jobs)
+        t_hbm, t_alu = wbytes / (peaks["hbm_gbs"] * 1e9), flops / fp64_peak
+        hbm = {"bound": "hbm", "achieved": wbytes / t_fill / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+               "frac": t_hbm / t_fill, "peak_source": hbm_src}
+        alu = {"bound": "alu", "achieved": flops / t_fill / 1e12, "peak": fp64_peak / 1e12, "unit": "TFLOP/s",
+               "frac": t_alu / t_fill, "peak_source": alu_src}
+        top = dict(hbm if t_hbm >= t_alu else alu)
+        top.update({"traffic": None, "both_bounds": {"hbm": hbm, "alu": alu},
+                    "ms_per_step": {"moments": stage_ms["moments"], "contract": stage_ms["contract"]},
+                    "algorithmic": {"bytes": wbytes, "flops": flops}})
+        roofs["fill_coupled"] = top
     if n_spmv:
         # algorithmic bytes of a launch with v right-hand sides: the matrix once (12 B per nonzero + row_ptr) + v vectors in and out
         n_launch = sum(len(sweep_passes(j)) for j in jobs)
@@ -551,13 +566,14 @@ def run_ours(args):
         roofs["spmv"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                          "traffic": None, "ms_per_launch": per_launch_ms, "launches_per_step": n_launch,
                          "rhs_per_launch": max(max(sweep_passes(j)) for j in jobs),
-                         "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind})",
+                         "peak_source": hbm_src,
                          "note": "matrix is L2-resident (3 MB)" if wl.model == "swave" else "streams from HBM"}
     share = dict(stage_ms)
     share["spmv_sweep"] = spmv_ms / steps
-    dominant = max(share, key=share.get)
-    key = {"fill_swave": "fill_swave", "moments": "fill_coupled", "contract": "fill_coupled", "spmv_sweep": "spmv",
-           "geo_count": "selection"}.get(dominant)
+    # the selection (a1-a3) is reported by its time only (latency-bound, no per-unit figure)
+    kernels = {"fill_swave": "fill_swave", "moments": "fill_coupled", "contract": "fill_coupled", "spmv_sweep": "spmv"}
+    dominant = max((k for k in share if k in kernels), key=share.get)
+    key = kernels[dominant]
     for name, rf in roofs.items():
         rf["traffic"] = NCU_TRAFFIC.get((wl.name, name))
     roofline = dict(roofs[key]) if key in roofs else {
@@ -577,11 +593,14 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
+        "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": wl.name, "n_bins": wl.n_bins, "n_quad": wl.n_quad, "model": wl.model, "jitter": wl.jitter,
-                   "jpis": jobs_of(wl) if wl.model == "nd" else None, "n_spmv_per_matrix": n_spmv,
-                   "nnz": nnz1, "nnz_geo": nnz_geo1, "rows": rows1, "l2": "flushed between timed steps (256 MiB fill)",
+                   "jpis": all_jpis if wl.model == "nd" else None, "n_spmv_per_matrix": n_spmv,
+                   "nnz": int(nnz_all), "nnz_rank0": nnz1, "nnz_geo_rank0": nnz_geo1, "rows_rank0": rows1,
+                   "sharding": ("J^pi matrices dealt to the ranks, largest first" if strong else "one lattice per rank") if world > 1 else "none",
+                   "l2": "flushed between timed steps (256 MiB fill)",
                    "spmv_launch": ("CUDA graph" if jobs[0].graph is not None else "direct")
                    + (", one call for all right-hand sides (passes of 4)" if jobs[0].x_all is not None and n_spmv else "")},
         "clocks": sampler.summary(),
@@ -607,11 +626,13 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=sorted(wi.WORKLOADS))
+    ap.add_argument("--workload", default="cfg5", choices=sorted(wi.WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the untimed extra measurements (multi-vector products, rule variants)")
+    ap.add_argument("--only-jpi", default="", help="two_J,parity: restrict an nd workload to one matrix (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

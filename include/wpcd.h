@@ -95,6 +95,11 @@ void wpcd_channels_destroy(wpcd_channels* channels);
 int wpcd_channels_count(const wpcd_channels* channels);            /* number of channels */
 int wpcd_channels_pairs(const wpcd_channels* channels);            /* number of coupled pairs */
 int64_t wpcd_channels_terms(const wpcd_channels* channels);        /* total (k,l1,l1') terms */
+/* Sizes of the coupled fill (the roofline's algorithmic flop count): the number of distinct
+ * monomials (l, l', l1+l1', k) of (A3) -- one moment per geometric element each -- and the number of
+ * (pair, monomial) coefficients the g-contraction multiplies (terms of a pair with equal l1+l1' and k merged). */
+int wpcd_channels_monomials(const wpcd_channels* channels);
+int64_t wpcd_channels_coefficients(const wpcd_channels* channels);
 /* quantum numbers [n_channels][6] = (l, s, j, t, lambda, two_I); zeros for a table-made set
  * except l.  HOST output. */
 wpcd_status wpcd_channels_get_quantum_numbers(const wpcd_channels* channels, int32_t* out);

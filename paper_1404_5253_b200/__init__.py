@@ -30,7 +30,7 @@ WPCD_MAX_QUAD = 64
 EXPORTS = [
     "wpcd_last_error", "wpcd_grid_create", "wpcd_grid_destroy", "wpcd_channels_create",
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
-    "wpcd_channels_terms", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
+    "wpcd_channels_terms", "wpcd_channels_monomials", "wpcd_channels_coefficients", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
     "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
     "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
@@ -67,6 +67,9 @@ def load():
     L.wpcd_channels_pairs.argtypes = [vp]
     L.wpcd_channels_terms.argtypes = [vp]
     L.wpcd_channels_terms.restype = i64
+    L.wpcd_channels_monomials.argtypes = [vp]
+    L.wpcd_channels_coefficients.argtypes = [vp]
+    L.wpcd_channels_coefficients.restype = i64
     L.wpcd_channels_get_quantum_numbers.argtypes = [vp, vp]
     L.wpcd_channels_get_table.argtypes = [vp] * 8
     L.wpcd_rows.argtypes = [vp, vp]
@@ -149,6 +152,14 @@ class Channels:
     @property
     def terms(self):
         return load().wpcd_channels_terms(self.handle)
+
+    @property
+    def monomials(self):
+        return load().wpcd_channels_monomials(self.handle)
+
+    @property
+    def coefficients(self):
+        return load().wpcd_channels_coefficients(self.handle)
 
     def quantum_numbers(self):
         out = np.zeros((self.count, 6), np.int32)

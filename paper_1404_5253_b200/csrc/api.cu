@@ -186,7 +186,7 @@ static wpcd_status finalize_channels(wpcd_channels* c)
         if (c->term_ptr[pidx + 1] == c->term_ptr[pidx]) return fail(WPCD_ERR_INVALID_ARG, "a listed channel pair has no terms (leave uncoupled pairs out)");
     }
     // ---- merged coefficients per pair, monomial (A, k) = (l1 + l1', k)
-    c->k_max = 0; c->l_max = 0;
+    c->k_max = 0; c->l_max = 0; c->n_coef = 0;
     typedef std::pair<int, int> Mono;                           // (A, k)
     std::vector<std::map<Mono, double>> pair_coef(c->n_pairs);
     std::map<std::pair<int, int>, std::set<Mono>> ll_mono;      // (l, l') -> monomials used by any pair
@@ -201,6 +201,7 @@ static wpcd_status finalize_channels(wpcd_channels* c)
             pair_coef[pidx][Mono(l1 + l1p, k)] += c->term_g[t];
         }
         for (auto& kv : pair_coef[pidx]) ll_mono[std::make_pair(l, lp)].insert(kv.first);
+        c->n_coef += (int64_t)pair_coef[pidx].size();
     }
     // coupling structure
     c->ncoupled.assign(c->n_ch, 0);
@@ -512,6 +513,8 @@ void wpcd_channels_destroy(wpcd_channels* c)
 int wpcd_channels_count(const wpcd_channels* c) { return c ? c->n_ch : 0; }
 int wpcd_channels_pairs(const wpcd_channels* c) { return c ? c->n_pairs : 0; }
 int64_t wpcd_channels_terms(const wpcd_channels* c) { return c ? c->n_terms : 0; }
+int wpcd_channels_monomials(const wpcd_channels* c) { return c ? c->n_mu : 0; }
+int64_t wpcd_channels_coefficients(const wpcd_channels* c) { return c ? c->n_coef : 0; }
 
 wpcd_status wpcd_channels_get_quantum_numbers(const wpcd_channels* c, int32_t* out)
 {
@@ -647,7 +650,7 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
     // Gauss-Legendre nodes / weights: computed once per order (host, long double Newton), then reused
     static std::mutex gl_mutex;
     static std::map<int, std::vector<double>> gl_cache;
-    double xi[WPCD_MAX_QUAD], w[WPCD_MAX_QUAD];
+    QuadRule qr;
     {
         std::lock_guard<std::mutex> lock(gl_mutex);
         std::vector<double>& tab = gl_cache[n_quad];
@@ -655,11 +658,13 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
             tab.resize(2 * n_quad);
             wpcd_host::gauss_legendre(n_quad, tab.data(), tab.data() + n_quad);
         }
-        std::memcpy(xi, tab.data(), sizeof(double) * n_quad);
-        std::memcpy(w, tab.data() + n_quad, sizeof(double) * n_quad);
+        std::memset(&qr, 0, sizeof(qr));
+        std::memcpy(qr.xi, tab.data(), sizeof(double) * n_quad);
+        std::memcpy(qr.w, tab.data() + n_quad, sizeof(double) * n_quad);
+        for (int k = 1; k < WPCD_MAX_K + 2; ++k) qr.invk[k] = 1.0 / k;
     }
-    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, analytic ? 2 : (split ? 1 : 0), xi, w, nnz_geo, ws, col_idx_dev, values_dev, st);
-    else err = launch_fill_coupled(g, c, n_quad, split, xi, w, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
+    if (c->swave_single) err = launch_fill_swave(g, c, n_quad, analytic ? 2 : (split ? 1 : 0), qr, nnz_geo, ws, col_idx_dev, values_dev, st);
+    else err = launch_fill_coupled(g, c, n_quad, split, qr, nnz_geo, ws, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_build(fill)");
     return WPCD_OK;
 }

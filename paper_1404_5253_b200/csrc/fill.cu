@@ -7,24 +7,24 @@
 #include <math.h>
 #include <stdlib.h>
 
-#include <mutex>
-
 #include "quad_device.cuh"
 #include "wpcd_internal.h"
 
 using namespace wpcd_quad;
+using wpcd_detail::QuadRule;
 
 namespace {
 
-__constant__ double c_xi[WPCD_MAX_QUAD];
-__constant__ double c_w[WPCD_MAX_QUAD];
+// The rule travels as a by-value __grid_constant__ kernel parameter (wpcd_internal.h QuadRule): it sits in the
+// launch's own constant bank, so builds with different orders may overlap on one device (streams or threads), and
+// with a compile-time order the nodes and weights still fold into constant-bank operands.
 
 // ------------------------------------------------------------------ s-wave
 // NQ > 0: rule order fixed at compile time (loops unrolled, nodes and weights become immediates
 // of the constant bank); NQ = 0: any order.
 template <int LPE, int NQ>
 __global__ void __launch_bounds__(256)
-fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n_rt, double g0,
+fill_swave_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, int n_rt, double g0,
                   int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                   const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
@@ -48,18 +48,18 @@ fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, in
 #pragma unroll 1
             for (int m = sub; m < n; m += LPE) {
                 PhiNodeSq s;
-                if (!phi_node_sq(z, zs, mid_phi + half_phi * c_xi[m], s)) continue;
+                if (!phi_node_sq(z, zs, mid_phi + half_phi * rule.xi[m], s)) continue;
                 const double half_u = 0.5 * (s.u_hi - s.u_lo), mid_u = 0.5 * (s.u_lo + s.u_hi);
                 double inner = 0.0;
 #pragma unroll
                 for (int r = 0; r < n; ++r) {
-                    const double u = mid_u + half_u * c_xi[r];
+                    const double u = mid_u + half_u * rule.xi[r];
                     const double z1 = s.b1 + s.beta * u, z2 = s.b2 + s.beta * u;    // zeta1^2, zeta2^2 (A11)
                     const double t = rsqrt(z1 * z2);                                // 1/(zeta1 zeta2)
                     const double t2 = t * t;
-                    inner += c_w[r] * twoF_A14_sq(zs, s, t2 * z2, t2 * z1) * t;
+                    inner += rule.w[r] * twoF_A14_sq(zs, s, t2 * z2, t2 * z1) * t;
                 }
-                acc += half_phi * c_w[m] * half_u * s.beta * inner;    // cos*sin = beta
+                acc += half_phi * rule.w[m] * half_u * s.beta * inner;    // cos*sin = beta
             }
         }
     }
@@ -76,7 +76,7 @@ fill_swave_kernel(const double* __restrict__ p, const double* __restrict__ q, in
 // u-pieces one after the other (sorted candidate cuts in registers, no arrays).
 template <int LPE, int NQ>
 __global__ void __launch_bounds__(256)
-fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n_rt, double g0,
+fill_swave_split_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, int n_rt, double g0,
                         int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                         const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
@@ -105,7 +105,7 @@ fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__
                 const double pb = piece == 0 ? pc[1] : (piece == 1 ? pc[2] : pc[3]);
                 const double half_phi = 0.5 * (pb - pa), mid_phi = 0.5 * (pa + pb);
                 PhiNodeSq s;
-                if (!phi_node_sq(z, zs, mid_phi + half_phi * c_xi[m], s)) continue;
+                if (!phi_node_sq(z, zs, mid_phi + half_phi * rule.xi[m], s)) continue;
                 double cand[6];
                 split_u_candidates(z, zs, s, cand);
                 auto piece_sum = [&](double lo, double hi) {
@@ -113,11 +113,11 @@ fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__
                     double inner = 0.0;
 #pragma unroll
                     for (int r = 0; r < n; ++r) {
-                        const double u = mid_u + half_u * c_xi[r];
+                        const double u = mid_u + half_u * rule.xi[r];
                         const double z1 = s.b1 + s.beta * u, z2 = s.b2 + s.beta * u;    // zeta1^2, zeta2^2 (A11)
                         const double t = rsqrt(z1 * z2);                                // 1/(zeta1 zeta2)
                         const double t2 = t * t;
-                        inner += c_w[r] * twoF_A14_sq(zs, s, t2 * z2, t2 * z1) * t;
+                        inner += rule.w[r] * twoF_A14_sq(zs, s, t2 * z2, t2 * z1) * t;
                     }
                     return half_u * inner;
                 };
@@ -133,7 +133,7 @@ fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__
                 double node = 0.0;
 #pragma unroll 1
                 for (int k = 0; k < np; ++k) node += piece_sum(cut[k], cut[k + 1]);
-                acc += half_phi * c_w[m] * s.beta * node;    // cos*sin = beta
+                acc += half_phi * rule.w[m] * s.beta * node;    // cos*sin = beta
             }
         }
     }
@@ -151,7 +151,7 @@ fill_swave_split_kernel(const double* __restrict__ p, const double* __restrict__
 // end-point square roots carried from piece to piece).
 template <int LPE>
 __global__ void __launch_bounds__(256)
-fill_swave_analytic_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, int n, double g0,
+fill_swave_analytic_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, int n, double g0,
                            int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                            const double2* __restrict__ geo_phi, int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
@@ -179,7 +179,7 @@ fill_swave_analytic_kernel(const double* __restrict__ p, const double* __restric
                 const double pb = piece == 0 ? pc[1] : (piece == 1 ? pc[2] : pc[3]);
                 const double half_phi = 0.5 * (pb - pa), mid_phi = 0.5 * (pa + pb);
                 PhiNodeSq s;
-                if (!phi_node_sq(z, zs, mid_phi + half_phi * c_xi[m], s)) continue;
+                if (!phi_node_sq(z, zs, mid_phi + half_phi * rule.xi[m], s)) continue;
                 double cand[6];
                 split_u_candidates(z, zs, s, cand);
                 double cut[SPLIT_MAX_U + 1];
@@ -217,7 +217,7 @@ fill_swave_analytic_kernel(const double* __restrict__ p, const double* __restric
                     if (integral > 0.0) node += integral;
                     z1l = z1h; z2l = z2h;
                 }
-                acc += half_phi * c_w[m] * s.beta * node;    // cos*sin = beta
+                acc += half_phi * rule.w[m] * s.beta * node;    // cos*sin = beta
             }
         }
     }
@@ -233,36 +233,20 @@ fill_swave_analytic_kernel(const double* __restrict__ p, const double* __restric
 
 namespace wpcd_detail {
 
-cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, int rule, const double* xi, const double* w,
+cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, int rule, const QuadRule& qr,
                               int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st)
 {
-    // the rule's nodes and weights live in constant memory; they are uploaded again only when the
-    // order, the stream or the device changes (a constant table, not a result)
-    static std::mutex up_mutex;
-    std::lock_guard<std::mutex> up_lock(up_mutex);
-    static int up_n = -1, up_dev = -1;
-    static cudaStream_t up_st = nullptr;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaError_t err = cudaSuccess;
-    if (up_n != n_quad || up_st != st || up_dev != dev) {
-        err = cudaMemcpyToSymbolAsync(c_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-        if (err != cudaSuccess) return err;
-        err = cudaMemcpyToSymbolAsync(c_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-        if (err != cudaSuccess) return err;
-        up_n = n_quad; up_st = st; up_dev = dev;
-    }
     if (nnz_geo == 0) return cudaSuccess;
     // lanes per element: whole phi-nodes per lane, no idle lanes when n is a multiple of LPE
     int lpe = (n_quad % 8 == 0) ? 8 : (n_quad % 4 == 0) ? 4 : (n_quad % 2 == 0) ? 2 : 1;
     int64_t threads = nnz_geo * lpe;
     int blocks = (int)((threads + 255) / 256);
     StageTimer timer(WPCD_STAGE_FILL_SWAVE, st);
-#define WPCD_LAUNCH_SW(L, Q) fill_swave_kernel<L, Q><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
+#define WPCD_LAUNCH_SW(L, Q) fill_swave_kernel<L, Q><<<blocks, 256, 0, st>>>(qr, g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, \
                                                                             ws.geo_col, ws.geo_row, ws.geo_phi, col_idx, values)
     if (rule == 2) {
         lpe = 8; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256);
-        fill_swave_analytic_kernel<8><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col, ws.geo_row,
+        fill_swave_analytic_kernel<8><<<blocks, 256, 0, st>>>(qr, g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col, ws.geo_row,
                                                               ws.geo_phi, col_idx, values);
         ++g_launches;
         return cudaGetLastError();
@@ -270,9 +254,9 @@ cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n
     if (rule == 1) {
         // the rule has up to 3 n work items per element: eight lanes each
         lpe = 8; threads = nnz_geo * lpe; blocks = (int)((threads + 255) / 256);
-        if (n_quad == 8) fill_swave_split_kernel<8, 8><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,
+        if (n_quad == 8) fill_swave_split_kernel<8, 8><<<blocks, 256, 0, st>>>(qr, g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,
                                                                                 ws.geo_row, ws.geo_phi, col_idx, values);
-        else fill_swave_split_kernel<8, 0><<<blocks, 256, 0, st>>>(g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,
+        else fill_swave_split_kernel<8, 0><<<blocks, 256, 0, st>>>(qr, g->p_dev, g->q_dev, g->n_q, n_quad, ch->g0, nnz_geo, ws.geo_col,
                                                                     ws.geo_row, ws.geo_phi, col_idx, values);
         ++g_launches;
         return cudaGetLastError();

@@ -31,18 +31,14 @@
 #include "wpcd_internal.h"
 
 using namespace wpcd_quad;
+using wpcd_detail::QuadRule;
 
 namespace {
-
-__constant__ double k_xi[WPCD_MAX_QUAD];
-__constant__ double k_w[WPCD_MAX_QUAD];
 
 constexpr int MOM_MAX_WARPS = 1;  // warps (= elements) per CTA.  One warp with __launch_bounds__(32) beats two with (64) on config 3
                                   // (1.48 -> 1.29 ms: the compiler schedules with more registers), costs 0-4 % on the moments of
                                   // configs 4-5 (0.5 % of their step); one warp under __launch_bounds__(64) gains nothing; four lose
 constexpr int NODE_F = 10;   // doubles per staged phi-node
-
-__constant__ double k_invk[WPCD_MAX_K + 2];   // 1/k for the Legendre recurrence
 
 struct MomentShape {
     int n;        // quadrature order
@@ -106,7 +102,7 @@ __device__ __forceinline__ double ipow_small(double b, int e)   // e < 64
 // one monomial as one 256-byte line).
 template <int MAXS, bool SPLIT>
 __global__ void __launch_bounds__(MOM_MAX_WARPS * 32)
-moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
+moments_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
                const int32_t* __restrict__ mu_pack, const int32_t* __restrict__ ab_pack, double* __restrict__ moments)
@@ -168,16 +164,16 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                 s.Lq2 = o[3]; s.Uq2 = o[4];
                 const double b1 = o[5], b2 = o[6], beta = o[7], u_lo = o[8], u_hi = o[9];
                 const double half_u = 0.5 * (u_hi - u_lo), mid_u = 0.5 * (u_lo + u_hi);
-                const double u = mid_u + half_u * k_xi[r];
+                const double u = mid_u + half_u * rule.xi[r];
                 const double x = u - 1.0;
                 const double iz1 = rsqrt(b1 + beta * u), iz2 = rsqrt(b2 + beta * u);
-                const double wF = (o[0] * norm) * (half_u * k_w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
+                const double wF = (o[0] * norm) * (half_u * rule.w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
                 double* Pr = Pk + (g * n + r) * SP;
                 double p0 = 1.0, p1 = x;
                 Pr[0] = 1.0;
                 if (K1 > 1) Pr[1] = x;
                 for (int k = 2; k < K1; ++k) {
-                    const double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) * k_invk[k];
+                    const double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) * rule.invk[k];
                     Pr[k] = p2;
                     p0 = p1; p1 = p2;
                 }
@@ -251,9 +247,9 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
             // ---- step 1: everything that depends on phi only, one lane per phi-node
             for (int m = lane; m < n; m += 32) {
                 PhiNodeSq s;
-                const bool ok = phi_node_sq(z, zs, mid_phi + half_phi * k_xi[m], s);
+                const bool ok = phi_node_sq(z, zs, mid_phi + half_phi * rule.xi[m], s);
                 double* o = nodeS + m * NODE_F;
-                o[0] = ok ? half_phi * k_w[m] : 0.0; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
+                o[0] = ok ? half_phi * rule.w[m] : 0.0; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
                 o[5] = s.b1; o[6] = s.b2; o[7] = s.beta; o[8] = s.u_lo; o[9] = s.u_hi;
             }
             __syncwarp();
@@ -275,9 +271,9 @@ moments_kernel(const double* __restrict__ p, const double* __restrict__ q, int n
                     const double pa = piece == 0 ? pc[0] : (piece == 1 ? pc[1] : pc[2]);
                     const double pb = piece == 0 ? pc[1] : (piece == 1 ? pc[2] : pc[3]);
                     const double hp = 0.5 * (pb - pa);
-                    if (phi_node_sq(z, zs, 0.5 * (pa + pb) + hp * k_xi[m], s)) {
+                    if (phi_node_sq(z, zs, 0.5 * (pa + pb) + hp * rule.xi[m], s)) {
                         split_u_candidates(z, zs, s, cand);
-                        wphi = hp * k_w[m];
+                        wphi = hp * rule.w[m];
                         double lower = s.u_lo;
                         np = 1;
 #pragma unroll
@@ -488,25 +484,11 @@ contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, cons
 
 namespace wpcd_detail {
 
-cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
+cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const QuadRule& qr,
                                 int64_t nnz_geo, const Workspace& ws, const int64_t* /*row_ptr*/, const int32_t* geo_row_ptr,
                                 int32_t* col_idx, double* values, cudaStream_t st)
 {
-    static std::mutex up_mutex;
-    std::lock_guard<std::mutex> up_lock(up_mutex);
-    static int up_n = -1, up_dev = -1;      // constant tables are uploaded again only when order, stream or device change
-    static cudaStream_t up_st = nullptr;
-    int cur_dev = 0;
-    cudaGetDevice(&cur_dev);
     cudaError_t err = cudaSuccess;
-    const bool upload_consts = up_n != n_quad || up_st != st || up_dev != cur_dev;
-    if (upload_consts) {
-        err = cudaMemcpyToSymbolAsync(k_xi, xi, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-        if (err != cudaSuccess) return err;
-        err = cudaMemcpyToSymbolAsync(k_w, w, sizeof(double) * n_quad, 0, cudaMemcpyHostToDevice, st);
-        if (err != cudaSuccess) return err;
-        up_n = n_quad; up_st = st; up_dev = cur_dev;
-    }
     if (nnz_geo == 0 || ch->n_pairs == 0) return cudaSuccess;
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
@@ -517,13 +499,6 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.n_ab = ch->n_ab;
     sh.n_ll = ch->n_ll; sh.n_trip = ch->n_trip; sh.n_mu = ch->n_mu;
     if ((sh.SP - 4) * sh.IS >= 65536) return cudaErrorInvalidValue;
-    if (upload_consts) {
-        double invk[WPCD_MAX_K + 2];
-        invk[0] = 0.0;
-        for (int k = 1; k < WPCD_MAX_K + 2; ++k) invk[k] = 1.0 / k;
-        err = cudaMemcpyToSymbolAsync(k_invk, invk, sizeof(invk), 0, cudaMemcpyHostToDevice, st);
-        if (err != cudaSuccess) return err;
-    }
     const int mom_warps = MOM_MAX_WARPS;
     const size_t mom_smem = sizeof(double) * ((size_t)((((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + 1) & ~1) + (size_t)mom_warps * moment_smem_doubles(sh));
     size_t ct_smem = 0;
@@ -562,7 +537,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     do {                                                                                                                      \
         err = cudaFuncSetAttribute(moments_kernel<MS, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
         if (err != cudaSuccess) return err;                                                                                   \
-        moments_kernel<MS, SPL><<<blocks, mom_warps * 32, mom_smem, st>>>(g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
+        moments_kernel<MS, SPL><<<blocks, mom_warps * 32, mom_smem, st>>>(qr, g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
                                                                      ws.geo_row, ws.geo_phi, ch->ll_pack_dev,                 \
                                                                      ch->trip_pack_dev, ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);         \
     } while (0)

@@ -51,6 +51,7 @@ struct wpcd_channels {
     int model = 0;
     int n_ch = 0, n_pairs = 0;
     int64_t n_terms = 0;
+    int64_t n_coef = 0;          // (pair, monomial) coefficients: terms of a pair with equal (l1 + l1', k) merged
     bool swave_single = false;   // one channel, one term k=l1=l1'=0, l=l'=0
     double g0 = 0.0;
     std::vector<int32_t> qn;     // [n_ch*6]
@@ -86,6 +87,14 @@ struct wpcd_channels {
 };
 
 namespace wpcd_detail {
+
+// Gauss-Legendre rule of one build, passed BY VALUE to the fill kernels (a __grid_constant__ parameter: every launch
+// carries its own copy in its constant bank, so builds of different orders may overlap in time on one device).
+struct QuadRule {
+    double xi[WPCD_MAX_QUAD];
+    double w[WPCD_MAX_QUAD];
+    double invk[WPCD_MAX_K + 2];   // 1/k for the Legendre recurrence of the coupled fill
+};
 
 void set_error(const std::string& msg);
 extern int64_t g_launches;
@@ -123,9 +132,9 @@ cudaError_t launch_geo_gather(const wpcd_grid* g, const int32_t* geo_row_ptr_dev
                               double2* geo_phi, cudaStream_t st);
 
 // fill.cu
-cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, int rule, const double* xi, const double* w,
+cudaError_t launch_fill_swave(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, int rule, const QuadRule& qr,
                               int64_t nnz_geo, const Workspace& ws, int32_t* col_idx, double* values, cudaStream_t st);
-cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const double* xi, const double* w,
+cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int n_quad, bool split, const QuadRule& qr,
                                 int64_t nnz_geo, const Workspace& ws, const int64_t* row_ptr, const int32_t* geo_row_ptr,
                                 int32_t* col_idx, double* values, cudaStream_t st);
 

@@ -21,6 +21,18 @@ def assign_round_robin(items, rank, world):
     return [it for k, it in enumerate(items) if k % world == rank]
 
 
+def assign_balanced(items, costs, rank, world):
+    """Items dealt largest cost first to the least loaded rank (ties: lowest rank); the items of `rank`, in the order of `items`.
+    Every rank computes the same assignment from the same (items, costs)."""
+    load = [0.0] * world
+    owner = {}
+    for k in sorted(range(len(items)), key=lambda k: (-float(costs[k]), k)):
+        r = min(range(world), key=lambda r: (load[r], r))
+        owner[k] = r
+        load[r] += float(costs[k])
+    return [it for k, it in enumerate(items) if owner[k] == rank]
+
+
 def reduce_step(dist, device, ms_local, units_local):
     """(max over ranks of the step time in ms, sum over ranks of the units processed)."""
     import torch

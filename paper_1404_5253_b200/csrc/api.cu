@@ -134,15 +134,20 @@ Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base)
     ws.geo_phi = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)nnz_geo));
     ws.chunk = 0;
     ws.moments = nullptr;
-    ws.slab_tab = nullptr;
+    ws.elem_rec = nullptr;
+    ws.counters = nullptr;
+    ws.n_chunks = 0;
     if (ch && !ch->swave_single) {
-        ws.slab_tab = take(16 * std::max<size_t>(ch->slabs.size(), 1));
-        // moment block: at most ~256 MiB, a multiple of 32 elements
-        int64_t chunk = (int64_t)((256ull << 20) / (sizeof(double) * (size_t)std::max(ch->n_mu, 1)));
+        ws.elem_rec = reinterpret_cast<int4*>(take(sizeof(int4) * (size_t)nnz_geo));
+        // moment block: at most ~64 MiB (it stays in L2 between the kernel that writes it and the one that reads it), a
+        // multiple of 32 elements
+        int64_t chunk = (int64_t)((64ull << 20) / (sizeof(double) * (size_t)std::max(ch->n_mu, 1)));
         chunk = std::max<int64_t>(32, (chunk / 32) * 32);
         chunk = std::min<int64_t>(chunk, ((nnz_geo + 31) / 32) * 32);
         chunk = std::max<int64_t>(chunk, 32);
         ws.chunk = chunk;
+        ws.n_chunks = (nnz_geo + chunk - 1) / chunk;
+        ws.counters = reinterpret_cast<unsigned int*>(take(sizeof(unsigned int) * (size_t)std::max<int64_t>(ws.n_chunks, 1)));
         ws.moments = reinterpret_cast<double*>(take(sizeof(double) * (size_t)chunk * (size_t)ch->n_mu));
     }
     ws.bytes = off;
@@ -251,88 +256,59 @@ static wpcd_status finalize_channels(wpcd_channels* c)
         for (auto& kv : pair_coef[pidx]) sig.push_back(kv.first);
         class_pairs[ClassKey(l, lp, sig)].push_back(pidx);
     }
-    // ---- slabs: class pieces (split at pair granularity when needed) packed into <= WPCD_SLAB_BYTES blobs
-    c->slabs.clear(); c->slab_blob.clear();
+    // ---- contraction tables: l-groups -> row channels gamma -> items (at most 8 pairs of the group with one l' and one monomial set)
+    c->ct_lgroups.clear(); c->ct_pairs.clear(); c->ct_items.clear(); c->ct_idx.clear(); c->ct_g.clear();
+    c->ct_ncoup_max = 0; c->ct_nmono_max = 0;
     {
-        struct Piece { const ClassKey* key; int m_first, m_count, nm, p_first, p_count, flags; };
-        auto piece_fixed = [](int nm) { return sizeof(wpcd_class_desc) + ((sizeof(int32_t) * nm + 15) & ~(size_t)15); };
-        auto per_pair = [](int nm) { return sizeof(wpcd_pair_meta) + sizeof(double) * nm; };
-        // pieces beyond the first WPCD_MAX_NM monomials of a class accumulate into stored values: they go
-        // to later PASSES (separate launches), so that no accumulation can overtake its store
-        std::vector<std::vector<Piece>> slab_pieces;
-        std::vector<int> slab_pass;
-        size_t max_sig = 0;
-        for (auto& kv : class_pairs) max_sig = std::max(max_sig, std::get<2>(kv.first).size());
-        for (int pass = 0; pass * WPCD_MAX_NM < (int)max_sig || pass == 0; ++pass) {
-            slab_pieces.emplace_back(); slab_pass.push_back(pass);
-            size_t used = sizeof(wpcd_slab_header);
-            for (auto& kv : class_pairs) {
-                const std::vector<Mono>& sig = std::get<2>(kv.first);
-                const int m_first = pass * WPCD_MAX_NM;
-                const int m_count = std::min<int>(WPCD_MAX_NM, (int)sig.size() - m_first);
-                if (m_count <= 0) continue;
-                const int total_p = (int)kv.second.size();
-                int nm = 4 * ((m_count + 3) / 4), p_first = 0;
-                while (p_first < total_p) {
-                    size_t room = WPCD_SLAB_BYTES > used ? WPCD_SLAB_BYTES - used : 0;
-                    int fit = room > piece_fixed(nm) + per_pair(nm) ? (int)((room - piece_fixed(nm)) / per_pair(nm)) : 0;
-                    if (fit == 0) {
-                        if (slab_pieces.back().empty()) return fail(WPCD_ERR_UNSUPPORTED, "a single channel pair does not fit a contraction slab");
-                        slab_pieces.emplace_back(); slab_pass.push_back(pass); used = sizeof(wpcd_slab_header); continue;
+        std::vector<std::vector<int>> pairs_of(c->n_ch);
+        for (int pidx = 0; pidx < c->n_pairs; ++pidx) pairs_of[c->pair_gamma[pidx]].push_back(pidx);
+        std::set<int> ls;
+        for (int a = 0; a < c->n_ch; ++a)
+            if (c->ncoupled[a] > 0) ls.insert(c->channel_l[a]);
+        for (int l : ls) {
+            int mu_lo = INT32_MAX, mu_hi = -1;
+            for (auto& kv : mu_index)
+                if (std::get<0>(kv.first) == l) { mu_lo = std::min(mu_lo, kv.second); mu_hi = std::max(mu_hi, kv.second); }
+            wpcd_ct_lgroup lg = {mu_lo, mu_hi - mu_lo + 1, (int32_t)c->ct_items.size(), 0};
+            c->ct_nmono_max = std::max(c->ct_nmono_max, lg.n_mono);
+            // row channels of the group, and its pairs sorted into classes: (l', exactly the same monomials)
+            std::map<std::pair<int, std::vector<Mono>>, std::vector<int>> groups;
+            for (int ga = 0; ga < c->n_ch; ++ga) {
+                if (c->channel_l[ga] != l || c->ncoupled[ga] == 0) continue;
+                c->ct_ncoup_max = std::max(c->ct_ncoup_max, c->ncoupled[ga]);
+                for (int pidx : pairs_of[ga]) {
+                    std::vector<Mono> sig;
+                    for (auto& kv : pair_coef[pidx]) sig.push_back(kv.first);
+                    groups[std::make_pair(c->channel_l[c->pair_gammap[pidx]], sig)].push_back(pidx);
+                }
+            }
+            // items: at most 8 pairs of one class
+            for (auto& kv : groups) {
+                const int lp = kv.first.first;
+                const std::vector<Mono>& sig = kv.first.second;
+                const int ns = (int)sig.size(), kt = (ns + 3) / 4;
+                for (size_t p_first = 0; p_first < kv.second.size(); p_first += 8) {
+                    const int np = (int)std::min<size_t>(8, kv.second.size() - p_first);
+                    wpcd_ct_item it = {np, kt, (int32_t)c->ct_idx.size(), (int32_t)c->ct_g.size(), (int32_t)c->ct_pairs.size(), 0, 0, 0};
+                    for (int q = 0; q < np; ++q) {
+                        const int pidx = kv.second[p_first + q], ga = c->pair_gamma[pidx];
+                        c->ct_pairs.push_back(make_int4((int)chan_off[ga], c->ncoupled[ga], pair_ci[pidx], c->pair_gammap[pidx]));
                     }
-                    int p_count = std::min(fit, total_p - p_first);
-                    slab_pieces.back().push_back({&kv.first, m_first, m_count, nm, p_first, p_count, pass > 0 ? 1 : 0});
-                    used += piece_fixed(nm) + per_pair(nm) * p_count;
-                    p_first += p_count;
+                    for (int m = 0; m < 4 * kt; ++m) {
+                        const Mono& mo = sig[std::min(m, ns - 1)];
+                        c->ct_idx.push_back(mu_index[std::make_tuple(l, lp, mo.first, mo.second)] - mu_lo);
+                    }
+                    for (int k = 0; k < kt; ++k)            // [k][pair][4]: only the item's own pairs are stored
+                        for (int q = 0; q < np; ++q)
+                            for (int mm = 0; mm < 4; ++mm) {
+                                const int m = 4 * k + mm;
+                                c->ct_g.push_back(m < ns ? pair_coef[kv.second[p_first + q]][sig[m]] : 0.0);
+                            }
+                    c->ct_items.push_back(it);
                 }
             }
-            if (slab_pieces.back().empty()) { slab_pieces.pop_back(); slab_pass.pop_back(); }
-        }
-        size_t slab_no = 0;
-        for (auto& pieces : slab_pieces) {
-            // layout: header | descs | index lists | metas | G
-            size_t off_desc = sizeof(wpcd_slab_header);
-            size_t off_idx = off_desc + sizeof(wpcd_class_desc) * pieces.size();
-            size_t idx_bytes = 0, n_meta = 0, n_g = 0;
-            for (auto& pc : pieces) { idx_bytes += (sizeof(int32_t) * pc.nm + 15) & ~(size_t)15; n_meta += pc.p_count; n_g += (size_t)pc.p_count * pc.nm; }
-            size_t off_meta = off_idx + idx_bytes;
-            size_t off_g = off_meta + sizeof(wpcd_pair_meta) * n_meta;
-            size_t bytes = (off_g + sizeof(double) * n_g + 15) & ~(size_t)15;
-            size_t start = c->slab_blob.size();
-            c->slab_blob.resize(start + bytes, 0);
-            unsigned char* base = c->slab_blob.data() + start;
-            wpcd_slab_header hdr = {(int32_t)pieces.size(), 0, 0, 0};
-            std::memcpy(base, &hdr, sizeof(hdr));
-            size_t cur_idx = off_idx, cur_meta = off_meta, cur_g = off_g;
-            double cost = 0.0;
-            for (size_t pi = 0; pi < pieces.size(); ++pi) {
-                const Piece& pc = pieces[pi];
-                int l = std::get<0>(*pc.key), lp = std::get<1>(*pc.key);
-                const std::vector<Mono>& sig = std::get<2>(*pc.key);
-                wpcd_class_desc d = {(int32_t)cur_idx, pc.nm, pc.p_count, (int32_t)cur_meta, (int32_t)cur_g, pc.flags, 0, 0};
-                std::memcpy(base + off_desc + sizeof(d) * pi, &d, sizeof(d));
-                std::vector<int32_t> idx(pc.nm);
-                for (int m = 0; m < pc.nm; ++m) {
-                    const Mono& mo = sig[pc.m_first + std::min(m, pc.m_count - 1)];   // padding repeats the last one (G = 0 there)
-                    idx[m] = mu_index[std::make_tuple(l, lp, mo.first, mo.second)];
-                }
-                std::memcpy(base + cur_idx, idx.data(), sizeof(int32_t) * pc.nm);
-                cur_idx += (sizeof(int32_t) * pc.nm + 15) & ~(size_t)15;
-                const std::vector<int>& plist = class_pairs[*pc.key];
-                for (int q = 0; q < pc.p_count; ++q) {
-                    int pidx = plist[pc.p_first + q];
-                    int ga = c->pair_gamma[pidx];
-                    wpcd_pair_meta m = {(int32_t)chan_off[ga], c->ncoupled[ga], pair_ci[pidx], c->pair_gammap[pidx]};
-                    std::memcpy(base + cur_meta, &m, sizeof(m));
-                    cur_meta += sizeof(m);
-                    std::vector<double> row(pc.nm, 0.0);
-                    for (int mi = 0; mi < pc.m_count; ++mi) row[mi] = pair_coef[pidx][sig[pc.m_first + mi]];
-                    std::memcpy(base + cur_g, row.data(), sizeof(double) * pc.nm);
-                    cur_g += sizeof(double) * pc.nm;
-                }
-                cost += (double)pc.p_count * (pc.nm + 12) + 2.0 * pc.nm + 20.0;
-            }
-            c->slabs.push_back({start, bytes, (int)pieces.size(), cost, slab_pass[slab_no++]});
+            lg.item_end = (int32_t)c->ct_items.size();
+            c->ct_lgroups.push_back(lg);
         }
     }
     c->swave_single = (c->n_ch == 1 && c->n_pairs == 1 && c->n_terms == 1 && c->channel_l[0] == 0 && c->term_k[0] == 0);
@@ -343,20 +319,24 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return WPCD_OK; }
     // all device tables in ONE allocation and ONE copy (eight separate synchronous copies cost ~55 us per handle)
     auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
-    const size_t sz[8] = {sizeof(int32_t) * c->ncoupled.size(), sizeof(int64_t) * chan_off.size(), sizeof(int32_t) * c->coupled_gp.size(),
-                          sizeof(int32_t) * c->ll_pack.size(),  sizeof(int32_t) * c->trip_pack.size(), sizeof(int32_t) * c->mu_pack.size(),
-                          sizeof(int32_t) * c->ab_pack.size(),  c->slab_blob.size()};
-    const void* src[8] = {c->ncoupled.data(), chan_off.data(), c->coupled_gp.data(), c->ll_pack.data(), c->trip_pack.data(),
-                          c->mu_pack.data(), c->ab_pack.data(), c->slab_blob.data()};
-    size_t off[9];
+    constexpr int NT = 12;
+    const size_t sz[NT] = {sizeof(int32_t) * c->ncoupled.size(), sizeof(int64_t) * chan_off.size(), sizeof(int32_t) * c->coupled_gp.size(),
+                           sizeof(int32_t) * c->ll_pack.size(),  sizeof(int32_t) * c->trip_pack.size(), sizeof(int32_t) * c->mu_pack.size(),
+                           sizeof(int32_t) * c->ab_pack.size(),  sizeof(wpcd_ct_item) * c->ct_items.size(), sizeof(int32_t) * c->ct_idx.size(),
+                           sizeof(double) * c->ct_g.size(),      sizeof(int4) * c->ct_pairs.size(),
+                           sizeof(wpcd_ct_lgroup) * c->ct_lgroups.size()};
+    const void* src[NT] = {c->ncoupled.data(), chan_off.data(), c->coupled_gp.data(), c->ll_pack.data(), c->trip_pack.data(),
+                           c->mu_pack.data(), c->ab_pack.data(), c->ct_items.data(), c->ct_idx.data(), c->ct_g.data(), c->ct_pairs.data(),
+                           c->ct_lgroups.data()};
+    size_t off[NT + 1];
     off[0] = 0;
-    for (int k = 0; k < 8; ++k) off[k + 1] = off[k] + pad(std::max<size_t>(sz[k], 1));
-    std::vector<unsigned char> blob(off[8], 0);
-    for (int k = 0; k < 8; ++k)
+    for (int k = 0; k < NT; ++k) off[k + 1] = off[k] + pad(std::max<size_t>(sz[k], 1));
+    std::vector<unsigned char> blob(off[NT], 0);
+    for (int k = 0; k < NT; ++k)
         if (sz[k]) std::memcpy(blob.data() + off[k], src[k], sz[k]);
     cudaError_t err = cudaSuccess;
-    c->tables_dev = static_cast<unsigned char*>(pool_alloc(off[8], false, &err));
-    if (err == cudaSuccess) err = cudaMemcpy(c->tables_dev, blob.data(), off[8], cudaMemcpyHostToDevice);
+    c->tables_dev = static_cast<unsigned char*>(pool_alloc(off[NT], false, &err));
+    if (err == cudaSuccess) err = cudaMemcpy(c->tables_dev, blob.data(), off[NT], cudaMemcpyHostToDevice);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_channels_create");
     c->ncoupled_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[0]);
     c->chan_off_dev = reinterpret_cast<int64_t*>(c->tables_dev + off[1]);
@@ -365,7 +345,11 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->trip_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[4]);
     c->mu_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[5]);
     c->ab_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[6]);
-    c->slab_blob_dev = c->tables_dev + off[7];
+    c->ct_items_dev = reinterpret_cast<wpcd_ct_item*>(c->tables_dev + off[7]);
+    c->ct_idx_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[8]);
+    c->ct_g_dev = reinterpret_cast<double*>(c->tables_dev + off[9]);
+    c->ct_pairs_dev = reinterpret_cast<int4*>(c->tables_dev + off[10]);
+    c->ct_lgroups_dev = reinterpret_cast<wpcd_ct_lgroup*>(c->tables_dev + off[11]);
     return WPCD_OK;
 }
 

@@ -98,8 +98,8 @@ __device__ __forceinline__ double ipow_small(double b, int e)   // e < 64
     return r;
 }
 
-// Moment layout: [tile of 32 elements][mu][element in tile] (the contraction reads 32 elements of
-// one monomial as one 256-byte line).
+// Moment layout: element-major, moments[element - e_begin][mu] (coalesced stores here; the contraction stages the
+// contiguous range of one l-group per element).
 template <int MAXS, bool SPLIT>
 __global__ void __launch_bounds__(MOM_MAX_WARPS * 32)
 moments_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
@@ -307,11 +307,10 @@ moments_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__
             }
         }
     }
-    const int64_t el = e - e_begin;
-    double* out = moments + ((size_t)(el >> 5) * n_mu) * 32 + (el & 31);
+    double* out = moments + (size_t)(e - e_begin) * n_mu;       // element-major: one contiguous row per element
 #pragma unroll
     for (int s = 0; s < MAXS; ++s)
-        if (lane + 32 * s < n_mu) out[(size_t)(lane + 32 * s) * 32] = acc[s];
+        if (lane + 32 * s < n_mu) out[lane + 32 * s] = acc[s];
 }
 
 }  // namespace
@@ -320,163 +319,114 @@ namespace {
 
 constexpr int CT_THREADS = 256;
 constexpr int CT_WARPS = CT_THREADS / 32;
+constexpr int CT_E = WPCD_CT_ELEMS;
 
-__device__ __forceinline__ uint32_t smem_u32(const void* ptr) { return (uint32_t)__cvta_generic_to_shared(ptr); }
-
-// One slab of classes, global -> shared, as a single TMA bulk copy tracked by an mbarrier.
-__device__ __forceinline__ void slab_to_smem(unsigned char* dst, const unsigned char* src, uint32_t bytes, uint64_t* mbar)
+// (grp, cnt, gcol, row) of every geometric element: what the contraction needs to place its values.
+__global__ void __launch_bounds__(256)
+elem_rec_kernel(int64_t nnz_geo, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
+                const int32_t* __restrict__ geo_row_ptr, int4* __restrict__ rec)
 {
-    if (threadIdx.x == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(bytes) : "memory");
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                     ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(mbar)) : "memory");
-    }
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(mbar)) : "memory");
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nnz_geo) return;
+    const int r = geo_row[e], grp = geo_row_ptr[r];
+    rec[e] = make_int4(grp, geo_row_ptr[r + 1] - grp, geo_col[e], r);
 }
 
-struct TileLane {
-    bool valid;
-    int grp, cnt, pos, gcol;
-    const double* stage;    // this warp's staged class block, [m][32], offset by the lane
-};
-
-// Asynchronous copy (cp.async, 8 bytes per lane and monomial) of one class block of a tile's moment
-// row into the warp's staging buffer: it flies while the previous class is being contracted.
-__device__ __forceinline__ void stage_class(const wpcd_class_desc& d, const unsigned char* slab, const double* mrow_lane,
-                                            double* stage_lane)
+// The same MMA without "volatile": the compiler may interleave independent accumulator chains.
+__device__ __forceinline__ void dmma_884_nv(double& c0, double& c1, double a, double b)
 {
-    const int4* idx = reinterpret_cast<const int4*>(slab + d.idx_off);
-    uint32_t dst = smem_u32(stage_lane);
-    const int quads = d.nm >> 2;
-#pragma unroll 2
-    for (int m = 0; m < quads; ++m, dst += 1024) {
-        const int4 i4 = idx[m];
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(mrow_lane + i4.x * 32) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 256), "l"(mrow_lane + i4.y * 32) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 512), "l"(mrow_lane + i4.z * 32) : "memory");
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 768), "l"(mrow_lane + i4.w * 32) : "memory");
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// All pairs of one class for the 32 elements of a warp tile.  NM = padded monomial count.
-template <int NM>
-__device__ __forceinline__ void contract_class(const wpcd_class_desc& d, const unsigned char* slab, const TileLane& tl,
-                                               const double (&M)[NM], int64_t nnz_geo, int n_geo,
-                                               int32_t* __restrict__ col_idx, double* __restrict__ values)
+// Contraction.  Work unit = (tile of 32 consecutive geometric elements, l-group).  The CTA stages the tile's moments of
+// that l (element-major rows, one contiguous piece per element) in shared memory; its warps then take the group's items,
+// no barrier in between.  Item: D[element][pair] = M[element][monomial] G[pair][monomial] on the FP64 tensor cores -- A
+// fragments from the staged moments, B fragments (coefficient table in fragment order) through L1 -- then the 8 x 32
+// results go through a small per-warp buffer, so that lane = element: a pair's values for the elements of one geometric
+// row are consecutive in CSR row (gamma, r), and a warp store covers the tile's piece of that row (the next tile, handled
+// within microseconds, continues it).
+__global__ void __launch_bounds__(CT_THREADS, 3)
+contract_kernel(int64_t e0, int64_t e1, int64_t nnz_geo, int n_geo, const int4* __restrict__ elem_rec, unsigned int* __restrict__ ticket,
+                const double* __restrict__ moments, int n_mu, const wpcd_ct_lgroup* __restrict__ lgroups, int n_lgroups,
+                const wpcd_ct_item* __restrict__ items, const int32_t* __restrict__ ct_idx, const double* __restrict__ ct_g,
+                const int4* __restrict__ ct_pairs, int ms_stride, int32_t* __restrict__ col_idx, double* __restrict__ values)
 {
-    const bool add = (d.flags & 1) != 0;
-    const int4* meta = reinterpret_cast<const int4*>(slab + d.meta_off);
-    const double2* G = reinterpret_cast<const double2*>(slab + d.g_off);
-    const int n_pairs = d.n_pairs;
-    int pi = 0;
-    for (; pi + 1 < n_pairs; pi += 2) {
-        const double2* g0 = G + (size_t)pi * (NM / 2);
-        const double2* g1 = g0 + NM / 2;
-        double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-#pragma unroll
-        for (int m = 0; m < NM / 2; ++m) {
-            const double2 u = g0[m], v = g1[m];
-            a0 = fma(u.x, M[2 * m], a0); a1 = fma(u.y, M[2 * m + 1], a1);
-            b0 = fma(v.x, M[2 * m], b0); b1 = fma(v.y, M[2 * m + 1], b1);
-        }
-        const int4 ma = meta[pi], mb = meta[pi + 1];
-        if (tl.valid) {
-            const int64_t oa = (int64_t)ma.x * nnz_geo + (int64_t)ma.y * tl.grp + (int64_t)ma.z * tl.cnt + tl.pos;
-            const int64_t ob = (int64_t)mb.x * nnz_geo + (int64_t)mb.y * tl.grp + (int64_t)mb.z * tl.cnt + tl.pos;
-            values[oa] = add ? values[oa] + (a0 + a1) : a0 + a1; col_idx[oa] = ma.w * n_geo + tl.gcol;
-            values[ob] = add ? values[ob] + (b0 + b1) : b0 + b1; col_idx[ob] = mb.w * n_geo + tl.gcol;
-        }
-    }
-    if (pi < n_pairs) {
-        const double2* g0 = G + (size_t)pi * (NM / 2);
-        double a0 = 0.0, a1 = 0.0;
-#pragma unroll
-        for (int m = 0; m < NM / 2; ++m) { const double2 u = g0[m]; a0 = fma(u.x, M[2 * m], a0); a1 = fma(u.y, M[2 * m + 1], a1); }
-        const int4 ma = meta[pi];
-        if (tl.valid) {
-            const int64_t oa = (int64_t)ma.x * nnz_geo + (int64_t)ma.y * tl.grp + (int64_t)ma.z * tl.cnt + tl.pos;
-            values[oa] = add ? values[oa] + (a0 + a1) : a0 + a1; col_idx[oa] = ma.w * n_geo + tl.gcol;
-        }
-    }
-}
-
-// slab_tab[s] = (blob offset, bytes, first CTA, CTA count)
-__global__ void __launch_bounds__(CT_THREADS, 2)
-contract_kernel(int64_t e_begin, int64_t e_end, int64_t nnz_geo, int n_geo, const int32_t* __restrict__ geo_col,
-                const int32_t* __restrict__ geo_row, const int32_t* __restrict__ geo_row_ptr,
-                const double* __restrict__ moments, int n_mu, const unsigned char* __restrict__ slab_blob,
-                const int4* __restrict__ slab_tab, int n_slabs, int stage_off, int32_t* __restrict__ col_idx,
-                double* __restrict__ values)
-{
-    extern __shared__ __align__(128) unsigned char slab[];
-    __shared__ __align__(8) uint64_t mbar;
-    int s = 0;
-    while (s + 1 < n_slabs && (int)blockIdx.x >= slab_tab[s + 1].z) ++s;
-    const int4 st = slab_tab[s];
-    slab_to_smem(slab, slab_blob + st.x, (uint32_t)st.y, &mbar);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_classes = reinterpret_cast<const wpcd_slab_header*>(slab)->n_classes;
-    const wpcd_class_desc* desc = reinterpret_cast<const wpcd_class_desc*>(slab + sizeof(wpcd_slab_header));
-    const int64_t n_tiles = (e_end - e_begin + 31) / 32;
-    const int64_t warps_here = (int64_t)st.w * CT_WARPS;
-    // staging buffers behind the slab: [warp][32 monomials][32 lanes]
-    double* stage_lane = reinterpret_cast<double*>(slab + stage_off) + (size_t)warp * (WPCD_MAX_NM * 32) + lane;
-    int64_t tile = (int64_t)((int)blockIdx.x - st.z) * CT_WARPS + warp;
-    if (tile < n_tiles && n_classes > 0) stage_class(desc[0], slab, moments + (size_t)tile * n_mu * 32 + lane, stage_lane);
-    for (; tile < n_tiles; tile += warps_here) {
-        const int64_t e = e_begin + tile * 32 + lane;
-        TileLane tl;
-        tl.valid = e < e_end;
-        const int64_t ec = tl.valid ? e : e_end - 1;      // idle lanes shadow the last element (loads stay in range)
-        const int r = geo_row[ec];
-        tl.gcol = geo_col[ec];
-        tl.grp = geo_row_ptr[r];
-        tl.cnt = geo_row_ptr[r + 1] - tl.grp;
-        tl.pos = (int)(ec - tl.grp);
-        tl.stage = stage_lane;
-        const double* mrow_lane = moments + (size_t)tile * n_mu * 32 + lane;
-        for (int ci = 0; ci < n_classes; ++ci) {
-            const wpcd_class_desc d = desc[ci];
-            // the block of class ci has been copied to the staging buffer: move it to registers, then let
-            // the copy of the next block (next class, or first class of this warp's next tile) fly
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-            __syncwarp();
-#define WPCD_CT(NMV)                                                                                              \
-    {                                                                                                             \
-        double M[NMV];                                                                                            \
-        _Pragma("unroll") for (int m = 0; m < NMV; ++m) M[m] = stage_lane[m * 32];                                \
-        __syncwarp();                                                                                             \
-        if (ci + 1 < n_classes) stage_class(desc[ci + 1], slab, mrow_lane, stage_lane);                           \
-        else if (tile + warps_here < n_tiles)                                                                     \
-            stage_class(desc[0], slab, moments + (size_t)(tile + warps_here) * n_mu * 32 + lane, stage_lane);      \
-        contract_class<NMV>(d, slab, tl, M, nnz_geo, n_geo, col_idx, values);                                     \
-    }
-            switch (d.nm) {
-            case 4: WPCD_CT(4) break;
-            case 8: WPCD_CT(8) break;
-            case 12: WPCD_CT(12) break;
-            case 16: WPCD_CT(16) break;
-            case 20: WPCD_CT(20) break;
-            case 24: WPCD_CT(24) break;
-            case 28: WPCD_CT(28) break;
-            default: WPCD_CT(32) break;
+    extern __shared__ __align__(16) double ct_sm[];
+    double* Ms = ct_sm;                                                   // [CT_E][ms_stride]
+    double* Sw = Ms + CT_E * ms_stride + (threadIdx.x >> 5) * (8 * 33);   // this warp's [8][33] transposition buffer
+    __shared__ unsigned int s_unit;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quad = lane & 3, oct = lane >> 2;
+    const int64_t n_tiles = (e1 - e0 + CT_E - 1) / CT_E;
+    const uint64_t n_units = (uint64_t)n_tiles * n_lgroups;
+    for (;;) {
+        if (tid == 0) s_unit = atomicAdd(ticket, 1u);
+        __syncthreads();
+        const unsigned int u = s_unit;
+        if (u >= n_units) return;
+        const unsigned int tile = u / n_lgroups;
+        const wpcd_ct_lgroup lg = lgroups[u - tile * n_lgroups];
+        const int64_t es = e0 + (int64_t)tile * CT_E;
+        const int m = (int)min((int64_t)CT_E, e1 - es);
+        // ---- stage the moments of this l for the tile's elements: warp = element row, lanes along the monomials
+        {
+            const double* src = moments + (size_t)(es - e0) * n_mu + lg.mu_lo;
+            for (int ei = warp; ei < m; ei += CT_WARPS) {
+                const double* s = src + (size_t)ei * n_mu;
+                double* d = Ms + ei * ms_stride;
+                for (int mi = lane; mi < lg.n_mono; mi += 32) d[mi] = __ldcs(s + mi);
             }
-#undef WPCD_CT
         }
+        // this lane's element: where its geometric row starts in the pattern, the row's length, its position and column
+        const bool ev = lane < m;
+        const int4 rec = ev ? __ldg(elem_rec + es + lane) : make_int4(0, 0, 0, 0);      // grp, cnt, gcol, row
+        const int pos = (int)(es + lane - rec.x);
+        __syncthreads();
+        const double* r0 = Ms + min(oct, m - 1) * ms_stride;
+        const double* r1 = Ms + min(8 + oct, m - 1) * ms_stride;
+        const double* r2 = Ms + min(16 + oct, m - 1) * ms_stride;
+        const double* r3 = Ms + min(24 + oct, m - 1) * ms_stride;
+        for (int ii = lg.item_begin + warp; ii < lg.item_end; ii += CT_WARPS) {
+            const wpcd_ct_item it = items[ii];
+            const int kt = it.kt, np = it.n_pairs;
+            const int32_t* idx = ct_idx + it.idx_off + quad;
+            const double* gfr = ct_g + it.g_off + lane;        // [k][np][4]: lane (oct, quad) reads entry oct * 4 + quad = lane of step k
+            const bool bl = oct < np;
+            const int gstep = 4 * np;
+            // lane q < np: the record of pair q (prefix of ncoupled over gamma, ncoupled(gamma), rank of gamma', gamma')
+            const int4 pr = lane < np ? __ldg(ct_pairs + it.pair_off + lane) : make_int4(0, 0, 0, 0);
+            const int64_t my_base = (int64_t)pr.x * nnz_geo;
+            const int my_gp = pr.w * n_geo;
+            double c[4][2];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
+#pragma unroll 2
+            for (int k = 0; k < kt; ++k) {
+                const int mi = __ldg(idx + 4 * k);
+                const double b = bl ? __ldg(gfr + gstep * k) : 0.0;
+                dmma_884_nv(c[0][0], c[0][1], r0[mi], b);
+                dmma_884_nv(c[1][0], c[1][1], r1[mi], b);
+                dmma_884_nv(c[2][0], c[2][1], r2[mi], b);
+                dmma_884_nv(c[3][0], c[3][1], r3[mi], b);
+            }
+            // lane holds out[element 8 j + oct][pair 2 quad + h]: transpose through the warp's buffer, row = pair, lane = element
+            __syncwarp();
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) Sw[(2 * quad + h) * 33 + 8 * j + oct] = c[j][h];
+            __syncwarp();
+            for (int q = 0; q < np; ++q) {
+                const int64_t base = __shfl_sync(0xffffffffu, my_base, q);
+                const int ncoup = __shfl_sync(0xffffffffu, pr.y, q), ci = __shfl_sync(0xffffffffu, pr.z, q);
+                const int gp = __shfl_sync(0xffffffffu, my_gp, q);
+                if (ev) {
+                    const int64_t o = base + ((int64_t)ncoup * rec.x + (ci * rec.y + pos));
+                    __stcs(values + o, Sw[q * 33 + lane]);
+                    __stcs(col_idx + o, gp + rec.z);
+                }
+            }
+        }
+        __syncthreads();     // Ms is free again
     }
 }
 
@@ -492,8 +442,8 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if (nnz_geo == 0 || ch->n_pairs == 0) return cudaSuccess;
     if (ch->n_mu > 32 * 32 || 2 * ch->l_max + 2 > 127) return cudaErrorInvalidValue;
     MomentShape sh;
-    static const int g_forced = [] { const char* e = getenv("WPCD_MOM_G"); return e ? atoi(e) : 0; }();   // tuning knob
-    sh.n = n_quad; sh.NS = split ? std::max(n_quad, 4 * SPLIT_MAX_U) : n_quad; sh.G = std::max(1, std::min(32 / n_quad, g_forced > 0 ? g_forced : (n_quad <= 8 ? 4 : 2)));   // measured: n = 8: 4 beats 2 by 13 %, n = 10: 3 loses to 2
+    sh.n = n_quad; sh.NS = split ? std::max(n_quad, 4 * SPLIT_MAX_U) : n_quad;
+    sh.G = std::max(1, std::min(32 / n_quad, n_quad <= 8 ? 4 : 2));   // measured: n = 8: 4 beats 2 by 13 %, n = 10: 3 loses to 2
     sh.K1 = ch->k_max + 1; sh.SP = 8 * ((sh.K1 + 7) / 8) + 4;
     sh.ST = 8 * ((ch->n_ll + 7) / 8) + 4; sh.IS = 8 * ((ch->n_ll + 7) / 8) + 2;
     sh.LM1 = ch->l_max + 1; sh.CP = 2 * ch->l_max + 3; sh.n_ab = ch->n_ab;
@@ -501,36 +451,14 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if ((sh.SP - 4) * sh.IS >= 65536) return cudaErrorInvalidValue;
     const int mom_warps = MOM_MAX_WARPS;
     const size_t mom_smem = sizeof(double) * ((size_t)((((sh.LM1 * sh.LM1 + sh.n_trip + 1) >> 1) + 1) & ~1) + (size_t)mom_warps * moment_smem_doubles(sh));
-    size_t ct_smem = 0;
-    double cost_sum = 0.0;
-    for (auto& sl : ch->slabs) { ct_smem = std::max(ct_smem, sl.bytes); cost_sum += sl.cost; }
-    const int stage_off = (int)((ct_smem + 127) & ~(size_t)127);
-    ct_smem = (size_t)stage_off + sizeof(double) * CT_WARPS * WPCD_MAX_NM * 32;
-    if (ct_smem > 227 * 1024 || mom_smem > 227 * 1024) return cudaErrorInvalidValue;
-    // CTAs per slab in proportion to its cost, two CTAs per SM per pass
+    if (mom_smem > 227 * 1024) return cudaErrorInvalidValue;
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int n_slabs = (int)ch->slabs.size();
-    int n_pass = 0;
-    for (auto& sl : ch->slabs) n_pass = std::max(n_pass, sl.pass + 1);
-    std::vector<int4> tab(n_slabs);
-    std::vector<int> pass_first(n_pass + 1, 0), pass_ctas(n_pass, 0);
-    for (int pass = 0, s = 0; pass < n_pass; ++pass) {       // slabs are stored pass by pass
-        double cost_pass = 0.0;
-        pass_first[pass] = s;
-        for (int t = s; t < n_slabs && ch->slabs[t].pass == pass; ++t) cost_pass += ch->slabs[t].cost;
-        for (; s < n_slabs && ch->slabs[s].pass == pass; ++s) {
-            int cnt = std::max(1, (int)llround(2.0 * sms * ch->slabs[s].cost / std::max(cost_pass, 1.0)));
-            tab[s] = make_int4((int)ch->slabs[s].offset, (int)ch->slabs[s].bytes, pass_ctas[pass], cnt);
-            pass_ctas[pass] += cnt;
-        }
-        pass_first[pass + 1] = s;
-    }
-    (void)cost_sum;
-    int4* tab_dev = reinterpret_cast<int4*>(ws.slab_tab);
-    err = cudaMemcpyAsync(tab_dev, tab.data(), sizeof(int4) * n_slabs, cudaMemcpyHostToDevice, st);
-    if (err != cudaSuccess) return err;
+    // contraction: staged moments [32][ms_stride] + one [8][33] transposition buffer per warp + the run's geometric columns
+    const int ms_stride = ch->ct_nmono_max | 1;                 // odd: the A-fragment rows of a quarter-warp fall into different banks
+    const size_t ct_smem = sizeof(double) * ((size_t)CT_E * ms_stride + (size_t)CT_WARPS * 8 * 33);
+    if (ct_smem > 227 * 1024) return cudaErrorInvalidValue;
     const int n_geo = g->n_p * g->n_q;
     const int maxs = (ch->n_mu + 31) / 32;
 #define WPCD_MOM2(MS, SPL)                                                                                                        \
@@ -544,7 +472,20 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
 #define WPCD_MOM(MS) do { if (split) WPCD_MOM2(MS, true); else WPCD_MOM2(MS, false); } while (0)
     err = cudaFuncSetAttribute(contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem);
     if (err != cudaSuccess) return err;
-    for (int64_t e0 = 0; e0 < nnz_geo; e0 += ws.chunk) {
+    {
+        StageTimer timer(WPCD_STAGE_GEO_INDEX, st);
+        err = cudaMemsetAsync(ws.counters, 0, sizeof(unsigned int) * (size_t)ws.n_chunks, st);
+        if (err != cudaSuccess) return err;
+        elem_rec_kernel<<<(unsigned)((nnz_geo + 255) / 256), 256, 0, st>>>(nnz_geo, ws.geo_col, ws.geo_row, geo_row_ptr, ws.elem_rec);
+        ++g_launches;
+        if ((err = cudaGetLastError()) != cudaSuccess) return err;
+    }
+    int ct_blocks_per_sm = 0;
+    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ct_blocks_per_sm, contract_kernel, CT_THREADS, ct_smem);
+    if (err != cudaSuccess) return err;
+    const unsigned ct_blocks = (unsigned)(sms * std::max(1, ct_blocks_per_sm));
+    int64_t chunk_no = 0;
+    for (int64_t e0 = 0; e0 < nnz_geo; e0 += ws.chunk, ++chunk_no) {
         const int64_t e1 = std::min(nnz_geo, e0 + ws.chunk);
         {
             const unsigned blocks = (unsigned)((e1 - e0 + mom_warps - 1) / mom_warps);
@@ -560,14 +501,12 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         }
         {
             StageTimer timer(WPCD_STAGE_CONTRACT, st);
-            for (int pass = 0; pass < n_pass; ++pass) {
-                contract_kernel<<<pass_ctas[pass], CT_THREADS, ct_smem, st>>>(e0, e1, nnz_geo, n_geo, ws.geo_col, ws.geo_row, geo_row_ptr,
-                                                                              ws.moments, ch->n_mu, ch->slab_blob_dev,
-                                                                              tab_dev + pass_first[pass],
-                                                                              pass_first[pass + 1] - pass_first[pass], stage_off, col_idx, values);
-                ++g_launches;
-                if ((err = cudaGetLastError()) != cudaSuccess) return err;
-            }
+            // persistent CTAs pulling (tile, l-group) units from a work queue
+            contract_kernel<<<ct_blocks, CT_THREADS, ct_smem, st>>>(e0, e1, nnz_geo, n_geo, ws.elem_rec, ws.counters + chunk_no, ws.moments, ch->n_mu,
+                                                                    ch->ct_lgroups_dev, (int)ch->ct_lgroups.size(), ch->ct_items_dev, ch->ct_idx_dev,
+                                                                    ch->ct_g_dev, ch->ct_pairs_dev, ms_stride, col_idx, values);
+            ++g_launches;
+            if ((err = cudaGetLastError()) != cudaSuccess) return err;
         }
     }
 #undef WPCD_MOM

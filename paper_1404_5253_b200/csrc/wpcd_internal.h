@@ -33,19 +33,21 @@ struct wpcd_grid {
 
 // ---- tables of the coupled-channel fill --------------------------
 // The moment row of a geometric element holds, (l, l') block after block, the distinct monomials
-//   mu = (k, A):  P_k(x) cos^{A+1} sin^{l+l'-A+1} / (zeta1^{l'+1} zeta2^{l+1}).
-// A contraction CLASS is a set of channel pairs of one (l, l') that use exactly the same monomials
-// (at most WPCD_MAX_NM per piece): its coefficients form a dense matrix G[pair][monomial], nm =
-// 4 ceil(n/4) columns.  The classes are packed into SLABS (<= WPCD_SLAB_BYTES of shared memory each),
-// one byte blob per slab that the contraction kernel copies to shared memory verbatim:
-//   SlabHeader | ClassDesc[n_classes] | index lists | PairMeta ... | G ...   (every piece 16-byte aligned)
-struct wpcd_slab_header { int32_t n_classes, pad0, pad1, pad2; };
-struct wpcd_class_desc { int32_t idx_off, nm, n_pairs, meta_off, g_off, flags, pad1, pad2; };   // offsets in bytes from the slab start; idx = positions in the moment row; flags bit 0: add to the stored value
-struct wpcd_pair_meta { int32_t chan_off, ncoup, ci, gammap; };   // row-block offset, #coupled of gamma, rank of gamma', gamma'
-constexpr size_t WPCD_SLAB_BYTES = 46 * 1024;   // + 64 KB of staging buffers per CTA: two CTAs per SM
-constexpr int WPCD_MAX_NM = 32;          // monomials per class the register kernel handles
-
-struct wpcd_slab { size_t offset, bytes; int n_classes; double cost; int pass; };
+//   mu = (k, A):  P_k(x) cos^{A+1} sin^{l+l'-A+1} / (zeta1^{l'+1} zeta2^{l+1}),
+// so all monomials of one row-channel momentum l are ONE contiguous range of the row (an "l-group").
+// The contraction value[element][pair] = sum_m M[element][m] G[pair][m] runs on the FP64 tensor cores
+// (mma.sync m8n8k4: 8 elements x 8 pairs x 4 monomials per step).  An ITEM is a set of at most 8 pairs (gamma, gamma')
+// of one l-group with the same l' and exactly the same monomials, its tables in MMA fragment order:
+//   idx   [4 kt]           positions of the item's monomials inside the l-group's range (padding repeats the last one)
+//   g     [kt][n_pairs][4] B fragments: lane (lane/4 < n_pairs) holds G[pair lane/4][monomial 4 k + lane%4]  (0 where padded)
+//   pairs [n_pairs]        (prefix of ncoupled over gamma, ncoupled(gamma), rank of gamma' in the row, gamma')
+// A CTA takes (tile of 32 consecutive geometric elements, l-group), stages the tile's moments of that l in shared
+// memory and deals the group's items to its warps.  The values of a pair for the elements of one geometric row are one
+// run of CSR row (gamma, r) (a row's entries are [gamma' rank][geometric entry]) and leave the warp
+// through a small transposition buffer as coalesced stores.
+struct wpcd_ct_item { int32_t n_pairs, kt, idx_off, g_off, pair_off, pad0, pad1, pad2; };
+struct wpcd_ct_lgroup { int32_t mu_lo, n_mono, item_begin, item_end; };                            // items of all its row channels
+constexpr int WPCD_CT_ELEMS = 32;        // elements of a geometric row per work unit
 
 struct wpcd_channels {
     int model = 0;
@@ -68,9 +70,13 @@ struct wpcd_channels {
     std::vector<int32_t> mu_pack;     // [n_mu]   trip | ab << 16
     std::vector<int32_t> ab_pack;     // [n_ab]   (A+1) | (B+1) << 8       distinct exponent pairs of cos, sin
     int n_ab = 0;
-    // contraction slabs
-    std::vector<wpcd_slab> slabs;
-    std::vector<unsigned char> slab_blob;
+    // contraction tables (host copies; the device copies sit in tables_dev)
+    std::vector<wpcd_ct_lgroup> ct_lgroups;
+    std::vector<int4> ct_pairs;              // per pair of an item: (chan_off, ncoupled, ci, gamma')
+    std::vector<wpcd_ct_item> ct_items;      // row channel after row channel
+    std::vector<int32_t> ct_idx;
+    std::vector<double> ct_g;
+    int ct_ncoup_max = 0, ct_nmono_max = 0;
     // device tables (one allocation, tables_dev; the typed pointers below point into it)
     unsigned char* tables_dev = nullptr;
     int32_t* ncoupled_dev = nullptr;          // [n_ch]   number of gamma' coupled to gamma
@@ -81,7 +87,11 @@ struct wpcd_channels {
     int32_t* trip_pack_dev = nullptr;
     int32_t* mu_pack_dev = nullptr;
     int32_t* ab_pack_dev = nullptr;
-    unsigned char* slab_blob_dev = nullptr;
+    wpcd_ct_lgroup* ct_lgroups_dev = nullptr;
+    int4* ct_pairs_dev = nullptr;
+    wpcd_ct_item* ct_items_dev = nullptr;
+    int32_t* ct_idx_dev = nullptr;
+    double* ct_g_dev = nullptr;
     std::vector<int32_t> ncoupled;
     int64_t total_coupled = 0;
 };
@@ -116,8 +126,10 @@ struct Workspace {
     int32_t* geo_col;    // [nnz_geo]
     int32_t* geo_row;    // [nnz_geo]
     double2* geo_phi;    // [nnz_geo]  (phi_a, phi_b)
-    double* moments;     // [chunk * n_mu] (coupled channels only)
-    void* slab_tab;      // [n_slabs] int4 (coupled channels only)
+    double* moments;     // [(chunk + 32) * n_mu], element-major (coupled channels only)
+    int4* elem_rec;      // [nnz_geo] (first entry of the geometric row, its length, geometric column, row) (coupled channels only)
+    unsigned int* counters;  // [n_chunks]: the work-queue ticket of each chunk's contraction launch
+    int64_t n_chunks;
     int64_t chunk;       // geometric elements per moment chunk
     size_t bytes;
 };

@@ -245,71 +245,80 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->n_ab = (int)c->ab_pack.size();
     if (c->n_ab >= 32768) return fail(WPCD_ERR_UNSUPPORTED, "too many cos/sin exponent pairs");
     c->n_mu = (int)c->mu_pack.size();
-    // ---- contraction classes: pairs of one (l, l') that use exactly the same monomial set (for the nd
-    // tables this separates the (lambda, lambda') values, whose k-ranges differ); a set of more than
-    // WPCD_MAX_NM monomials is cut into pieces, the first stores, the others accumulate
-    typedef std::tuple<int, int, std::vector<Mono>> ClassKey;
-    std::map<ClassKey, std::vector<int>> class_pairs;
-    for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
-        int l = c->channel_l[c->pair_gamma[pidx]], lp = c->channel_l[c->pair_gammap[pidx]];
-        std::vector<Mono> sig;
-        for (auto& kv : pair_coef[pidx]) sig.push_back(kv.first);
-        class_pairs[ClassKey(l, lp, sig)].push_back(pidx);
-    }
-    // ---- contraction tables: l-groups -> row channels gamma -> items (at most 8 pairs of the group with one l' and one monomial set)
-    c->ct_lgroups.clear(); c->ct_pairs.clear(); c->ct_items.clear(); c->ct_idx.clear(); c->ct_g.clear();
-    c->ct_ncoup_max = 0; c->ct_nmono_max = 0;
-    {
-        std::vector<std::vector<int>> pairs_of(c->n_ch);
-        for (int pidx = 0; pidx < c->n_pairs; ++pidx) pairs_of[c->pair_gamma[pidx]].push_back(pidx);
-        std::set<int> ls;
-        for (int a = 0; a < c->n_ch; ++a)
-            if (c->ncoupled[a] > 0) ls.insert(c->channel_l[a]);
-        for (int l : ls) {
-            int mu_lo = INT32_MAX, mu_hi = -1;
-            for (auto& kv : mu_index)
-                if (std::get<0>(kv.first) == l) { mu_lo = std::min(mu_lo, kv.second); mu_hi = std::max(mu_hi, kv.second); }
-            wpcd_ct_lgroup lg = {mu_lo, mu_hi - mu_lo + 1, (int32_t)c->ct_items.size(), 0};
-            c->ct_nmono_max = std::max(c->ct_nmono_max, lg.n_mono);
-            // row channels of the group, and its pairs sorted into classes: (l', exactly the same monomials)
-            std::map<std::pair<int, std::vector<Mono>>, std::vector<int>> groups;
-            for (int ga = 0; ga < c->n_ch; ++ga) {
-                if (c->channel_l[ga] != l || c->ncoupled[ga] == 0) continue;
-                c->ct_ncoup_max = std::max(c->ct_ncoup_max, c->ncoupled[ga]);
-                for (int pidx : pairs_of[ga]) {
-                    std::vector<Mono> sig;
-                    for (auto& kv : pair_coef[pidx]) sig.push_back(kv.first);
-                    groups[std::make_pair(c->channel_l[c->pair_gammap[pidx]], sig)].push_back(pidx);
-                }
-            }
-            // items: at most 8 pairs of one class
-            for (auto& kv : groups) {
-                const int lp = kv.first.first;
-                const std::vector<Mono>& sig = kv.first.second;
-                const int ns = (int)sig.size(), kt = (ns + 3) / 4;
-                for (size_t p_first = 0; p_first < kv.second.size(); p_first += 8) {
-                    const int np = (int)std::min<size_t>(8, kv.second.size() - p_first);
-                    wpcd_ct_item it = {np, kt, (int32_t)c->ct_idx.size(), (int32_t)c->ct_g.size(), (int32_t)c->ct_pairs.size(), 0, 0, 0};
-                    for (int q = 0; q < np; ++q) {
-                        const int pidx = kv.second[p_first + q], ga = c->pair_gamma[pidx];
-                        c->ct_pairs.push_back(make_int4((int)chan_off[ga], c->ncoupled[ga], pair_ci[pidx], c->pair_gammap[pidx]));
-                    }
-                    for (int m = 0; m < 4 * kt; ++m) {
-                        const Mono& mo = sig[std::min(m, ns - 1)];
-                        c->ct_idx.push_back(mu_index[std::make_tuple(l, lp, mo.first, mo.second)] - mu_lo);
-                    }
-                    for (int k = 0; k < kt; ++k)            // [k][pair][4]: only the item's own pairs are stored
-                        for (int q = 0; q < np; ++q)
-                            for (int mm = 0; mm < 4; ++mm) {
-                                const int m = 4 * k + mm;
-                                c->ct_g.push_back(m < ns ? pair_coef[kv.second[p_first + q]][sig[m]] : 0.0);
-                            }
-                    c->ct_items.push_back(it);
-                }
-            }
-            lg.item_end = (int32_t)c->ct_items.size();
-            c->ct_lgroups.push_back(lg);
+    // ---- contraction tables: (l, l') groups -> items (at most 8 pairs of the group with exactly the same monomials: for the nd
+    // tables a class separates the (lambda, lambda') values, whose k-ranges differ);
+    // every group's tables are one blob [items | pairs | idx | g] that the kernel copies to shared memory verbatim
+    c->ct_groups.clear(); c->ct_blob.clear();
+    c->ct_nmono_max = 0; c->ct_blob_max = 0; c->ct_ncoup_max = 0;
+    for (int a = 0; a < c->n_ch; ++a) c->ct_ncoup_max = std::max(c->ct_ncoup_max, c->ncoupled[a]);
+    for (auto& llkv : ll_mono) {       // the monomials of one (l, l') are one contiguous range of the moment row (mu_index is ordered by (l, l'))
+        const int l = llkv.first.first, lp = llkv.first.second;
+        int mu_lo = INT32_MAX, mu_hi = -1;
+        for (auto& ak : llkv.second) {
+            const int mu = mu_index[std::make_tuple(l, lp, ak.first, ak.second)];
+            mu_lo = std::min(mu_lo, mu); mu_hi = std::max(mu_hi, mu);
         }
+        // the group's pairs sorted into classes: exactly the same monomials
+        std::map<std::vector<Mono>, std::vector<int>> classes;
+        for (int pidx = 0; pidx < c->n_pairs; ++pidx) {
+            if (c->channel_l[c->pair_gamma[pidx]] != l || c->channel_l[c->pair_gammap[pidx]] != lp) continue;
+            std::vector<Mono> sig;
+            for (auto& kv : pair_coef[pidx]) sig.push_back(kv.first);
+            classes[sig].push_back(pidx);
+        }
+        std::vector<wpcd_ct_item> items;
+        std::vector<int4> prs;              // per pair: (prefix of ncoupled over gamma, ncoupled(gamma), rank of gamma' in the row, gamma')
+        std::vector<int32_t> idx;
+        std::vector<double> gfr;
+        auto pad16 = [](size_t b) { return (b + 15) & ~(size_t)15; };
+        auto blob_size = [&](size_t ni, size_t npr, size_t nidx, size_t ng) {
+            return pad16(sizeof(wpcd_ct_item) * ni) + pad16(sizeof(int4) * npr) + pad16(sizeof(int32_t) * nidx) + pad16(sizeof(double) * ng);
+        };
+        auto flush = [&]() {             // the items gathered so far become one group
+            if (items.empty()) return;
+            wpcd_ct_group g;
+            g.mu_lo = mu_lo; g.n_mono = mu_hi - mu_lo + 1; g.n_items = (int32_t)items.size();
+            g.blob_off = (int32_t)c->ct_blob.size();
+            g.pairs_off = (int32_t)pad16(sizeof(wpcd_ct_item) * items.size());
+            g.idx_off = g.pairs_off + (int32_t)pad16(sizeof(int4) * prs.size());
+            g.g_off = g.idx_off + (int32_t)pad16(sizeof(int32_t) * idx.size());
+            g.blob_bytes = g.g_off + (int32_t)pad16(sizeof(double) * gfr.size());
+            c->ct_blob.resize(c->ct_blob.size() + g.blob_bytes, 0);
+            unsigned char* base = c->ct_blob.data() + g.blob_off;
+            std::memcpy(base, items.data(), sizeof(wpcd_ct_item) * items.size());
+            std::memcpy(base + g.pairs_off, prs.data(), sizeof(int4) * prs.size());
+            std::memcpy(base + g.idx_off, idx.data(), sizeof(int32_t) * idx.size());
+            std::memcpy(base + g.g_off, gfr.data(), sizeof(double) * gfr.size());
+            c->ct_nmono_max = std::max(c->ct_nmono_max, g.n_mono);
+            c->ct_blob_max = std::max(c->ct_blob_max, g.blob_bytes);
+            c->ct_groups.push_back(g);
+            items.clear(); prs.clear(); idx.clear(); gfr.clear();
+        };
+        for (auto& kv : classes) {
+            const std::vector<Mono>& sig = kv.first;
+            const int ns = (int)sig.size(), kt = (ns + 3) / 4;
+            for (size_t p_first = 0; p_first < kv.second.size(); p_first += 8) {
+                const int np = (int)std::min<size_t>(8, kv.second.size() - p_first);
+                // a group's blob stays below WPCD_CT_BLOB_BYTES (an (l, l') with many pairs becomes several groups)
+                if (blob_size(items.size() + 1, prs.size() + np, idx.size() + 4 * kt, gfr.size() + (size_t)kt * np * 4) > WPCD_CT_BLOB_BYTES) flush();
+                items.push_back({np, kt, (int32_t)idx.size(), (int32_t)gfr.size(), (int32_t)prs.size(), 0, 0, 0});
+                for (int q = 0; q < np; ++q) {
+                    const int pidx = kv.second[p_first + q], ga = c->pair_gamma[pidx];
+                    prs.push_back(make_int4((int)chan_off[ga], c->ncoupled[ga], pair_ci[pidx], c->pair_gammap[pidx]));
+                }
+                for (int m = 0; m < 4 * kt; ++m) {
+                    const Mono& mo = sig[std::min(m, ns - 1)];
+                    idx.push_back(mu_index[std::make_tuple(l, lp, mo.first, mo.second)] - mu_lo);
+                }
+                for (int k = 0; k < kt; ++k)            // [k][pair][4]: only the item's own pairs are stored
+                    for (int q = 0; q < np; ++q)
+                        for (int mm = 0; mm < 4; ++mm) {
+                            const int m = 4 * k + mm;
+                            gfr.push_back(m < ns ? pair_coef[kv.second[p_first + q]][sig[m]] : 0.0);
+                        }
+            }
+        }
+        flush();
     }
     c->swave_single = (c->n_ch == 1 && c->n_pairs == 1 && c->n_terms == 1 && c->channel_l[0] == 0 && c->term_k[0] == 0);
     if (c->swave_single) c->g0 = c->term_g[0];
@@ -319,15 +328,12 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return WPCD_OK; }
     // all device tables in ONE allocation and ONE copy (eight separate synchronous copies cost ~55 us per handle)
     auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
-    constexpr int NT = 12;
+    constexpr int NT = 9;
     const size_t sz[NT] = {sizeof(int32_t) * c->ncoupled.size(), sizeof(int64_t) * chan_off.size(), sizeof(int32_t) * c->coupled_gp.size(),
                            sizeof(int32_t) * c->ll_pack.size(),  sizeof(int32_t) * c->trip_pack.size(), sizeof(int32_t) * c->mu_pack.size(),
-                           sizeof(int32_t) * c->ab_pack.size(),  sizeof(wpcd_ct_item) * c->ct_items.size(), sizeof(int32_t) * c->ct_idx.size(),
-                           sizeof(double) * c->ct_g.size(),      sizeof(int4) * c->ct_pairs.size(),
-                           sizeof(wpcd_ct_lgroup) * c->ct_lgroups.size()};
+                           sizeof(int32_t) * c->ab_pack.size(),  sizeof(wpcd_ct_group) * c->ct_groups.size(), c->ct_blob.size()};
     const void* src[NT] = {c->ncoupled.data(), chan_off.data(), c->coupled_gp.data(), c->ll_pack.data(), c->trip_pack.data(),
-                           c->mu_pack.data(), c->ab_pack.data(), c->ct_items.data(), c->ct_idx.data(), c->ct_g.data(), c->ct_pairs.data(),
-                           c->ct_lgroups.data()};
+                           c->mu_pack.data(), c->ab_pack.data(), c->ct_groups.data(), c->ct_blob.data()};
     size_t off[NT + 1];
     off[0] = 0;
     for (int k = 0; k < NT; ++k) off[k + 1] = off[k] + pad(std::max<size_t>(sz[k], 1));
@@ -345,11 +351,8 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->trip_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[4]);
     c->mu_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[5]);
     c->ab_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[6]);
-    c->ct_items_dev = reinterpret_cast<wpcd_ct_item*>(c->tables_dev + off[7]);
-    c->ct_idx_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[8]);
-    c->ct_g_dev = reinterpret_cast<double*>(c->tables_dev + off[9]);
-    c->ct_pairs_dev = reinterpret_cast<int4*>(c->tables_dev + off[10]);
-    c->ct_lgroups_dev = reinterpret_cast<wpcd_ct_lgroup*>(c->tables_dev + off[11]);
+    c->ct_groups_dev = reinterpret_cast<wpcd_ct_group*>(c->tables_dev + off[7]);
+    c->ct_blob_dev = c->tables_dev + off[8];
     return WPCD_OK;
 }
 

@@ -320,6 +320,7 @@ namespace {
 constexpr int CT_THREADS = 256;
 constexpr int CT_WARPS = CT_THREADS / 32;
 constexpr int CT_E = WPCD_CT_ELEMS;
+constexpr int CT_MAX_TILES = 8;          // 32-element tiles per work unit, at most
 
 // (grp, cnt, gcol, row) of every geometric element: what the contraction needs to place its values.
 __global__ void __launch_bounds__(256)
@@ -338,95 +339,129 @@ __device__ __forceinline__ void dmma_884_nv(double& c0, double& c1, double a, do
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// Contraction.  Work unit = (tile of 32 consecutive geometric elements, l-group).  The CTA stages the tile's moments of
-// that l (element-major rows, one contiguous piece per element) in shared memory; its warps then take the group's items,
-// no barrier in between.  Item: D[element][pair] = M[element][monomial] G[pair][monomial] on the FP64 tensor cores -- A
-// fragments from the staged moments, B fragments (coefficient table in fragment order) through L1 -- then the 8 x 32
-// results go through a small per-warp buffer, so that lane = element: a pair's values for the elements of one geometric
-// row are consecutive in CSR row (gamma, r), and a warp store covers the tile's piece of that row (the next tile, handled
-// within microseconds, continues it).
+// Contraction.  Work unit = ((l, l') group, block of n_tb tiles of 32 consecutive geometric elements).
+// The CTA copies the group's tables (items, pair records, monomial positions, coefficient fragments: one blob) to shared
+// memory, stages the block's moments of that (l, l') range (element-major rows,
+// one contiguous piece per element) and deals (item, tile) pieces to its warps, no barrier in between.  Piece:
+// D[element][pair] = M[element][monomial] G[pair][monomial] on the FP64 tensor cores, every operand from shared memory;
+// then the 8 x 32 results go through a small per-warp buffer so that lane = element: a pair's values for the elements of
+// one geometric row are consecutive in CSR row (gamma, r), and a warp store covers the tile's piece of that row (the
+// neighbouring tile, handled by the same CTA in the same unit or within microseconds, continues it).
 __global__ void __launch_bounds__(CT_THREADS, 3)
 contract_kernel(int64_t e0, int64_t e1, int64_t nnz_geo, int n_geo, const int4* __restrict__ elem_rec, unsigned int* __restrict__ ticket,
-                const double* __restrict__ moments, int n_mu, const wpcd_ct_lgroup* __restrict__ lgroups, int n_lgroups,
-                const wpcd_ct_item* __restrict__ items, const int32_t* __restrict__ ct_idx, const double* __restrict__ ct_g,
-                const int4* __restrict__ ct_pairs, int ms_stride, int32_t* __restrict__ col_idx, double* __restrict__ values)
+                const double* __restrict__ moments, int n_mu, const wpcd_ct_group* __restrict__ groups, int n_groups,
+                const unsigned char* __restrict__ blob, int tab_bytes, int n_tb, int ms_stride, int32_t* __restrict__ col_idx,
+                double* __restrict__ values)
 {
-    extern __shared__ __align__(16) double ct_sm[];
-    double* Ms = ct_sm;                                                   // [CT_E][ms_stride]
-    double* Sw = Ms + CT_E * ms_stride + (threadIdx.x >> 5) * (8 * 33);   // this warp's [8][33] transposition buffer
+    extern __shared__ __align__(16) unsigned char ct_sm[];
+    unsigned char* tab = ct_sm;                                                         // the group's blob
+    double* Ms = reinterpret_cast<double*>(ct_sm + tab_bytes);                          // [n_tb * 32][ms_stride]
+    double* Sw = Ms + (size_t)n_tb * CT_E * ms_stride + (threadIdx.x >> 5) * (8 * 33);  // this warp's [8][33] transposition buffer
+    int4* rec_s = reinterpret_cast<int4*>(Ms + (size_t)n_tb * CT_E * ms_stride + CT_WARPS * 8 * 33);   // [n_tb * 32]
+    __shared__ longlong2 Pw_all[CT_WARPS][8];      // per warp: the current item's pairs, (row-block start, ncoupled << 32 | rank)
+    __shared__ int Gw_all[CT_WARPS][8];            //                                      gamma' * n_geo
+    longlong2* Pw = Pw_all[threadIdx.x >> 5];
+    int* Gw = Gw_all[threadIdx.x >> 5];
     __shared__ unsigned int s_unit;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, quad = lane & 3, oct = lane >> 2;
     const int64_t n_tiles = (e1 - e0 + CT_E - 1) / CT_E;
-    const uint64_t n_units = (uint64_t)n_tiles * n_lgroups;
+    const int64_t n_blocks = (n_tiles + n_tb - 1) / n_tb;
+    const uint64_t n_units = (uint64_t)n_blocks * n_groups;
+    int cur_group = -1;
+    wpcd_ct_group g = {0, 0, 0, 0, 0, 0, 0, 0};
+    unsigned int next_u = 0;                   // thread 0: the ticket drawn one unit ahead (its round trip hides behind the work)
+    if (tid == 0) next_u = atomicAdd(ticket, 1u);
     for (;;) {
-        if (tid == 0) s_unit = atomicAdd(ticket, 1u);
-        __syncthreads();
+        if (tid == 0) s_unit = next_u;
+        __syncthreads();                       // also: every warp is done with the previous unit's shared memory
         const unsigned int u = s_unit;
         if (u >= n_units) return;
-        const unsigned int tile = u / n_lgroups;
-        const wpcd_ct_lgroup lg = lgroups[u - tile * n_lgroups];
-        const int64_t es = e0 + (int64_t)tile * CT_E;
-        const int m = (int)min((int64_t)CT_E, e1 - es);
-        // ---- stage the moments of this l for the tile's elements: warp = element row, lanes along the monomials
-        {
-            const double* src = moments + (size_t)(es - e0) * n_mu + lg.mu_lo;
-            for (int ei = warp; ei < m; ei += CT_WARPS) {
-                const double* s = src + (size_t)ei * n_mu;
-                double* d = Ms + ei * ms_stride;
-                for (int mi = lane; mi < lg.n_mono; mi += 32) d[mi] = __ldcs(s + mi);
-            }
+        if (tid == 0) next_u = atomicAdd(ticket, 1u);
+        // tile block after tile block: all values of a block's elements are written within a short time (the pieces of a CSR
+        // row written by different groups then meet in L2 before they are evicted)
+        const int64_t blk = u / (unsigned)n_groups;
+        const int gi = (int)(u - (uint64_t)blk * n_groups);
+        if (gi != cur_group) {                 // new group: its tables go to shared memory
+            g = groups[gi];
+            cur_group = gi;
+            const uint4* src = reinterpret_cast<const uint4*>(blob + g.blob_off);
+            uint4* dst = reinterpret_cast<uint4*>(tab);
+            for (int i = tid; i < (g.blob_bytes >> 4); i += CT_THREADS)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst + i)), "l"(src + i) : "memory");
         }
-        // this lane's element: where its geometric row starts in the pattern, the row's length, its position and column
-        const bool ev = lane < m;
-        const int4 rec = ev ? __ldg(elem_rec + es + lane) : make_int4(0, 0, 0, 0);      // grp, cnt, gcol, row
-        const int pos = (int)(es + lane - rec.x);
+        const int64_t es = e0 + blk * n_tb * CT_E;
+        const int rows = (int)min((int64_t)n_tb * CT_E, e1 - es);
+        // ---- stage the moments of this (l, l') for the block's elements: warp = element row, lanes along the monomials
+        {
+            const double* src = moments + (size_t)(es - e0) * n_mu + g.mu_lo;
+            // asynchronous copies (8 bytes each: a row starts on an 8-byte boundary only), all in flight together
+            for (int ei = warp; ei < rows; ei += CT_WARPS) {
+                const double* s = src + (size_t)ei * n_mu;
+                const uint32_t d = (uint32_t)__cvta_generic_to_shared(Ms + ei * ms_stride);
+                for (int mi = lane; mi < g.n_mono; mi += 32)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + 8 * mi), "l"(s + mi) : "memory");
+            }
+            for (int i = tid; i < rows; i += CT_THREADS) rec_s[i] = __ldg(elem_rec + es + i);       // grp, cnt, gcol, row
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
         __syncthreads();
-        const double* r0 = Ms + min(oct, m - 1) * ms_stride;
-        const double* r1 = Ms + min(8 + oct, m - 1) * ms_stride;
-        const double* r2 = Ms + min(16 + oct, m - 1) * ms_stride;
-        const double* r3 = Ms + min(24 + oct, m - 1) * ms_stride;
-        for (int ii = lg.item_begin + warp; ii < lg.item_end; ii += CT_WARPS) {
+        const wpcd_ct_item* items = reinterpret_cast<const wpcd_ct_item*>(tab);
+        const int4* prs = reinterpret_cast<const int4*>(tab + g.pairs_off);
+        const int32_t* idx_s = reinterpret_cast<const int32_t*>(tab + g.idx_off);
+        const double* g_s = reinterpret_cast<const double*>(tab + g.g_off);
+        const int n_t = (rows + CT_E - 1) / CT_E;
+        const int n_pieces = g.n_items * n_t;
+        int ii = warp / n_t, t = warp - ii * n_t;               // piece = (item ii, tile t), item-major, dealt round-robin to the warps
+        for (int pc = warp; pc < n_pieces; pc += CT_WARPS) {
             const wpcd_ct_item it = items[ii];
             const int kt = it.kt, np = it.n_pairs;
-            const int32_t* idx = ct_idx + it.idx_off + quad;
-            const double* gfr = ct_g + it.g_off + lane;        // [k][np][4]: lane (oct, quad) reads entry oct * 4 + quad = lane of step k
+            // lane q < np: (prefix of ncoupled over gamma, ncoupled(gamma), rank of gamma', gamma') of pair q -> where the pair's
+            // values start in the CSR (entry 0 of row (gamma, 0) + rank * 0), its row-block factor, rank and column offset
+            if (lane < np) {
+                const int4 pr = prs[it.pair_off + lane];
+                Pw[lane] = make_longlong2((long long)pr.x * nnz_geo, ((long long)(unsigned)pr.y << 32) | (unsigned)pr.z);
+                Gw[lane] = pr.w * n_geo;
+            }
+            const int ib = it.idx_off + quad, gb = it.g_off + lane;     // [k][np][4]: lane (oct, quad) reads entry oct * 4 + quad = lane of step k
             const bool bl = oct < np;
             const int gstep = 4 * np;
-            // lane q < np: the record of pair q (prefix of ncoupled over gamma, ncoupled(gamma), rank of gamma', gamma')
-            const int4 pr = lane < np ? __ldg(ct_pairs + it.pair_off + lane) : make_int4(0, 0, 0, 0);
-            const int64_t my_base = (int64_t)pr.x * nnz_geo;
-            const int my_gp = pr.w * n_geo;
+            const int m = min(CT_E, rows - t * CT_E);
+            const int o0 = (t * CT_E + min(oct, m - 1)) * ms_stride, o1 = (t * CT_E + min(8 + oct, m - 1)) * ms_stride;
+            const int o2 = (t * CT_E + min(16 + oct, m - 1)) * ms_stride, o3 = (t * CT_E + min(24 + oct, m - 1)) * ms_stride;
             double c[4][2];
 #pragma unroll
             for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
 #pragma unroll 2
             for (int k = 0; k < kt; ++k) {
-                const int mi = __ldg(idx + 4 * k);
-                const double b = bl ? __ldg(gfr + gstep * k) : 0.0;
-                dmma_884_nv(c[0][0], c[0][1], r0[mi], b);
-                dmma_884_nv(c[1][0], c[1][1], r1[mi], b);
-                dmma_884_nv(c[2][0], c[2][1], r2[mi], b);
-                dmma_884_nv(c[3][0], c[3][1], r3[mi], b);
+                const int mi = idx_s[ib + 4 * k];
+                const double b = bl ? g_s[gb + gstep * k] : 0.0;
+                dmma_884_nv(c[0][0], c[0][1], Ms[o0 + mi], b);
+                dmma_884_nv(c[1][0], c[1][1], Ms[o1 + mi], b);
+                dmma_884_nv(c[2][0], c[2][1], Ms[o2 + mi], b);
+                dmma_884_nv(c[3][0], c[3][1], Ms[o3 + mi], b);
             }
             // lane holds out[element 8 j + oct][pair 2 quad + h]: transpose through the warp's buffer, row = pair, lane = element
-            __syncwarp();
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) Sw[(2 * quad + h) * 33 + 8 * j + oct] = c[j][h];
             __syncwarp();
-            for (int q = 0; q < np; ++q) {
-                const int64_t base = __shfl_sync(0xffffffffu, my_base, q);
-                const int ncoup = __shfl_sync(0xffffffffu, pr.y, q), ci = __shfl_sync(0xffffffffu, pr.z, q);
-                const int gp = __shfl_sync(0xffffffffu, my_gp, q);
-                if (ev) {
-                    const int64_t o = base + ((int64_t)ncoup * rec.x + (ci * rec.y + pos));
+            if (lane < m) {
+                const int4 rec = rec_s[t * CT_E + lane];            // this lane's element: grp, cnt, gcol, row
+                const int pos = (int)(es - rec.x) + t * CT_E + lane;
+                for (int q = 0; q < np; ++q) {
+                    const longlong2 pq = Pw[q];                     // (start of the pair's row block, ncoupled << 32 | rank)
+                    const int ncoup = (int)(pq.y >> 32), ci = (int)(unsigned)pq.y;
+                    const int64_t o = pq.x + (ncoup * rec.x + ci * rec.y + pos);       // < 2^31 inside a row block (checked by the host)
                     __stcs(values + o, Sw[q * 33 + lane]);
-                    __stcs(col_idx + o, gp + rec.z);
+                    __stcs(col_idx + o, Gw[q] + rec.z);
                 }
             }
+            __syncwarp();
+            t += CT_WARPS;
+            while (t >= n_t) { t -= n_t; ++ii; }
         }
-        __syncthreads();     // Ms is free again
     }
 }
 
@@ -455,10 +490,19 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    // contraction: staged moments [32][ms_stride] + one [8][33] transposition buffer per warp + the run's geometric columns
+    // contraction: the largest group blob + staged moments [n_tb * 32][ms_stride] + one [8][33] transposition buffer per warp
+    // + the block's element records.  n_tb: as many tiles per unit as leave room for three CTAs per SM (at least one).
     const int ms_stride = ch->ct_nmono_max | 1;                 // odd: the A-fragment rows of a quarter-warp fall into different banks
-    const size_t ct_smem = sizeof(double) * ((size_t)CT_E * ms_stride + (size_t)CT_WARPS * 8 * 33);
+    const int tab_bytes = (ch->ct_blob_max + 15) & ~15;
+    auto ct_bytes = [&](int n_tb) {
+        return (size_t)tab_bytes + sizeof(double) * ((size_t)n_tb * CT_E * ms_stride + (size_t)CT_WARPS * 8 * 33) + sizeof(int4) * (size_t)n_tb * CT_E;
+    };
+    int n_tb = CT_MAX_TILES;
+    while (n_tb > 1 && ct_bytes(n_tb) > (size_t)70 * 1024) --n_tb;
+    const size_t ct_smem = ct_bytes(n_tb);
     if (ct_smem > 227 * 1024) return cudaErrorInvalidValue;
+    // the contraction places a value with a 32-bit offset inside the row block of its channel
+    if ((int64_t)ch->ct_ncoup_max * nnz_geo + nnz_geo >= (int64_t)INT32_MAX) return cudaErrorInvalidValue;
     const int n_geo = g->n_p * g->n_q;
     const int maxs = (ch->n_mu + 31) / 32;
 #define WPCD_MOM2(MS, SPL)                                                                                                        \
@@ -501,10 +545,10 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         }
         {
             StageTimer timer(WPCD_STAGE_CONTRACT, st);
-            // persistent CTAs pulling (tile, l-group) units from a work queue
+            // persistent CTAs pulling (group, tile block) units from a work queue
             contract_kernel<<<ct_blocks, CT_THREADS, ct_smem, st>>>(e0, e1, nnz_geo, n_geo, ws.elem_rec, ws.counters + chunk_no, ws.moments, ch->n_mu,
-                                                                    ch->ct_lgroups_dev, (int)ch->ct_lgroups.size(), ch->ct_items_dev, ch->ct_idx_dev,
-                                                                    ch->ct_g_dev, ch->ct_pairs_dev, ms_stride, col_idx, values);
+                                                                    ch->ct_groups_dev, (int)ch->ct_groups.size(), ch->ct_blob_dev, tab_bytes, n_tb,
+                                                                    ms_stride, col_idx, values);
             ++g_launches;
             if ((err = cudaGetLastError()) != cudaSuccess) return err;
         }

@@ -41,12 +41,16 @@ struct wpcd_grid {
 //   idx   [4 kt]           positions of the item's monomials inside the l-group's range (padding repeats the last one)
 //   g     [kt][n_pairs][4] B fragments: lane (lane/4 < n_pairs) holds G[pair lane/4][monomial 4 k + lane%4]  (0 where padded)
 //   pairs [n_pairs]        (prefix of ncoupled over gamma, ncoupled(gamma), rank of gamma' in the row, gamma')
-// A CTA takes (tile of 32 consecutive geometric elements, l-group), stages the tile's moments of that l in shared
-// memory and deals the group's items to its warps.  The values of a pair for the elements of one geometric row are one
-// run of CSR row (gamma, r) (a row's entries are [gamma' rank][geometric entry]) and leave the warp
-// through a small transposition buffer as coalesced stores.
-struct wpcd_ct_item { int32_t n_pairs, kt, idx_off, g_off, pair_off, pad0, pad1, pad2; };
-struct wpcd_ct_lgroup { int32_t mu_lo, n_mono, item_begin, item_end; };                            // items of all its row channels
+// The pairs are grouped by (l, l') -- the monomials of one (l, l') are ONE contiguous range of the moment row -- and all
+// tables of a group form one blob [items | pairs | idx | g] (16-byte aligned pieces, offsets inside the blob) that the
+// contraction kernel copies to shared memory verbatim.  A CTA takes (group, block of a few 32-element tiles of consecutive
+// geometric elements), stages that range of the tiles' moments in shared memory and deals (item, tile) pieces to its
+// warps.  The values of a pair for the elements of one geometric row are one run of CSR row (gamma, r) (DESIGN.md
+// section 6: a row's entries are [gamma' rank][geometric entry]) and leave the warp through a small transposition
+// buffer as coalesced stores.
+struct wpcd_ct_item { int32_t n_pairs, kt, idx_off, g_off, pair_off, pad0, pad1, pad2; };     // offsets: elements of the group's arrays
+struct wpcd_ct_group { int32_t mu_lo, n_mono, n_items, blob_off, blob_bytes, pairs_off, idx_off, g_off; };   // byte offsets; items at 0
+constexpr size_t WPCD_CT_BLOB_BYTES = 16 * 1024;   // tables of one group (a single item may exceed it: then the group is that item)
 constexpr int WPCD_CT_ELEMS = 32;        // elements of a geometric row per work unit
 
 struct wpcd_channels {
@@ -71,12 +75,10 @@ struct wpcd_channels {
     std::vector<int32_t> ab_pack;     // [n_ab]   (A+1) | (B+1) << 8       distinct exponent pairs of cos, sin
     int n_ab = 0;
     // contraction tables (host copies; the device copies sit in tables_dev)
-    std::vector<wpcd_ct_lgroup> ct_lgroups;
-    std::vector<int4> ct_pairs;              // per pair of an item: (chan_off, ncoupled, ci, gamma')
-    std::vector<wpcd_ct_item> ct_items;      // row channel after row channel
-    std::vector<int32_t> ct_idx;
-    std::vector<double> ct_g;
-    int ct_ncoup_max = 0, ct_nmono_max = 0;
+    std::vector<wpcd_ct_group> ct_groups;
+    std::vector<unsigned char> ct_blob;      // group after group
+    int ct_nmono_max = 0, ct_blob_max = 0;   // largest monomial range / blob of a group
+    int ct_ncoup_max = 0;                    // largest number of coupled channels of a row
     // device tables (one allocation, tables_dev; the typed pointers below point into it)
     unsigned char* tables_dev = nullptr;
     int32_t* ncoupled_dev = nullptr;          // [n_ch]   number of gamma' coupled to gamma
@@ -87,11 +89,8 @@ struct wpcd_channels {
     int32_t* trip_pack_dev = nullptr;
     int32_t* mu_pack_dev = nullptr;
     int32_t* ab_pack_dev = nullptr;
-    wpcd_ct_lgroup* ct_lgroups_dev = nullptr;
-    int4* ct_pairs_dev = nullptr;
-    wpcd_ct_item* ct_items_dev = nullptr;
-    int32_t* ct_idx_dev = nullptr;
-    double* ct_g_dev = nullptr;
+    wpcd_ct_group* ct_groups_dev = nullptr;
+    unsigned char* ct_blob_dev = nullptr;
     std::vector<int32_t> ncoupled;
     int64_t total_coupled = 0;
 };

@@ -182,13 +182,16 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
                                         const double* values_dev, const double* x_dev, double* y_dev, int n_inter,
                                         void* cuda_stream);
 
-/* y = P0 x for a matrix built by wpcd_perm_build on (grid, channels), using its block structure: row (gamma,i,j)
- * holds, for every gamma' coupled to gamma, the same geometric columns shifted by gamma' * n_p * n_q, so only the
- * first block's column indices of each row are read: the matrix streams at 8 bytes per nonzero instead of the 12
- * of the general CSR product (the SpMV is HBM-bound).  row_ptr_dev, geo_row_ptr_dev as written
- * by wpcd_perm_count, col_idx_dev / values_dev by wpcd_perm_build, for THESE handles (not checked); x_dev, y_dev
- * [n_vec][rows], dev.  Each row is summed by one warp in a fixed order (deterministic; agrees with wpcd_perm_apply to
- * rounding).  Asynchronous; the first apply on arrays not built through this library synchronises the stream once. */
+/* y = P0 x for a matrix built by wpcd_perm_build on (grid, channels), using its block structure: P0 = (channel coupling
+ * mask) x (geometric pattern), i.e. row (gamma,i,j) holds, for every gamma' coupled to gamma, the same geometric columns
+ * shifted by gamma' * n_p * n_q.  One CTA per geometric row (i,j) gathers the values of x at those columns for all
+ * channels into shared memory once, and the n_channels rows of that (i,j) then stream only their VALUES: 8 bytes per
+ * nonzero from HBM instead of the 12 of the general CSR product, and one gather per (channel, geometric entry) instead of
+ * one per nonzero (the SpMV is HBM-bound).  Up to 4 vectors share one pass over the matrix.
+ * geo_row_ptr_dev as written by wpcd_perm_count, col_idx_dev / values_dev by wpcd_perm_build, for THESE handles (not
+ * checked; row_ptr_dev is not read); x_dev, y_dev [n_vec][rows], dev, x_dev must not alias y_dev.  Each row is summed in a
+ * fixed order (deterministic; agrees with wpcd_perm_apply to rounding).  Asynchronous.  At most 64 such products in
+ * flight per device at a time (the work-queue counters are a ring). */
 wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* grid, const wpcd_channels* channels, const int64_t* row_ptr_dev,
                                     const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
                                     const double* x_dev, double* y_dev, int n_vec, void* cuda_stream);
@@ -270,6 +273,16 @@ wpcd_status wpcd_trace_read(double* ms_out, int64_t* launches_out);
 
 /* Number of kernels the library has launched from this process (bench.py's gpu_launches). */
 int64_t wpcd_launch_count(void);
+
+/* Test and diagnosis switches (process-wide; the library reads no environment variable).  value 0 restores the
+ * library's own choice.  Keys:
+ *   "spmv_lanes_per_row"    4 / 8 / 16 / 32: force that lanes-per-row variant of wpcd_perm_apply
+ *   "spmv_no_pipeline"      1: never take the software-pipelined long-row variant
+ *   "no_pdl"                1: launch the products without programmatic dependent launch
+ *   "chain_mode"            1: wpcd_perm_apply_chain fuses whenever the matrix fits on chip, 2: never fuses
+ *   "blocked_tile_doubles"  > 0: size of the x tile of wpcd_perm_apply_blocked (small values exercise its chunked paths)
+ * WPCD_ERR_INVALID_ARG for an unknown key. */
+wpcd_status wpcd_debug_set(const char* key, int64_t value);
 
 #ifdef __cplusplus
 }

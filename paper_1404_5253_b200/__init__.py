@@ -33,7 +33,7 @@ EXPORTS = [
     "wpcd_channels_terms", "wpcd_channels_monomials", "wpcd_channels_coefficients", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
     "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
-    "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read",
+    "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read", "wpcd_debug_set",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
 
@@ -94,6 +94,7 @@ def load():
     L.wpcd_launch_count.restype = i64
     L.wpcd_trace_enable.argtypes = [i32]
     L.wpcd_trace_read.argtypes = [vp, vp]
+    L.wpcd_debug_set.argtypes = [ctypes.c_char_p, i64]
     _lib = L
     return L
 
@@ -372,6 +373,11 @@ def wpcd_trace_read():
     n = np.zeros(len(TRACE_STAGES), np.int64)
     _check(load().wpcd_trace_read(ms.ctypes.data, n.ctypes.data))
     return {name: (float(ms[i]), int(n[i])) for i, name in enumerate(TRACE_STAGES)}
+
+
+def wpcd_debug_set(key, value):
+    """Test / diagnosis switch of the library (keys: include/wpcd.h); value 0 restores the library's own choice."""
+    _check(load().wpcd_debug_set(key.encode(), int(value)))
 
 
 def wpcd_launch_count():

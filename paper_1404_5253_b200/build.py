@@ -9,7 +9,7 @@ LIB = os.path.join(HERE, "libwpcd.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 # pattern.cu holds the IEEE-contract predicate: no FMA contraction there
-UNITS = [("pattern.cu", ["-fmad=false"]), ("fill.cu", []), ("fill_coupled.cu", []), ("spmv.cu", []), ("spmv_chain.cu", []), ("kernel_apply.cu", []), ("api.cu", [])]
+UNITS = [("pattern.cu", ["-fmad=false"]), ("fill.cu", []), ("fill_coupled.cu", []), ("spmv.cu", []), ("spmv_blocked.cu", []), ("spmv_chain.cu", []), ("kernel_apply.cu", []), ("api.cu", [])]
 
 
 def _stale(target, sources):

@@ -16,7 +16,8 @@
 namespace wpcd_detail {
 
 static thread_local std::string t_error;
-int64_t g_launches = 0;
+std::atomic<int64_t> g_launches{0};
+DebugSwitches g_debug;
 
 void set_error(const std::string& msg) { t_error = msg; }
 
@@ -217,6 +218,18 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->total_coupled = chan_off[c->n_ch];
     c->coupled_gp.assign(c->n_pairs, 0);      // gamma' of block t of channel gamma, at chan_off[gamma] + t
     for (int pidx = 0; pidx < c->n_pairs; ++pidx) c->coupled_gp[chan_off[c->pair_gamma[pidx]] + pair_ci[pidx]] = c->pair_gammap[pidx];
+    c->run_ptr.assign(1, 0); c->runs.clear(); c->first_gamma = -1;
+    for (int a = 0; a < c->n_ch; ++a) {
+        for (int t = 0; t < c->ncoupled[a];) {
+            const int g0 = c->coupled_gp[chan_off[a] + t];
+            int len = 1;
+            while (t + len < c->ncoupled[a] && c->coupled_gp[chan_off[a] + t + len] == g0 + len) ++len;
+            c->runs.push_back(make_int4(t, g0, len, 0));
+            t += len;
+        }
+        c->run_ptr.push_back((int32_t)c->runs.size());
+        if (c->first_gamma < 0 && c->ncoupled[a] > 0) { c->first_gamma = a; c->first_gp = c->coupled_gp[chan_off[a]]; }
+    }
     // ---- moment row: one block per (l, l') with its distinct monomials; (l,l') list; (k,l,l') triples
     std::map<std::pair<int, int>, int> ll_index;
     c->ll_pack.clear();
@@ -328,12 +341,14 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return WPCD_OK; }
     // all device tables in ONE allocation and ONE copy (eight separate synchronous copies cost ~55 us per handle)
     auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
-    constexpr int NT = 9;
+    constexpr int NT = 11;
     const size_t sz[NT] = {sizeof(int32_t) * c->ncoupled.size(), sizeof(int64_t) * chan_off.size(), sizeof(int32_t) * c->coupled_gp.size(),
                            sizeof(int32_t) * c->ll_pack.size(),  sizeof(int32_t) * c->trip_pack.size(), sizeof(int32_t) * c->mu_pack.size(),
-                           sizeof(int32_t) * c->ab_pack.size(),  sizeof(wpcd_ct_group) * c->ct_groups.size(), c->ct_blob.size()};
+                           sizeof(int32_t) * c->ab_pack.size(),  sizeof(wpcd_ct_group) * c->ct_groups.size(), c->ct_blob.size(),
+                           sizeof(int32_t) * c->run_ptr.size(),  sizeof(int4) * c->runs.size()};
     const void* src[NT] = {c->ncoupled.data(), chan_off.data(), c->coupled_gp.data(), c->ll_pack.data(), c->trip_pack.data(),
-                           c->mu_pack.data(), c->ab_pack.data(), c->ct_groups.data(), c->ct_blob.data()};
+                           c->mu_pack.data(), c->ab_pack.data(), c->ct_groups.data(), c->ct_blob.data(), c->run_ptr.data(),
+                           c->runs.data()};
     size_t off[NT + 1];
     off[0] = 0;
     for (int k = 0; k < NT; ++k) off[k + 1] = off[k] + pad(std::max<size_t>(sz[k], 1));
@@ -353,6 +368,8 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->ab_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[6]);
     c->ct_groups_dev = reinterpret_cast<wpcd_ct_group*>(c->tables_dev + off[7]);
     c->ct_blob_dev = c->tables_dev + off[8];
+    c->run_ptr_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[9]);
+    c->runs_dev = reinterpret_cast<int4*>(c->tables_dev + off[10]);
     return WPCD_OK;
 }
 
@@ -728,12 +745,10 @@ wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* g, const wpcd_channels* c, 
     const int64_t rows = wpcd_rows(g, c);
     if (rows == 0 || n_vec == 0) return WPCD_OK;
     if (!row_ptr_dev || !geo_row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null pointer");
+    if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_apply_blocked: channel tables are not on a device (no CUDA device?)");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int n_geo = g->n_p * g->n_q;
-    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
-    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null matrix arrays");
-    cudaError_t err = launch_spmv_blocked(rows, n_geo, c->chan_off_dev, c->coupled_gp_dev, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev,
-                                          x_dev, y_dev, n_vec, st);
+    if (c->total_coupled > 0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked: null matrix arrays");
+    cudaError_t err = launch_spmv_blocked(g, c, geo_row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_blocked");
     return WPCD_OK;
 }
@@ -962,6 +977,19 @@ wpcd_status wpcd_trace_read(double* ms_out, int64_t* launches_out)
     return WPCD_OK;
 }
 
-int64_t wpcd_launch_count(void) { return g_launches; }
+int64_t wpcd_launch_count(void) { return g_launches.load(); }
+
+wpcd_status wpcd_debug_set(const char* key, int64_t value)
+{
+    if (!key) return fail(WPCD_ERR_INVALID_ARG, "wpcd_debug_set: null key");
+    const std::string k(key);
+    if (k == "spmv_lanes_per_row") g_debug.spmv_lanes_per_row = (int)value;
+    else if (k == "spmv_no_pipeline") g_debug.spmv_no_pipeline = (int)value;
+    else if (k == "no_pdl") g_debug.no_pdl = (int)value;
+    else if (k == "chain_mode") g_debug.chain_mode = (int)value;
+    else if (k == "blocked_tile_doubles") g_debug.blocked_tile_doubles = (int)value;
+    else return fail(WPCD_ERR_INVALID_ARG, "wpcd_debug_set: unknown key " + k);
+    return WPCD_OK;
+}
 
 }  // extern "C"

@@ -120,7 +120,7 @@ template <int NV>
 cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
                      double* y, double mean_row, cudaStream_t st)
 {
-    static const int forced = [] { const char* e = getenv("WPCD_SPMV_LPR"); return e ? atoi(e) : 0; }();   // tuning knob
+    const int forced = wpcd_detail::g_debug.spmv_lanes_per_row.load();
     if (forced == 4) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
     if (forced == 8) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
     if (forced == 16) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
@@ -130,8 +130,7 @@ cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_id
     if (mean_row <= 3.0) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
     if (mean_row <= 6.0) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
     if (mean_row <= 12.0) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    static const int pipe = [] { const char* e = getenv("WPCD_SPMV_PIPE"); return e ? atoi(e) : 1; }();   // tuning knob
-    if (pipe && mean_row >= 128.0) return launch<32, NV, true>(rows, row_ptr, col_idx, values, x, y, st);
+    if (!wpcd_detail::g_debug.spmv_no_pipeline.load() && mean_row >= 128.0) return launch<32, NV, true>(rows, row_ptr, col_idx, values, x, y, st);
     return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
 }
 
@@ -256,97 +255,6 @@ cudaError_t dispatch_interleaved(int64_t rows, const int64_t* row_ptr, const int
     return launch_interleaved<32, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
 }
 
-// ---------------------------------------------------------------- blocked product (coupled channels)
-// Row (gamma, i, j) of P0 holds, for every gamma' coupled to gamma, the SAME cnt(i,j) geometric columns shifted by
-// gamma' n_geo: entry idx of the row is block t = idx / cnt, geometric entry
-// s = idx % cnt, column geo_col[s] + gamma'_t n_geo.  One warp per row stages the cnt geometric columns (the first
-// block's col_idx) and the row's gamma' offsets in shared memory once, then streams ONLY the values: 8 bytes per
-// nonzero from HBM instead of 12.  Batches of BL_UNR x 32 consecutive entries, the next batch's values in flight
-// while the current one gathers (as the pipelined CSR kernel).
-constexpr int BL_UNR = 8;
-constexpr int BL_CAPG = 512;     // geometric entries of a row kept in shared memory (longer rows: indices re-read through L1)
-constexpr int BL_CAPC = 64;      // coupled channels of a row kept in shared memory
-
-__global__ void __launch_bounds__(256)
-spmv_blocked_kernel(int64_t rows, int n_geo, const int64_t* __restrict__ chan_off, const int32_t* __restrict__ coupled_gp,
-                    const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ geo_row_ptr,
-                    const int32_t* __restrict__ col_idx, const double* __restrict__ values, const double* __restrict__ x,
-                    double* __restrict__ y, int stage_rows)
-{
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    __shared__ int s_geo_all[8][BL_CAPG];
-    __shared__ int s_off_all[8][BL_CAPC];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int* s_geo = s_geo_all[warp];
-    int* s_off = s_off_all[warp];
-    const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (r >= rows) return;
-    const int gamma = (int)(r / n_geo), ij = (int)(r - (int64_t)gamma * n_geo);
-    // independent loads first, then the first batch of values, so that the stream starts while the tables are staged
-    const int64_t beg = row_ptr[r], end = row_ptr[r + 1];
-    const int cnt = geo_row_ptr[ij + 1] - geo_row_ptr[ij];
-    const int64_t co = chan_off[gamma];
-    double acc = 0.0;
-    if (cnt > 0 && end > beg) {
-        const int len = (int)(end - beg);
-        const double* vrow = values + beg;
-        double a[BL_UNR], a2[BL_UNR];
-#pragma unroll
-        for (int k = 0; k < BL_UNR; ++k) {
-            const int idx = k * 32 + lane;
-            a[k] = idx < len ? __ldcs(vrow + idx) : 0.0;
-        }
-        const int nc = len / cnt;
-        const bool staged = cnt <= BL_CAPG && nc <= BL_CAPC && stage_rows;
-        // gamma'_t n_geo of the row's blocks; lane 0's value is gamma'_0 n_geo
-        int off_first = 0;
-        for (int t = lane; t < nc; t += 32) {
-            const int o = __ldg(coupled_gp + co + t) * n_geo;
-            if (t == lane) off_first = o;
-            if (staged) s_off[t] = o;
-        }
-        const int gp0 = __shfl_sync(0xffffffffu, off_first, 0);
-        if (staged)
-            for (int s = lane; s < cnt; s += 32) s_geo[s] = __ldg(col_idx + beg + s) - gp0;      // geometric column
-        __syncwarp();
-        // (t, s) = (idx / cnt, idx % cnt) of this lane's next entry, advanced by 32 entries at a time without a division
-        const int q32 = 32 / cnt, r32 = 32 - q32 * cnt;
-        int t = lane / cnt, sg = lane - t * cnt;
-        if (staged) {
-            // two batches per trip, the registers of one batch refilled while the other gathers
-            auto batch = [&](double (&cur)[BL_UNR], double (&nxt)[BL_UNR], int i0) {
-#pragma unroll
-                for (int k = 0; k < BL_UNR; ++k) {
-                    const int idx = i0 + (BL_UNR + k) * 32 + lane;
-                    nxt[k] = idx < len ? __ldcs(vrow + idx) : 0.0;
-                }
-#pragma unroll
-                for (int k = 0; k < BL_UNR; ++k) {
-                    const int idx = i0 + k * 32 + lane;
-                    if (idx < len) acc = fma(cur[k], __ldg(x + (s_geo[sg] + s_off[t])), acc);
-                    sg += r32; t += q32;
-                    if (sg >= cnt) { sg -= cnt; ++t; }
-                }
-            };
-            for (int i0 = 0; i0 < len; i0 += 2 * BL_UNR * 32) {
-                batch(a, a2, i0);
-                batch(a2, a, i0 + BL_UNR * 32);
-            }
-        } else {
-            // a row with more geometric entries or coupled channels than the staging area holds: indices through L1
-            for (int idx = lane; idx < len; idx += 32) {
-                const int tt = idx / cnt, ss = idx - tt * cnt;
-                const int c = __ldg(col_idx + beg + ss) - gp0 + __ldg(coupled_gp + co + tt) * n_geo;
-                acc = fma(__ldcs(vrow + idx), __ldg(x + c), acc);
-            }
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) y[r] = acc;
-}
-
 // ---------------------------------------------------------------- FP64 FMA peak
 __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double seed)
 {
@@ -366,8 +274,7 @@ namespace wpcd_detail {
 
 bool use_pdl()
 {
-    static const bool on = [] { const char* e = getenv("WPCD_NO_PDL"); return !(e && e[0] == '1'); }();
-    return on;
+    return g_debug.no_pdl.load() == 0;
 }
 
 cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
@@ -395,30 +302,6 @@ cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const 
         double2* yv = reinterpret_cast<double2*>(y) + (int64_t)v * rows * (n_inter / 2);
         cudaError_t err = n_inter == 4 ? dispatch_interleaved<4>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st)
                                        : dispatch_interleaved<2>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st);
-        if (err != cudaSuccess) return err;
-    }
-    return cudaSuccess;
-}
-
-cudaError_t launch_spmv_blocked(int64_t rows, int n_geo, const int64_t* chan_off, const int32_t* coupled_gp, const int64_t* row_ptr,
-                                const int32_t* geo_row_ptr, const int32_t* col_idx, const double* values, const double* x, double* y,
-                                int n_vec, cudaStream_t st)
-{
-    static const int stage_rows = [] { const char* e = getenv("WPCD_SPMV_BLOCKED_UNSTAGED"); return (e && e[0] == '1') ? 0 : 1; }();   // test knob
-    for (int v = 0; v < n_vec; ++v) {
-        const int64_t blocks = (rows * 32 + 255) / 256;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)blocks);
-        cfg.blockDim = dim3(256);
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = use_pdl() ? 1 : 0;
-        ++g_launches;
-        cudaError_t err = cudaLaunchKernelEx(&cfg, spmv_blocked_kernel, rows, n_geo, chan_off, coupled_gp, row_ptr, geo_row_ptr, col_idx,
-                                             values, x + (int64_t)v * rows, y + (int64_t)v * rows, stage_rows);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;

@@ -260,8 +260,8 @@ cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_
                               const double* x, double* y, int n_iter, double mean_row, cudaStream_t st, int* fused)
 {
     *fused = 0;
-    static const bool off = [] { const char* e = getenv("WPCD_NO_CHAIN"); return e && e[0] == '1'; }();
-    if (off || n_iter < 2 || rows >= (int64_t)1 << 30) return cudaSuccess;
+    const int mode = g_debug.chain_mode.load();
+    if (mode == 2 || n_iter < 2 || rows >= (int64_t)1 << 30) return cudaSuccess;
     int dev = 0;
     cudaError_t err = cudaGetDevice(&dev);
     if (err != cudaSuccess) return err;
@@ -280,8 +280,7 @@ cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_
     const int64_t want_rows = std::min<int64_t>(2 * (rows / d.sms) + 256, 65535);
     const int64_t want_slots = want_entries / 2 + want_rows + 64;
     if (want_entries * 12 + (want_rows + 1) * 8 + want_slots * 4 > smem_budget) return cudaSuccess;
-    static const bool force = [] { const char* e = getenv("WPCD_FORCE_CHAIN"); return e && e[0] == '1'; }();
-    if (!force && (nnz < 16000 || nnz > 160000)) return cudaSuccess;      // the measured window (file header)
+    if (mode != 1 && (nnz < 16000 || nnz > 160000)) return cudaSuccess;      // the measured window (file header)
     const int cap_entries = (int)((want_entries + 1) & ~(int64_t)1), cap_rows = (int)want_rows, cap_slots = (int)want_slots;
     const size_t smem = (size_t)cap_entries * 12 + (size_t)(cap_rows + 1) * 8 + (size_t)cap_slots * 4;
     if (!d.counters) {

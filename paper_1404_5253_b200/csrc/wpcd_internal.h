@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -93,6 +94,12 @@ struct wpcd_channels {
     unsigned char* ct_blob_dev = nullptr;
     std::vector<int32_t> ncoupled;
     int64_t total_coupled = 0;
+    // blocked product: the gamma' coupled to gamma as runs of consecutive channels, (rank of the first, first gamma', length)
+    std::vector<int32_t> run_ptr;             // [n_ch + 1]
+    std::vector<int4> runs;
+    int32_t* run_ptr_dev = nullptr;
+    int4* runs_dev = nullptr;
+    int first_gamma = -1, first_gp = 0;       // the first channel that has entries, and the first gamma' coupled to it
 };
 
 namespace wpcd_detail {
@@ -106,7 +113,17 @@ struct QuadRule {
 };
 
 void set_error(const std::string& msg);
-extern int64_t g_launches;
+extern std::atomic<int64_t> g_launches;
+
+// Test / diagnosis switches behind wpcd_debug_set (include/wpcd.h); 0 = the library's own choice.
+struct DebugSwitches {
+    std::atomic<int> spmv_lanes_per_row{0};      // 4 / 8 / 16 / 32: force the lanes-per-row variant of the CSR product
+    std::atomic<int> spmv_no_pipeline{0};        // 1: never take the software-pipelined long-row variant
+    std::atomic<int> no_pdl{0};                  // 1: launch the products without programmatic dependent launch
+    std::atomic<int> chain_mode{0};              // 1: fused chain whenever the matrix fits on chip, 2: never
+    std::atomic<int> blocked_tile_doubles{0};    // > 0: size of the blocked product's x tile (small values exercise the chunked paths)
+};
+extern DebugSwitches g_debug;
 
 // RAII stage timer (wpcd_trace_enable): records an event pair around a kernel launch.
 struct StageTimer {
@@ -154,9 +171,9 @@ cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col
                         const double* x, double* y, int n_vec, double mean_row, cudaStream_t st);
 cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                                     const double* x, double* y, int n_vec, int n_inter, double mean_row, cudaStream_t st);
-cudaError_t launch_spmv_blocked(int64_t rows, int n_geo, const int64_t* chan_off, const int32_t* coupled_gp, const int64_t* row_ptr,
-                                const int32_t* geo_row_ptr, const int32_t* col_idx, const double* values, const double* x, double* y,
-                                int n_vec, cudaStream_t st);
+// spmv_blocked.cu
+cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
+                                const double* values, const double* x, double* y, int n_vec, cudaStream_t st);
 cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                               const double* x, double* y, int n_iter, double mean_row, cudaStream_t st, int* fused);
 cudaError_t run_fp64_peak(cudaStream_t st, double* flops_out);

@@ -714,23 +714,30 @@ def test_apply_blocked(wpcd):
             assert np.all(np.abs(yh[k] - ref) <= 1e-12 * scale + 1e-300), (gch.count, len(p), k)
 
 
-@pytest.mark.parametrize("knobs", [{"WPCD_SPMV_BLOCKED_UNSTAGED": "1"}])
-def test_apply_blocked_other_paths(knobs):
-    """The same cases through the path for rows too long for the shared-memory staging area (the knob is read once per
-    process, hence the child process)."""
-    import os
-    import subprocess
-    import sys
-
-    if os.environ.get("WPCD_BLOCKED_CHILD") == "1":
-        pytest.skip("already inside the forced run")
-    env = dict(os.environ, WPCD_BLOCKED_CHILD="1", **knobs)
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-m", "gpu", "-x", "-q",
-                        "-k", "test_apply_blocked and not other_paths", "-p", "no:cacheprovider"],
-                       env=env, cwd=root, capture_output=True, text=True, timeout=600)
-    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
-    assert "1 passed" in r.stdout
+def test_apply_blocked_chunked_paths(wpcd):
+    """The same product with a tiny x tile (wpcd_debug_set): geometric rows cut into column chunks, channels into channel
+    chunks, runs of coupled channels split at chunk boundaries; 1, 2, 3 and 5 vectors per call."""
+    torch = _torch()
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=1, two_T=1, j_pair_max=2)
+    p, q = wi.tan2_grid(9, 1.0, 0.1, seed=41), wi.tan2_grid(11, 0.8, 0.1, seed=42)
+    grid = wpcd.wpcd_grid_create(p, q)
+    m = wpcd.build_perm(grid, gch, 4)
+    rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
+    try:
+        for tile in (0, 7, 40, 256):
+            wpcd.wpcd_debug_set("blocked_tile_doubles", tile)
+            for n_vec in (1, 2, 3, 5):
+                xs = np.stack([wi.normal_vector(m.rows, k=820 + k) for k in range(n_vec)])
+                x = torch.from_numpy(xs).cuda()
+                y = torch.full_like(x, np.nan)
+                wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y, n_vec=n_vec)
+                yh = y.cpu().numpy()
+                for k in range(n_vec):
+                    ref = operm.spmv(rp, ci, v, xs[k])
+                    scale = operm.spmv(rp, ci, np.abs(v), np.abs(xs[k]))
+                    assert np.all(np.abs(yh[k] - ref) <= 1e-12 * scale + 1e-300), (tile, n_vec, k)
+    finally:
+        wpcd.wpcd_debug_set("blocked_tile_doubles", 0)
 
 
 def _chain_check(wpcd, torch, rows, rp, ci, v, rpd, cid, vd, n_iter, tag):
@@ -775,22 +782,32 @@ def test_apply_chain(wpcd):
                      n_iter, tag)
 
 
-def test_apply_chain_fused_everywhere():
-    """The same chain cases with the fused cooperative launch forced on for every matrix that fits on chip
-    (WPCD_FORCE_CHAIN=1 is read once per process, hence the child process)."""
-    import os
-    import subprocess
-    import sys
+def test_apply_chain_fused_everywhere(wpcd):
+    """The same chain cases with the fused cooperative launch forced on for every matrix that fits on chip, and forced off."""
+    try:
+        for mode in (1, 2):
+            wpcd.wpcd_debug_set("chain_mode", mode)
+            test_apply_chain(wpcd)
+    finally:
+        wpcd.wpcd_debug_set("chain_mode", 0)
 
-    if os.environ.get("WPCD_FORCE_CHAIN") == "1":
-        pytest.skip("already inside the forced run")
-    env = dict(os.environ, WPCD_FORCE_CHAIN="1")
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-m", "gpu", "-x", "-q",
-                        "-k", "test_apply_chain and not fused_everywhere", "-p", "no:cacheprovider"],
-                       env=env, cwd=root, capture_output=True, text=True, timeout=600)
-    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
-    assert "1 passed" in r.stdout
+
+def test_apply_forced_variants(wpcd):
+    """Every lanes-per-row variant of the CSR product on the same matrices (wpcd_debug_set), with and without the pipelined
+    long-row path and programmatic dependent launch."""
+    try:
+        for lanes in (4, 8, 16, 32):
+            wpcd.wpcd_debug_set("spmv_lanes_per_row", lanes)
+            test_apply_multi_vector_and_host(wpcd)
+        wpcd.wpcd_debug_set("spmv_lanes_per_row", 0)
+        wpcd.wpcd_debug_set("spmv_no_pipeline", 1)
+        wpcd.wpcd_debug_set("no_pdl", 1)
+        test_apply_long_rows_pipelined(wpcd)
+        with pytest.raises(wpcd.WpcdError, match="unknown key"):
+            wpcd.wpcd_debug_set("no_such_switch", 1)
+    finally:
+        for key in ("spmv_lanes_per_row", "spmv_no_pipeline", "no_pdl"):
+            wpcd.wpcd_debug_set(key, 0)
 
 
 def test_block_apply_and_kernel_apply(wpcd):

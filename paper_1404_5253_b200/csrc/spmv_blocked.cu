@@ -17,17 +17,17 @@
 
 namespace {
 
-constexpr int GB_THREADS = 256;
-constexpr int GB_WARPS = GB_THREADS / 32;
-constexpr int GB_UNR = 8;            // 32-entry batches of one segment whose value loads are issued together
+template <int NV> struct GbUnroll { static constexpr int value = NV >= 4 ? 4 : 8; };   // 32-entry batches of one segment whose value loads are issued together
 constexpr int GB_RING = 64;          // work-queue slots (concurrent launches)
 
 __device__ unsigned int g_queue[GB_RING][2];     // (next geometric row, CTAs done); the last CTA of a launch resets its slot
 
-// acc[v] += sum_i V[i] X[i * NV + v], i = 0 .. len-1, lanes strided; loads of GB_UNR batches in flight together
+// acc[v] += sum_i V[i] X[v * xs + i], i = 0 .. len-1, lanes strided; the value loads of GB_UNR batches in flight together
+// (one plane of X per vector: consecutive lanes read consecutive doubles, no bank conflicts)
 template <int NV>
-__device__ __forceinline__ void segment_dot(const double* __restrict__ V, const double* __restrict__ X, int len, int lane, double (&acc)[NV])
+__device__ __forceinline__ void segment_dot(const double* __restrict__ V, const double* __restrict__ X, int xs, int len, int lane, double (&acc)[NV])
 {
+    constexpr int GB_UNR = GbUnroll<NV>::value;
     for (int i0 = lane; i0 < len; i0 += 32 * GB_UNR) {
         double a[GB_UNR];
 #pragma unroll
@@ -37,14 +37,48 @@ __device__ __forceinline__ void segment_dot(const double* __restrict__ V, const 
             const int i = i0 + 32 * k;
             if (i < len) {
 #pragma unroll
-                for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], X[(size_t)i * NV + v], acc[v]);
+                for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], X[v * xs + i], acc[v]);
             }
         }
     }
 }
 
-// x, y: NV vectors, vector-major (x[v * ldx + column]).  cap: doubles of the X tile per vector.
+// The same with a software pipeline (the next batch's values are requested before this batch is multiplied): pays for two
+// vectors (4.8 against 5.7 ms on the 3.2e9-nonzero matrix), costs registers and CTAs per SM for one.
 template <int NV>
+__device__ __forceinline__ void segment_dot_pipelined(const double* __restrict__ V, const double* __restrict__ X, int xs, int len, int lane,
+                                                      double (&acc)[NV])
+{
+    constexpr int GB_UNR = GbUnroll<NV>::value;
+    double a[GB_UNR], a2[GB_UNR];
+#pragma unroll
+    for (int k = 0; k < GB_UNR; ++k) a[k] = lane + 32 * k < len ? __ldcs(V + lane + 32 * k) : 0.0;
+    for (int i0 = lane; i0 < len; i0 += 32 * GB_UNR) {
+        const int n0 = i0 + 32 * GB_UNR;
+#pragma unroll
+        for (int k = 0; k < GB_UNR; ++k) a2[k] = n0 + 32 * k < len ? __ldcs(V + n0 + 32 * k) : 0.0;
+#pragma unroll
+        for (int k = 0; k < GB_UNR; ++k) {
+            const int i = i0 + 32 * k;
+            if (i < len) {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], X[v * xs + i], acc[v]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < GB_UNR; ++k) a[k] = a2[k];
+    }
+}
+
+template <int NV>
+__device__ __forceinline__ void segment(const double* __restrict__ V, const double* __restrict__ X, int xs, int len, int lane, double (&acc)[NV])
+{
+    if (NV == 2) segment_dot_pipelined<NV>(V, X, xs, len, lane, acc);
+    else segment_dot<NV>(V, X, xs, len, lane, acc);
+}
+
+// x, y: NV vectors, vector-major (x[v * ldx + column]).  cap: doubles of the X tile per vector.
+template <int NV, int GB_THREADS>
 __global__ void __launch_bounds__(GB_THREADS)
 spmv_georow_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row_ptr, const int32_t* __restrict__ col_idx,
                    const double* __restrict__ values, const int64_t* __restrict__ chan_off, const int32_t* __restrict__ ncoupled,
@@ -52,10 +86,11 @@ spmv_georow_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row_ptr,
                    const double* __restrict__ x, double* __restrict__ y, int64_t ldx, int cap, int slot)
 {
     extern __shared__ __align__(16) double gb_sm[];
-    double* X = gb_sm;                                         // [channels of the chunk][cs][NV]
+    double* X = gb_sm;                                         // [NV][channels of the chunk][cs]
     double* ysum = X + (size_t)cap * NV;                       // [n_ch][NV]
     int32_t* gcol = reinterpret_cast<int32_t*>(ysum + (size_t)n_ch * NV);      // [cs]
     __shared__ unsigned int s_row;
+    constexpr int GB_WARPS = GB_THREADS / 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t nnz_geo = geo_row_ptr[n_geo];
     for (;;) {
@@ -82,7 +117,7 @@ spmv_georow_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row_ptr,
                         const int gg = i / cs, s = i - gg * cs;
                         const double* xp = x + (int64_t)(glo + gg) * n_geo + gcol[s];
 #pragma unroll
-                        for (int v = 0; v < NV; ++v) X[(size_t)i * NV + v] = __ldg(xp + v * ldx);
+                        for (int v = 0; v < NV; ++v) X[v * cap + i] = __ldg(xp + v * ldx);
                     }
                     __syncthreads();
                     for (int ga = warp; ga < n_ch; ga += GB_WARPS) {
@@ -100,10 +135,10 @@ spmv_georow_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row_ptr,
                             any = true;
                             const int t0 = run.x + (a0 - run.y);
                             if (cs == cnt) {
-                                segment_dot<NV>(vrow + (int64_t)t0 * cnt, X + (size_t)(a0 - glo) * cs * NV, (a1 - a0) * cnt, lane, acc);
+                                segment<NV>(vrow + (int64_t)t0 * cnt, X + (a0 - glo) * cs, cap, (a1 - a0) * cnt, lane, acc);
                             } else {
                                 for (int j = 0; j < a1 - a0; ++j)
-                                    segment_dot<NV>(vrow + (int64_t)(t0 + j) * cnt + s0, X + (size_t)(a0 - glo + j) * cs * NV, cs, lane, acc);
+                                    segment<NV>(vrow + (int64_t)(t0 + j) * cnt + s0, X + (a0 - glo + j) * cs, cap, cs, lane, acc);
                             }
                         }
                         if (!any) continue;
@@ -144,7 +179,12 @@ namespace wpcd_detail {
 
 bool use_pdl();
 
-template <int NV>
+// One vector: 256 threads and an x tile of 1536 doubles (measured on a B200, N = 150, 26 - 62 channels: 1280 - 1792
+// doubles stream the values at the HBM copy rate; from 2048 on fewer CTAs fit an SM and the rate drops by a quarter).
+// Several vectors: the tile holds NV planes; it is kept large enough for a whole average geometric row (3072 doubles
+// per vector), because every (channel chunk, row) costs a warp reduction per vector, and the CTA grows to 512 / 1024
+// threads so that the SM still has 32 - 64 warps streaming.
+template <int NV, int THREADS>
 static cudaError_t launch_georow(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
                                  const double* values, const double* x, double* y, int64_t ldx, cudaStream_t st)
 {
@@ -153,20 +193,21 @@ static cudaError_t launch_georow(const wpcd_grid* g, const wpcd_channels* ch, co
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    // X tile: 4096 doubles per vector (a geometric row of up to 4096 / n_ch entries is one chunk; N = 150: mean 39, max ~600)
     const int forced = g_debug.blocked_tile_doubles.load();
-    const int cap = forced > 0 ? forced : std::max(4096 / NV, 64);
+    const int cap = forced > 0 ? forced : (NV == 1 ? 1536 : 3072);        // doubles per vector
     const size_t smem = sizeof(double) * ((size_t)cap * NV + (size_t)ch->n_ch * NV) + sizeof(int32_t) * (size_t)cap;
-    cudaError_t err = cudaFuncSetAttribute(spmv_georow_kernel<NV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    cudaError_t err = cudaFuncSetAttribute(spmv_georow_kernel<NV, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     int per_sm = 0;
-    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spmv_georow_kernel<NV>, GB_THREADS, smem);
+    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spmv_georow_kernel<NV, THREADS>, THREADS, smem);
     if (err != cudaSuccess) return err;
     const int blocks = std::max(1, std::min(n_geo, sms * std::max(1, per_sm)));
     const int slot = (int)(next_slot.fetch_add(1) % GB_RING);
     ++g_launches;
-    spmv_georow_kernel<NV><<<blocks, GB_THREADS, smem, st>>>(n_geo, ch->n_ch, geo_row_ptr, col_idx, values, ch->chan_off_dev, ch->ncoupled_dev,
-                                                            ch->run_ptr_dev, ch->runs_dev, ch->first_gamma, ch->first_gp, x, y, ldx, cap, slot);
+    spmv_georow_kernel<NV, THREADS><<<blocks, THREADS, smem, st>>>(n_geo, ch->n_ch, geo_row_ptr, col_idx, values, ch->chan_off_dev,
+                                                                  ch->ncoupled_dev, ch->run_ptr_dev, ch->runs_dev, ch->first_gamma, ch->first_gp,
+                                                                  x, y, ldx, cap, slot);
     return cudaGetLastError();
 }
 
@@ -179,9 +220,10 @@ cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, con
         const double* xv = x + (int64_t)v * rows;
         double* yv = y + (int64_t)v * rows;
         cudaError_t err;
-        if (n_vec - v >= 4) { err = launch_georow<4>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 4; }
-        else if (n_vec - v >= 2) { err = launch_georow<2>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 2; }
-        else { err = launch_georow<1>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 1; }
+        if (n_vec - v >= 8) { err = launch_georow<8, 1024>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 8; }
+        else if (n_vec - v >= 4) { err = launch_georow<4, 1024>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 4; }
+        else if (n_vec - v >= 2) { err = launch_georow<2, 512>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 2; }
+        else { err = launch_georow<1, 256>(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, st); v += 1; }
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;

@@ -726,7 +726,7 @@ def test_apply_blocked_chunked_paths(wpcd):
     try:
         for tile in (0, 7, 40, 256):
             wpcd.wpcd_debug_set("blocked_tile_doubles", tile)
-            for n_vec in (1, 2, 3, 5):
+            for n_vec in (1, 2, 3, 5, 9, 15):
                 xs = np.stack([wi.normal_vector(m.rows, k=820 + k) for k in range(n_vec)])
                 x = torch.from_numpy(xs).cuda()
                 y = torch.full_like(x, np.nan)

@@ -280,8 +280,9 @@ def run_ours(args):
             # one call, the library shares each pass over the matrix among 4 of them
             wpcd.wpcd_perm_apply(job.rows, job.row_ptr, job.col_idx, job.values, job.x_all, job.y_all, n_vec=n_spmv)
             return
+        # coupled channels: the product through the block structure of P0 (same CSR arrays, values streamed only: 8 B per nonzero)
         for k in range(n_spmv):
-            wpcd.wpcd_perm_apply(job.rows, job.row_ptr, job.col_idx, job.values, job.x[k % job.n_x], job.y)
+            wpcd.wpcd_perm_apply_blocked(grid, job.channels, job.row_ptr, job.geo_row_ptr, job.col_idx, job.values, job.x[k % job.n_x], job.y)
 
     def sweep_passes(job):
         """[right-hand sides per launch] of one sweep (mirrors the library: passes of 4, then 2, then 1)."""
@@ -427,17 +428,33 @@ def run_ours(args):
         msi = a.elapsed_time(b) / reps
         spmm["interleaved4_ms_per_pass"] = msi
         spmm["interleaved4_matrix_GBps"] = (12.0 * job.nnz + 8.0 * job.rows) / (msi * 1e-3) / 1e9
-        # the product through the block structure of P0 (8 bytes per nonzero instead of 12)
-        for _ in range(2):
-            wpcd.wpcd_perm_apply_blocked(grid, job.channels, job.row_ptr, job.geo_row_ptr, job.col_idx, job.values, x4, y4, n_vec=1)
-        a.record()
-        for _ in range(reps):
-            wpcd.wpcd_perm_apply_blocked(grid, job.channels, job.row_ptr, job.geo_row_ptr, job.col_idx, job.values, x4, y4, n_vec=1)
-        b.record()
-        torch.cuda.synchronize()
-        msb = a.elapsed_time(b) / reps
-        spmm["blocked_ms_per_product"] = msb
-        spmm["blocked_matrix_GBps"] = (8.0 * job.nnz + 16.0 * job.rows) / (msb * 1e-3) / 1e9
+        # the general CSR product (12 B per nonzero) and the product through the block structure of P0 (8 B per nonzero), one vector
+        for name, fn in (("csr", lambda: wpcd.wpcd_perm_apply(job.rows, job.row_ptr, job.col_idx, job.values, x4[0], y4[0])),
+                         ("blocked", lambda: wpcd.wpcd_perm_apply_blocked(grid, job.channels, job.row_ptr, job.geo_row_ptr, job.col_idx,
+                                                                          job.values, x4, y4, n_vec=1))):
+            for _ in range(2):
+                fn()
+            a.record()
+            for _ in range(reps):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            spmm[name + "_ms_per_product"] = a.elapsed_time(b) / reps
+        spmm["csr_matrix_GBps"] = (12.0 * job.nnz + 24.0 * job.rows) / (spmm["csr_ms_per_product"] * 1e-3) / 1e9
+        spmm["blocked_matrix_GBps"] = (8.0 * job.nnz + 16.0 * job.rows) / (spmm["blocked_ms_per_product"] * 1e-3) / 1e9
+        # many right-hand sides (P0 is reused for ~100 energies): 8 vectors share one pass of the blocked product
+        x8 = torch.from_numpy(np.stack([wi.normal_vector(job.rows, k=200 + k) for k in range(8)])).cuda().contiguous()
+        y8 = torch.empty_like(x8)
+        for nv in (2, 4, 8):
+            for _ in range(2):
+                wpcd.wpcd_perm_apply_blocked(grid, job.channels, job.row_ptr, job.geo_row_ptr, job.col_idx, job.values, x8, y8, n_vec=nv)
+            a.record()
+            for _ in range(reps):
+                wpcd.wpcd_perm_apply_blocked(grid, job.channels, job.row_ptr, job.geo_row_ptr, job.col_idx, job.values, x8, y8, n_vec=nv)
+            b.record()
+            torch.cuda.synchronize()
+            spmm["blocked_nvec%d_ms_per_pass" % nv] = a.elapsed_time(b) / reps
+        del x8, y8
         # one application of the factored kernel K = O P0 O^T V1 G1 (synthetic O, V1, G1)
         n_ch = job.channels.count
         o_h, v_h, g_h = wi.kernel_factors(n_ch, grid.n_p, grid.n_q)
@@ -499,8 +516,8 @@ def run_ours(args):
                                           job.x_all, job.y_all, n_vec=n_spmv)
                 continue
             for k in range(n_spmv):
-                wpcd.wpcd_perm_apply_host(job.rows, job.row_ptr, job.col_idx, job.values, job.x_host[k % job.n_x], job.y_host,
-                                          job.x[0], job.y)
+                wpcd.wpcd_perm_apply_blocked_host(g2, ch2, job.row_ptr, job.geo_row_ptr, job.col_idx, job.values, job.x_host[k % job.n_x],
+                                                  job.y_host, job.x[0], job.y)
     e2e_steps = max(1, min(args.steps, 20 if wl.model == "swave" else 3))
     e2e_step()
     torch.cuda.synchronize()
@@ -558,16 +575,27 @@ def run_ours(args):
                     "algorithmic": {"bytes": wbytes, "flops": flops}})
         roofs["fill_coupled"] = top
     if n_spmv:
-        # algorithmic bytes of a launch with v right-hand sides: the matrix once (12 B per nonzero + row_ptr) + v vectors in and out
+        # algorithmic bytes of a launch with v right-hand sides: the matrix once + v vectors in and out.  The CSR product
+        # (s-wave workloads) reads 12 B per nonzero + row_ptr; the blocked product (coupled channels) reads the values only,
+        # 8 B per nonzero, the geometric pattern (4 B per geometric entry) and x once per (channel, geometric entry)
+        blocked = wl.model == "nd"
         n_launch = sum(len(sweep_passes(j)) for j in jobs)
-        sbytes = sum(sum(12.0 * j.nnz + 8.0 * j.rows + v * 16.0 * j.rows for v in sweep_passes(j)) for j in jobs)
+        if blocked:
+            sbytes = sum(sum(8.0 * j.nnz + 4.0 * j.nnz_geo + v * (8.0 * j.channels.count * j.nnz_geo + 8.0 * j.rows) for v in sweep_passes(j))
+                         for j in jobs)
+        else:
+            sbytes = sum(sum(12.0 * j.nnz + 8.0 * j.rows + v * 16.0 * j.rows for v in sweep_passes(j)) for j in jobs)
+        csr_bytes = sum(sum(12.0 * j.nnz + 8.0 * j.rows + v * 16.0 * j.rows for v in sweep_passes(j)) for j in jobs)
         per_launch_ms = spmv_ms / (steps * n_launch)
         ach = sbytes / (spmv_ms / steps * 1e-3) / 1e9
         roofs["spmv"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                          "traffic": None, "ms_per_launch": per_launch_ms, "launches_per_step": n_launch,
                          "rhs_per_launch": max(max(sweep_passes(j)) for j in jobs),
+                         "kernel_name": "spmv_georow_kernel<1,256> (wpcd_perm_apply_blocked)" if blocked else "spmv_kernel (wpcd_perm_apply)",
+                         "algorithmic_bytes_per_step": sbytes,
+                         "csr_equivalent_GBps": csr_bytes / (spmv_ms / steps * 1e-3) / 1e9,
                          "peak_source": hbm_src,
-                         "note": "matrix is L2-resident (3 MB)" if wl.model == "swave" else "streams from HBM"}
+                         "note": "matrix is L2-resident (3 MB)" if wl.model == "swave" else "values stream from HBM, 8 B per nonzero"}
     share = dict(stage_ms)
     share["spmv_sweep"] = spmv_ms / steps
     # the selection (a1-a3) is reported by its time only (latency-bound, no per-unit figure)

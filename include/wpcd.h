@@ -251,6 +251,13 @@ wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const
                                  const double* values_dev, const double* x_host, double* y_host, int n_vec,
                                  double* x_dev, double* y_dev, void* cuda_stream);
 
+/* wpcd_perm_apply_blocked with HOST vectors: copies x_host -> x_dev (scratch, dev, n_vec*rows doubles), applies, copies
+ * y_dev (scratch) -> y_host, then synchronises.  Pinned host memory makes the copies asynchronous. */
+wpcd_status wpcd_perm_apply_blocked_host(const wpcd_grid* grid, const wpcd_channels* channels, const int64_t* row_ptr_dev,
+                                         const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                         const double* x_host, double* y_host, int n_vec, double* x_dev, double* y_dev,
+                                         void* cuda_stream);
+
 /* FP64 FMA microbenchmark (the roofline denominator of the fill kernel):
  * runs a dependent-chain-free DFMA loop on the whole chip and returns achieved FLOP/s
  * (2 per DFMA) in *flops_out (host).  Synchronises. */

@@ -32,7 +32,7 @@ EXPORTS = [
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_monomials", "wpcd_channels_coefficients", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
+    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_perm_apply_blocked_host", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
     "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read", "wpcd_debug_set",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
@@ -85,6 +85,7 @@ def load():
     L.wpcd_perm_apply_complex.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_interleaved.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_blocked.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    L.wpcd_perm_apply_blocked_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
     L.wpcd_perm_apply_chain.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_block_apply.argtypes = [i32, i32, i32, vp, i32, vp, vp, i32, vp]
     L.wpcd_kernel_apply.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -292,6 +293,17 @@ def wpcd_perm_apply_blocked(grid, channels, row_ptr, geo_row_ptr, col_idx, value
     _check(load().wpcd_perm_apply_blocked(grid.handle, channels.handle, _dev_ptr(row_ptr, torch.int64), _dev_ptr(geo_row_ptr, torch.int32),
                                           _dev_ptr(col_idx, torch.int32), _dev_ptr(values, torch.float64), _dev_ptr(x, torch.float64),
                                           _dev_ptr(y, torch.float64), n_vec, _stream_ptr(stream)))
+
+
+def wpcd_perm_apply_blocked_host(grid, channels, row_ptr, geo_row_ptr, col_idx, values, x_host, y_host, x_dev, y_dev, n_vec=1, stream=None):
+    """wpcd_perm_apply_blocked with CPU float64 tensors x_host / y_host (pinned for async copies); x_dev / y_dev: device scratch."""
+    import torch
+
+    assert not x_host.is_cuda and not y_host.is_cuda and x_host.dtype == torch.float64 and y_host.dtype == torch.float64
+    _check(load().wpcd_perm_apply_blocked_host(grid.handle, channels.handle, _dev_ptr(row_ptr, torch.int64), _dev_ptr(geo_row_ptr, torch.int32),
+                                               _dev_ptr(col_idx, torch.int32), _dev_ptr(values, torch.float64),
+                                               ctypes.c_void_p(x_host.data_ptr()), ctypes.c_void_p(y_host.data_ptr()), n_vec,
+                                               _dev_ptr(x_dev, torch.float64), _dev_ptr(y_dev, torch.float64), _stream_ptr(stream)))
 
 
 def wpcd_perm_apply_chain(rows, row_ptr, col_idx, values, x, y, n_iter, stream=None):

@@ -936,6 +936,27 @@ wpcd_status wpcd_perm_apply_host(int64_t rows, const int64_t* row_ptr_dev, const
     return WPCD_OK;
 }
 
+wpcd_status wpcd_perm_apply_blocked_host(const wpcd_grid* g, const wpcd_channels* c, const int64_t* row_ptr_dev, const int32_t* geo_row_ptr_dev,
+                                         const int32_t* col_idx_dev, const double* values_dev, const double* x_host, double* y_host,
+                                         int n_vec, double* x_dev, double* y_dev, void* cuda_stream)
+{
+    if (!g || !c) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_host: null handle");
+    if (n_vec < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_host: negative size");
+    const int64_t rows = wpcd_rows(g, c);
+    if (rows == 0 || n_vec == 0) return WPCD_OK;
+    if (!x_host || !y_host || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_host: null pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t bytes = sizeof(double) * (size_t)rows * (size_t)n_vec;
+    cudaError_t err = cudaMemcpyAsync(x_dev, x_host, bytes, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_blocked_host(H2D)");
+    wpcd_status s = wpcd_perm_apply_blocked(g, c, row_ptr_dev, geo_row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, cuda_stream);
+    if (s != WPCD_OK) return s;
+    err = cudaMemcpyAsync(y_host, y_dev, bytes, cudaMemcpyDeviceToHost, st);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_blocked_host(D2H)");
+    return WPCD_OK;
+}
+
 wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out)
 {
     if (!flops_out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_fp64_peak: null pointer");

@@ -708,10 +708,15 @@ def test_apply_blocked(wpcd):
         y = torch.full_like(x, np.nan)
         wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y, n_vec=3)
         yh = y.cpu().numpy()
+        xh_pin = torch.from_numpy(xs).pin_memory()
+        yh_pin = torch.full((3, m.rows), np.nan, dtype=torch.float64).pin_memory()
+        wpcd.wpcd_perm_apply_blocked_host(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, xh_pin, yh_pin, torch.empty_like(x),
+                                          torch.empty_like(x), n_vec=3)
         for k in range(3):
             ref = operm.spmv(rp, ci, v, xs[k])
             scale = operm.spmv(rp, ci, np.abs(v), np.abs(xs[k]))
             assert np.all(np.abs(yh[k] - ref) <= 1e-12 * scale + 1e-300), (gch.count, len(p), k)
+            assert np.array_equal(yh_pin[k].numpy(), yh[k])            # same kernel, same summation order
 
 
 def test_apply_blocked_chunked_paths(wpcd):

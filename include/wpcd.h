@@ -27,8 +27,11 @@
  *     alike with primed indices; columns strictly ascending inside a row.
  *   - there is no CPU fallback: without a CUDA device every compute call
  *     returns WPCD_ERR_CUDA.
- *   - a handle must not be used by two host threads at the same time, and wpcd_perm_build calls must not
- *     overlap in time on one device (threads or streams): the quadrature rule lives in constant memory.
+ *   - a GRID handle carries the staged result of its last selection pass (scratch written by wpcd_perm_count, read by
+ *     wpcd_perm_build): the count and build calls on ONE grid handle must not overlap in time -- issue them from one
+ *     thread, and let a build that is still running on its stream finish (or order the next count behind it on the
+ *     same stream) before counting on that handle again.  Different grid handles, and any number of channel handles,
+ *     may be used concurrently from different threads and streams (the quadrature rule travels with each launch).
  */
 #ifndef WPCD_H
 #define WPCD_H

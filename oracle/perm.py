@@ -14,7 +14,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "perm_oracle.c")
 _SO = os.path.join(_HERE, "_perm_oracle.so")
+_SO_EXT = os.path.join(_HERE, "_perm_oracle_ext.so")      # the same source with -DWPO_EXTENDED (rule arithmetic in long double)
 _lib = None
+_lib_ext = None
 
 _D = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
 _I32 = np.ctypeslib.ndpointer(np.int32, flags="C_CONTIGUOUS")
@@ -22,11 +24,25 @@ _I64 = np.ctypeslib.ndpointer(np.int64, flags="C_CONTIGUOUS")
 
 
 def build(force=False):
-    """Compile perm_oracle.c (gcc, -ffp-contract=off) next to this file."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", _SRC, "-lm", "-o", _SO]
-        subprocess.check_call(cmd)
+    """Compile perm_oracle.c (gcc, -ffp-contract=off) next to this file: the FP64 oracle and its long-double twin."""
+    for so, extra in ((_SO, []), (_SO_EXT, ["-DWPO_EXTENDED"])):
+        if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+            cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC"] + extra + [_SRC, "-lm", "-o", so]
+            subprocess.check_call(cmd)
     return _SO
+
+
+def lib_extended():
+    """The -DWPO_EXTENDED build: same statements, rule arithmetic in long double (only wpo_elements_rule is used from it)."""
+    global _lib_ext
+    if _lib_ext is None:
+        build()
+        L = ctypes.CDLL(_SO_EXT)
+        i32, i64 = ctypes.c_int, ctypes.c_int64
+        L.wpo_elements_rule.argtypes = [i32, i32, _D, _D, i64, _I32, _I32, _I32, _I32, i32, _D, _D, i32,
+                                        i32, _I32, _I32, _I64, _I32, _I32, _I32, _D, _D, _D]
+        _lib_ext = L
+    return _lib_ext
 
 
 def lib():
@@ -103,9 +119,10 @@ def gauss_legendre(n):
     return np.ascontiguousarray(xi), np.ascontiguousarray(w)
 
 
-def element_values(p, q, ei, ej, eip, ejp, n_quad, table, split=False):
+def element_values(p, q, ei, ej, eip, ejp, n_quad, table, split=False, extended=False):
     """Values (A15) by rule R(n_quad) -- the kink-split rule RS(n_quad) if split is True / 1, the rule RA(n_quad) with the
     exact u-integral (s-wave term only) if split == 2 -- of the listed geometric elements, all pairs.
+    extended=True: the same rule with its arithmetic in long double (results rounded to double at the end).
     Returns (val, absval), each [n_elem, n_pairs]."""
     if int(split) == 2:
         one = np.diff(table.term_ptr) == 1
@@ -117,7 +134,7 @@ def element_values(p, q, ei, ej, eip, ejp, n_quad, table, split=False):
     ne = len(ei)
     val = np.zeros((ne, table.n_pairs))
     absval = np.zeros((ne, table.n_pairs))
-    lib().wpo_elements_rule(len(p) - 1, len(q) - 1, p, q, ne, ei, ej, eip, ejp, n_quad, xi, w, int(split),
+    (lib_extended() if extended else lib()).wpo_elements_rule(len(p) - 1, len(q) - 1, p, q, ne, ei, ej, eip, ejp, n_quad, xi, w, int(split),
                        table.n_pairs, table.pair_l, table.pair_lp, table.term_ptr, table.term_k,
                        table.term_l1, table.term_l1p, table.term_g, val, absval)
     return val, absval

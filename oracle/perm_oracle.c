@@ -177,83 +177,94 @@ void wpo_geo_fill(int n_p, int n_q, const double* p, const double* q,
  * Sum over (k,l1,l1') is taken PER NODE, before integrating (R8).
  */
 #define WPO_MAXPOW 24
-static void element_values(double a, double b, double c, double d,
-                           double L1, double U1, double L2, double U2,
-                           int n, const double* xi, const double* w, int split,
-                           int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
-                           const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
-                           const int32_t* term_l1p, const double* term_g,
-                           double* val, double* absval)
+/* Arithmetic type of the rule.  The default build is plain FP64 (the precision the CUDA path is compared with).  With
+ * -DWPO_EXTENDED the SAME statements run in long double (x87, 64-bit mantissa): the reference that tells rounding of the
+ * FP64 evaluations apart from each other on the ill-conditioned first-bin cells (tests: oracle/perm.py, extended=True).
+ * Inputs, Gauss-Legendre nodes and outputs stay double; the predicate and the polygon are the FP64 ones in both builds. */
+#ifdef WPO_EXTENDED
+typedef long double real;
+#define RM(f) f##l
+#else
+typedef double real;
+#define RM(f) f
+#endif
+static void element_values_inner(double a_, double b_, double c_, double d_,
+                                 double L1_, double U1_, double L2_, double U2_,
+                                 int n, const double* xi, const double* w, int split,
+                                 int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
+                                 const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
+                                 const int32_t* term_l1p, const double* term_g,
+                                 real* val, real* absval)
 {
-    for (int cidx = 0; cidx < n_pairs; ++cidx) { val[cidx] = 0.0; absval[cidx] = 0.0; }
+    const real a = a_, b = b_, c = c_, d = d_, L1 = L1_, U1 = U1_, L2 = L2_, U2 = U2_;
     wpo_pt poly[WPO_MAXV];
     int nv = 0;
-    if (!wpo_overlap(a, b, c, d, L1, U1, L2, U2, poly, &nv)) return;
+    if (!wpo_overlap(a_, b_, c_, d_, L1_, U1_, L2_, U2_, poly, &nv)) return;
     /* phi-range: angular extent of the polygon Pi (rule R1b) */
-    double phi_a = 1e300, phi_b = -1e300;
+    real phi_a = 1e300, phi_b = -1e300;
     for (int v = 0; v < nv; ++v) {
         if (poly[v].s == 0.0 && poly[v].t == 0.0) continue; /* the origin has no angle */
-        double ang = atan2(poly[v].t, poly[v].s);
-        phi_a = fmin(phi_a, ang);
-        phi_b = fmax(phi_b, ang);
+        real ang = RM(atan2)(poly[v].t, poly[v].s);
+        phi_a = RM(fmin)(phi_a, ang);
+        phi_b = RM(fmax)(phi_b, ang);
     }
     if (!(phi_a < phi_b)) return;
-    double norm = 1.0 / sqrt((U2 - L2) * (b - a) * (U1 - L1) * (d - c)); /* (d_i dbar_j d_i' dbar_j')^{-1/2}, A5/A9 */
+    real norm = 1.0 / RM(sqrt)((U2 - L2) * (b - a) * (U1 - L1) * (d - c)); /* (d_i dbar_j d_i' dbar_j')^{-1/2}, A5/A9 */
     /* Rule R(n): one piece in phi, one piece in u.  Rule RS(n) (split != 0, R14): the phi-range is
      * cut at the rectangle-corner angles where the active member of Lq = max(a/C, c/S) or Uq = min(b/C, d/S)
      * switches (tan phi = c/a, tan phi = d/b), and at every phi-node the u-range is cut at the abscissae where two
      * members of Qmax = min(Uq, U1/zeta1, U2/zeta2) or of Qmin = max(Lq, L1/zeta1, L2/zeta2) of (A14) cross
      * (zeta^2 is linear in u, so each crossing is a closed form); n-point Gauss-Legendre on every piece. */
-    double phi_cut[4];
+    real phi_cut[4];
     int n_phi_piece = 1;
     phi_cut[0] = phi_a;
     if (split) {
-        double c1 = atan2(c, a), c2 = atan2(d, b);
-        double lo = fmin(c1, c2), hi = fmax(c1, c2);
+        real c1 = RM(atan2)(c, a), c2 = RM(atan2)(d, b);
+        real lo = RM(fmin)(c1, c2), hi = RM(fmax)(c1, c2);
         if (lo > phi_a && lo < phi_b) phi_cut[n_phi_piece++] = lo;
         if (hi > phi_cut[n_phi_piece - 1] && hi < phi_b) phi_cut[n_phi_piece++] = hi;
     }
     phi_cut[n_phi_piece] = phi_b;
     for (int piece = 0; piece < n_phi_piece; ++piece) {
-    double half_phi = 0.5 * (phi_cut[piece + 1] - phi_cut[piece]), mid_phi = 0.5 * (phi_cut[piece] + phi_cut[piece + 1]);
+    real half_phi = 0.5 * (phi_cut[piece + 1] - phi_cut[piece]), mid_phi = 0.5 * (phi_cut[piece] + phi_cut[piece + 1]);
     for (int m = 0; m < n; ++m) {
-        double phi = mid_phi + half_phi * xi[m];
-        double wphi = half_phi * w[m];
-        double C = cos(phi), S = sin(phi);
+        real phi = mid_phi + half_phi * xi[m];
+        real wphi = half_phi * w[m];
+        real C = RM(cos)(phi), S = RM(sin)(phi);
         /* Q-limits from the rectangle, A12 */
-        double Lq = fmax(a / C, c / S), Uq = fmin(b / C, d / S);
+        real Lq = RM(fmax)(a / C, c / S), Uq = RM(fmin)(b / C, d / S);
         if (!(Lq < Uq)) continue;
         /* zeta of A11 in the variable u = 1 + x (R7: same rule, conditioned near the
          * pi1 = 0 / pi2 = 0 corners x = -1):  zeta1^2 = b1 + beta u,  zeta2^2 = b2 + beta u */
-        double b1 = (C - 0.5 * S) * (C - 0.5 * S);
-        double b2 = (0.5 * C - S) * (0.5 * C - S);
-        double beta = C * S;
+        real b1 = (C - 0.5 * S) * (C - 0.5 * S);
+        real b2 = (0.5 * C - S) * (0.5 * C - S);
+        real beta = C * S;
         /* u-support of F > 0 (closed form; zeta^2 linear in u) */
-        double u_lo = 0.0, u_hi = 2.0;
-        if (L1 > 0.0) u_lo = fmax(u_lo, ((L1 / Uq) * (L1 / Uq) - b1) / beta);
-        if (L2 > 0.0) u_lo = fmax(u_lo, ((L2 / Uq) * (L2 / Uq) - b2) / beta);
+        real u_lo = 0.0, u_hi = 2.0;
+        if (L1 > 0.0) u_lo = RM(fmax)(u_lo, ((L1 / Uq) * (L1 / Uq) - b1) / beta);
+        if (L2 > 0.0) u_lo = RM(fmax)(u_lo, ((L2 / Uq) * (L2 / Uq) - b2) / beta);
         if (Lq > 0.0) {
-            u_hi = fmin(u_hi, ((U1 / Lq) * (U1 / Lq) - b1) / beta);
-            u_hi = fmin(u_hi, ((U2 / Lq) * (U2 / Lq) - b2) / beta);
+            u_hi = RM(fmin)(u_hi, ((U1 / Lq) * (U1 / Lq) - b1) / beta);
+            u_hi = RM(fmin)(u_hi, ((U2 / Lq) * (U2 / Lq) - b2) / beta);
         }
         {   /* L1/zeta1 < U2/zeta2  <=>  beta u (L1^2-U2^2) < U2^2 b1 - L1^2 b2 */
-            double D = L1 * L1 - U2 * U2, R = U2 * U2 * b1 - L1 * L1 * b2;
-            if (D > 0.0) u_hi = fmin(u_hi, R / (beta * D));
-            else if (D < 0.0) u_lo = fmax(u_lo, R / (beta * D));
+            real D = L1 * L1 - U2 * U2, R = U2 * U2 * b1 - L1 * L1 * b2;
+            if (D > 0.0) u_hi = RM(fmin)(u_hi, R / (beta * D));
+            else if (D < 0.0) u_lo = RM(fmax)(u_lo, R / (beta * D));
             else if (!(0.0 < R)) continue;
         }
         {   /* L2/zeta2 < U1/zeta1  <=>  beta u (L2^2-U1^2) < U1^2 b2 - L2^2 b1 */
-            double D = L2 * L2 - U1 * U1, R = U1 * U1 * b2 - L2 * L2 * b1;
-            if (D > 0.0) u_hi = fmin(u_hi, R / (beta * D));
-            else if (D < 0.0) u_lo = fmax(u_lo, R / (beta * D));
+            real D = L2 * L2 - U1 * U1, R = U1 * U1 * b2 - L2 * L2 * b1;
+            if (D > 0.0) u_hi = RM(fmin)(u_hi, R / (beta * D));
+            else if (D < 0.0) u_lo = RM(fmax)(u_lo, R / (beta * D));
             else if (!(0.0 < R)) continue;
         }
         if (!(u_lo < u_hi)) continue;
-        double u_cut[8];
+        real u_cut[8];
         int n_u_piece = 1;
         u_cut[0] = u_lo;
         if (split) {
-            double cand[6];
+            real cand[6];
             int nc = 0;
             cand[nc++] = ((U1 / Uq) * (U1 / Uq) - b1) / beta;                         /* Uq = U1/zeta1 */
             cand[nc++] = ((U2 / Uq) * (U2 / Uq) - b2) / beta;                         /* Uq = U2/zeta2 */
@@ -264,7 +275,7 @@ static void element_values(double a, double b, double c, double d,
             }
             if (L1 != L2) cand[nc++] = (L2 * L2 * b1 - L1 * L1 * b2) / (beta * (L1 * L1 - L2 * L2)); /* L1/zeta1 = L2/zeta2 */
             for (int i1 = 1; i1 < nc; ++i1) {                                         /* ascending */
-                double key = cand[i1];
+                real key = cand[i1];
                 int i0 = i1 - 1;
                 while (i0 >= 0 && cand[i0] > key) { cand[i0 + 1] = cand[i0]; --i0; }
                 cand[i0 + 1] = key;
@@ -274,11 +285,11 @@ static void element_values(double a, double b, double c, double d,
         }
         u_cut[n_u_piece] = u_hi;
         /* powers of cos, sin */
-        double cp[WPO_MAXPOW], sp[WPO_MAXPOW];
+        real cp[WPO_MAXPOW], sp[WPO_MAXPOW];
         cp[0] = 1.0; sp[0] = 1.0;
         for (int e = 1; e < WPO_MAXPOW; ++e) { cp[e] = cp[e - 1] * C; sp[e] = sp[e - 1] * S; }
         for (int upiece = 0; upiece < n_u_piece; ++upiece) {
-        double half_u = 0.5 * (u_cut[upiece + 1] - u_cut[upiece]), mid_u = 0.5 * (u_cut[upiece] + u_cut[upiece + 1]);
+        real half_u = 0.5 * (u_cut[upiece + 1] - u_cut[upiece]), mid_u = 0.5 * (u_cut[upiece] + u_cut[upiece + 1]);
         if (split == 2) {
             /* Rule RA(n) (R15), s-wave term only (k = l1 = l1' = 0, l = l' = 0): on a piece between two
              * cuts the active members of (A14)'s min and max do not change, each is a constant or a constant over
@@ -289,66 +300,66 @@ static void element_values(double a, double b, double c, double d,
              *   I2 = int du / (zeta1 zeta2^3)   = (2/beta) (1/zeta2l^2 - 1/zeta2h^2) / (zeta1h/zeta2h + zeta1l/zeta2l)
              * (l, h = lower, upper end of the piece; the forms for I1, I2 have no cancellation when b1 -> b2).
              * The active members are read off at the midpoint of the piece. */
-            double ul = u_cut[upiece], uh = u_cut[upiece + 1];
-            double z1m = sqrt(b1 + beta * mid_u), z2m = sqrt(b2 + beta * mid_u);
-            double dA = 0.0, dB = 0.0, dC = 0.0;
+            real ul = u_cut[upiece], uh = u_cut[upiece + 1];
+            real z1m = RM(sqrt)(b1 + beta * mid_u), z2m = RM(sqrt)(b2 + beta * mid_u);
+            real dA = 0.0, dB = 0.0, dC = 0.0;
             {   /* Qmax^2 = min(Uq^2, U1^2/zeta1^2, U2^2/zeta2^2) */
-                double m0 = Uq, m1 = U1 / z1m, m2 = U2 / z2m;
+                real m0 = Uq, m1 = U1 / z1m, m2 = U2 / z2m;
                 if (m0 <= m1 && m0 <= m2) dA += Uq * Uq; else if (m1 <= m2) dB += U1 * U1; else dC += U2 * U2;
             }
             {   /* Qmin^2 = max(Lq^2, L1^2/zeta1^2, L2^2/zeta2^2) */
-                double m0 = Lq, m1 = L1 / z1m, m2 = L2 / z2m;
+                real m0 = Lq, m1 = L1 / z1m, m2 = L2 / z2m;
                 if (m0 >= m1 && m0 >= m2) dA -= Lq * Lq; else if (m1 >= m2) dB -= L1 * L1; else dC -= L2 * L2;
             }
-            double z1l = sqrt(b1 + beta * ul), z2l = sqrt(b2 + beta * ul);
-            double z1h = sqrt(b1 + beta * uh), z2h = sqrt(b2 + beta * uh);
+            real z1l = RM(sqrt)(b1 + beta * ul), z2l = RM(sqrt)(b2 + beta * ul);
+            real z1h = RM(sqrt)(b1 + beta * uh), z2h = RM(sqrt)(b2 + beta * uh);
             /* differences of the ends written without cancellation: zeta_h - zeta_l = beta du / (zeta_h + zeta_l),
              * 1/zeta_l^2 - 1/zeta_h^2 = beta du / (zeta_l^2 zeta_h^2) */
-            double du = uh - ul;
-            double integral = 0.0;
+            real du = uh - ul;
+            real integral = 0.0;
             if (dA != 0.0)
-                integral += dA * (2.0 / beta) * log1p((beta * du / (z1h + z1l) + beta * du / (z2h + z2l)) / (z1l + z2l));
+                integral += dA * (2.0 / beta) * RM(log1p)((beta * du / (z1h + z1l) + beta * du / (z2h + z2l)) / (z1l + z2l));
             if (dB != 0.0) integral += dB * 2.0 * du / (z1l * z1l * z1h * z1h) / (z2h / z1h + z2l / z1l);
             if (dC != 0.0) integral += dC * 2.0 * du / (z2l * z2l * z2h * z2h) / (z1h / z2h + z1l / z2l);
             if (integral > 0.0) {
                 for (int cidx = 0; cidx < n_pairs; ++cidx) {
-                    double g = term_g[term_ptr[cidx]];
+                    real g = term_g[term_ptr[cidx]];
                     val[cidx] += wphi * 0.5 * integral * g * C * S;
-                    absval[cidx] += wphi * 0.5 * integral * fabs(g) * C * S;
+                    absval[cidx] += wphi * 0.5 * integral * RM(fabs)(g) * C * S;
                 }
             }
             continue;
         }
         for (int r = 0; r < n; ++r) {
-            double u = mid_u + half_u * xi[r];
-            double x = u - 1.0;
-            double wx = half_u * w[r];
-            double zeta1 = sqrt(b1 + beta * u), zeta2 = sqrt(b2 + beta * u);
+            real u = mid_u + half_u * xi[r];
+            real x = u - 1.0;
+            real wx = half_u * w[r];
+            real zeta1 = RM(sqrt)(b1 + beta * u), zeta2 = RM(sqrt)(b2 + beta * u);
             /* F of A14, clamped (R5) */
-            double Qmax = fmin(fmin(Uq, U1 / zeta1), U2 / zeta2);
-            double Qmin = fmax(fmax(Lq, L1 / zeta1), L2 / zeta2);
+            real Qmax = RM(fmin)(RM(fmin)(Uq, U1 / zeta1), U2 / zeta2);
+            real Qmin = RM(fmax)(RM(fmax)(Lq, L1 / zeta1), L2 / zeta2);
             if (!(Qmax > Qmin)) continue;
-            double F = 0.5 * (Qmax * Qmax - Qmin * Qmin);
+            real F = 0.5 * (Qmax * Qmax - Qmin * Qmin);
             /* Legendre polynomials by the three-term recurrence */
-            double P[WPO_MAXPOW];
+            real P[WPO_MAXPOW];
             P[0] = 1.0; P[1] = x;
             for (int k = 2; k < WPO_MAXPOW; ++k) P[k] = ((2 * k - 1) * x * P[k - 1] - (k - 1) * P[k - 2]) / k;
-            double z1p[WPO_MAXPOW], z2p[WPO_MAXPOW]; /* zeta^m */
+            real z1p[WPO_MAXPOW], z2p[WPO_MAXPOW]; /* zeta^m */
             z1p[0] = 1.0; z2p[0] = 1.0;
             for (int e = 1; e < WPO_MAXPOW; ++e) { z1p[e] = z1p[e - 1] * zeta1; z2p[e] = z2p[e - 1] * zeta2; }
-            double wF = wphi * wx * F;
+            real wF = wphi * wx * F;
             for (int cidx = 0; cidx < n_pairs; ++cidx) {
                 int l = pair_l[cidx], lp = pair_lp[cidx];
-                double sum = 0.0, asum = 0.0;
+                real sum = 0.0, asum = 0.0;
                 for (int64_t tt = term_ptr[cidx]; tt < term_ptr[cidx + 1]; ++tt) {
                     int l1 = term_l1[tt], l1p = term_l1p[tt];
-                    int A = l1 + l1p;                 /* power of q  = Q cos(phi) (R1) */
-                    int B = (l - l1) + (lp - l1p);    /* power of q' = Q sin(phi) */
-                    double term = term_g[tt] * P[term_k[tt]] * cp[A + 1] * sp[B + 1];
+                    int A = l1 + l1p;                 /* power of q  = Q RM(cos)(phi) (R1) */
+                    int B = (l - l1) + (lp - l1p);    /* power of q' = Q RM(sin)(phi) */
+                    real term = term_g[tt] * P[term_k[tt]] * cp[A + 1] * sp[B + 1];
                     sum += term;
-                    asum += fabs(term);
+                    asum += RM(fabs)(term);
                 }
-                double denom = z1p[lp + 1] * z2p[l + 1];
+                real denom = z1p[lp + 1] * z2p[l + 1];
                 val[cidx] += wF * sum / denom;
                 absval[cidx] += wF * asum / denom;
             }
@@ -357,6 +368,24 @@ static void element_values(double a, double b, double c, double d,
     }
     } /* phi pieces */
     for (int cidx = 0; cidx < n_pairs; ++cidx) { val[cidx] *= norm; absval[cidx] *= norm; }
+}
+
+
+static void element_values(double a, double b, double c, double d,
+                           double L1, double U1, double L2, double U2,
+                           int n, const double* xi, const double* w, int split,
+                           int n_pairs, const int32_t* pair_l, const int32_t* pair_lp,
+                           const int64_t* term_ptr, const int32_t* term_k, const int32_t* term_l1,
+                           const int32_t* term_l1p, const double* term_g,
+                           double* val_out, double* absval_out)
+{
+    for (int cidx = 0; cidx < n_pairs; ++cidx) { val_out[cidx] = 0.0; absval_out[cidx] = 0.0; }
+    real* val = (real*)calloc(2 * (size_t)n_pairs, sizeof(real));   /* the sums are kept in the rule's arithmetic type */
+    real* absval = val + n_pairs;
+    element_values_inner(a, b, c, d, L1, U1, L2, U2, n, xi, w, split, n_pairs, pair_l, pair_lp, term_ptr, term_k, term_l1, term_l1p, term_g,
+                         val, absval);
+    for (int cidx = 0; cidx < n_pairs; ++cidx) { val_out[cidx] = (double)val[cidx]; absval_out[cidx] = (double)absval[cidx]; }
+    free(val);
 }
 
 /* Values of n_elem listed geometric elements (row cell (ei,ej), column cell (eip,ejp),

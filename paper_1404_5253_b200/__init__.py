@@ -420,4 +420,9 @@ def build_perm(grid, channels, n_quad, stream=None, device="cuda"):
     ws_bytes = wpcd_perm_workspace_bytes(channels, nnz_geo)
     workspace = torch.empty(max(ws_bytes, 256), dtype=torch.uint8, device=device)
     wpcd_perm_build(grid, channels, n_quad, row_ptr, geo_row_ptr, workspace, col_idx, values, stream)
+    if stream is not None and not isinstance(stream, int) and stream != torch.cuda.current_stream():
+        # the tensors were allocated on torch's current stream but are used on `stream`: tell the caching allocator, so that
+        # the workspace (dropped on return, while the asynchronous build may still run) is not handed out too early
+        for t in (workspace, row_ptr, geo_row_ptr, col_idx, values):
+            t.record_stream(stream)
     return PermCSR(rows, nnz, nnz_geo, row_ptr, col_idx, values, geo_row_ptr)

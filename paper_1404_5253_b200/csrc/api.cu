@@ -32,15 +32,17 @@ static wpcd_status cuda_fail(cudaError_t err, const char* where)
     return fail(WPCD_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(err));
 }
 
-static bool g_trace_on = false;
+static std::atomic<bool> g_trace_on{false};
 struct TraceRec { int stage; cudaEvent_t e0, e1; };
 static std::vector<TraceRec> g_trace;
+static std::mutex g_trace_mutex;       // guards g_trace and g_trace_spare
 
 static std::vector<cudaEvent_t> g_trace_spare;      // timing events are reused: creating one costs more than recording it
 
 static cudaEvent_t trace_event()
 {
     cudaEvent_t e = nullptr;
+    std::lock_guard<std::mutex> lock(g_trace_mutex);
     if (!g_trace_spare.empty()) { e = g_trace_spare.back(); g_trace_spare.pop_back(); }
     else cudaEventCreate(&e);
     return e;
@@ -56,6 +58,7 @@ StageTimer::~StageTimer()
 {
     if (!e0) return;
     cudaEventRecord(e1, st);
+    std::lock_guard<std::mutex> lock(g_trace_mutex);
     g_trace.push_back({stage, e0, e1});
 }
 
@@ -548,7 +551,7 @@ int64_t wpcd_geo_rows(const wpcd_grid* g) { return g ? (int64_t)g->n_p * g->n_q 
 // Selection pass on grid g: predicate, per-row counts, staged verdicts, scan, and (when c is
 // given) the row pointer of the full matrix.  Synchronises the stream (the caller needs nnz_geo);
 // repeats the pass with a larger staging area if it overflowed.
-static wpcd_status run_selection(wpcd_grid* g, const wpcd_channels* c, int32_t* geo_row_ptr_dev, int64_t* row_ptr_dev,
+static wpcd_status run_selection(const wpcd_grid* g, const wpcd_channels* c, int32_t* geo_row_ptr_dev, int64_t* row_ptr_dev,
                                  cudaStream_t st, const char* who)
 {
     const int n_geo = g->n_p * g->n_q;
@@ -583,15 +586,14 @@ static wpcd_status run_selection(wpcd_grid* g, const wpcd_channels* c, int32_t* 
     return fail(WPCD_ERR_ALLOC, std::string(who) + ": staging area kept overflowing");
 }
 
-wpcd_status wpcd_perm_count(const wpcd_grid* g_in, const wpcd_channels* c, int n_quad, void* cuda_stream, int64_t* row_ptr_dev,
+wpcd_status wpcd_perm_count(const wpcd_grid* g, const wpcd_channels* c, int n_quad, void* cuda_stream, int64_t* row_ptr_dev,
                             int32_t* geo_row_ptr_dev, int64_t* nnz_out, int64_t* nnz_geo_out)
 {
-    if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
+    if (!g || !c || !row_ptr_dev || !geo_row_ptr_dev || !nnz_out || !nnz_geo_out)
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_count: null pointer");
     n_quad &= ~(WPCD_RULE_KINK_SPLIT | WPCD_RULE_ANALYTIC_U);       // the pattern does not depend on the rule
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_count: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_count: channel tables are not on a device (no CUDA device?)");
-    wpcd_grid* g = const_cast<wpcd_grid*>(g_in);   // the staging scratch inside the handle is mutable state
     int64_t rows = wpcd_rows(g, c);
     if (rows > (int64_t)INT32_MAX) return fail(WPCD_ERR_OVERFLOW, "wpcd_perm_count: column index would not fit int32");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -614,11 +616,11 @@ size_t wpcd_perm_workspace_bytes(const wpcd_channels* c, int64_t nnz_geo)
     return carve_workspace(c, nnz_geo, nullptr).bytes;
 }
 
-wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n_quad, void* cuda_stream, const int64_t* row_ptr_dev,
+wpcd_status wpcd_perm_build(const wpcd_grid* g, const wpcd_channels* c, int n_quad, void* cuda_stream, const int64_t* row_ptr_dev,
                             const int32_t* geo_row_ptr_dev, void* workspace_dev, size_t workspace_bytes, int32_t* col_idx_dev,
                             double* values_dev)
 {
-    if (!g_in || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
+    if (!g || !c || !row_ptr_dev || !geo_row_ptr_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_build: null pointer");
     const bool analytic = (n_quad & WPCD_RULE_ANALYTIC_U) != 0;
     const bool split = (n_quad & WPCD_RULE_KINK_SPLIT) != 0 || analytic;
     n_quad &= ~(WPCD_RULE_KINK_SPLIT | WPCD_RULE_ANALYTIC_U);
@@ -626,7 +628,6 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g_in, const wpcd_channels* c, int n
         return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: WPCD_RULE_ANALYTIC_U is for the s-wave term (k = l = l' = 0) only");
     if (n_quad < 1 || n_quad > WPCD_MAX_QUAD) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_build: n_quad out of range");
     if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_build: channel tables are not on a device (no CUDA device?)");
-    wpcd_grid* g = const_cast<wpcd_grid*>(g_in);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     if (!g->stage_valid) {
         // no selection pass has run on this handle (geo_row_ptr came from elsewhere): redo it into
@@ -968,6 +969,7 @@ wpcd_status wpcd_fp64_peak(void* cuda_stream, double* flops_out)
 wpcd_status wpcd_trace_enable(int on)
 {
     g_trace_on = on != 0;
+    std::lock_guard<std::mutex> lock(g_trace_mutex);
     if (g_trace_on) {                       // have the timing events ready before the region that is timed
         while (g_trace_spare.size() < 2048) {
             cudaEvent_t e = nullptr;
@@ -983,6 +985,7 @@ wpcd_status wpcd_trace_read(double* ms_out, int64_t* launches_out)
     if (!ms_out) return fail(WPCD_ERR_INVALID_ARG, "wpcd_trace_read: null pointer");
     for (int i = 0; i < WPCD_TRACE_STAGES; ++i) { ms_out[i] = 0.0; if (launches_out) launches_out[i] = 0; }
     cudaError_t err = cudaSuccess;
+    std::lock_guard<std::mutex> lock(g_trace_mutex);
     for (auto& r : g_trace) {
         float ms = 0.f;
         cudaError_t e = cudaEventSynchronize(r.e1);

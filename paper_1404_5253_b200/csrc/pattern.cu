@@ -29,6 +29,9 @@
 //                       verdicts into the ascending column list geo_col / geo_row / geo_phi.
 #include <math.h>
 
+#include <map>
+#include <mutex>
+
 #include "wpcd_internal.h"
 
 namespace {
@@ -153,7 +156,7 @@ geo_select_kernel(const double* __restrict__ p_g, const double* __restrict__ q_g
                   int32_t* __restrict__ geo_counts, int32_t* __restrict__ stage_off, int32_t* __restrict__ stage_len,
                   int32_t* __restrict__ stage_col, double4* __restrict__ stage_ext, int32_t* __restrict__ ctrl)
 {
-    extern __shared__ double smem_d[];
+    extern __shared__ __align__(16) double smem_d[];     // 16 bytes: the tangent table is read as double2
     double2* tanp = reinterpret_cast<double2*>(smem_d);          // [n_p] (4 U / 3, 2 U / 3), U = p[i+1]
     double* p = smem_d + 2 * n_p;             // [n_p+1]
     double* q = p + (n_p + 1);                // [n_q+1]
@@ -367,14 +370,22 @@ static size_t select_smem(const wpcd_grid* g)
     return sizeof(double) * (size_t)(g->n_p + g->n_q + 2 + 2 * g->n_p) + sizeof(int32_t) * (size_t)ROWS_PER_BLOCK * (2 * g->n_p + 1);
 }
 
-cudaError_t ensure_stage(wpcd_grid* g, int64_t want_cap)
+cudaError_t ensure_stage(const wpcd_grid* g, int64_t want_cap)
 {
     cudaError_t err = cudaSuccess;
     if (!g->select_ready) {
+        // the attribute belongs to the kernel (per device), not to the grid, and a call replaces it: keep the largest request
+        static std::mutex attr_mutex;
+        static std::map<int, size_t> attr_max;
         const size_t need = select_smem(g);
         if (need > 227 * 1024) return cudaErrorInvalidValue;   // n_p beyond what one CTA can stage
-        if (need > 48 * 1024) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        std::lock_guard<std::mutex> lock(attr_mutex);
+        size_t& have = attr_max[dev];
+        if (need > 48 * 1024 && need > have) {
             if ((err = cudaFuncSetAttribute(geo_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need)) != cudaSuccess) return err;
+            have = need;
         }
         g->select_ready = true;
     }
@@ -393,7 +404,7 @@ cudaError_t ensure_stage(wpcd_grid* g, int64_t want_cap)
 }
 
 // Predicate + per-row counts + staged verdicts (a1) and, in its last CTA, the scan (a2).  No sync.
-cudaError_t launch_geo_select(wpcd_grid* g, int32_t* geo_row_ptr_dev, cudaStream_t st)
+cudaError_t launch_geo_select(const wpcd_grid* g, int32_t* geo_row_ptr_dev, cudaStream_t st)
 {
     const int n_geo = g->n_p * g->n_q;
     const int blocks = (n_geo + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK;

@@ -40,6 +40,7 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
         if (PIPE) {
             // long rows streamed from HBM: the index/value loads of batch b+1 are in flight while the
             // gathers and multiply-adds of batch b run (software pipeline, two batches of registers)
+            // a slot beyond the row end carries column -1 and is skipped: no x is read for it (x[0] may be Inf or NaN)
             double a[UNR], a2[UNR];
             int c[UNR], c2[UNR];
             int64_t e0 = beg + sub;
@@ -48,7 +49,7 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
                 const int64_t e = e0 + (int64_t)k * LPR;
                 const bool in = e < end;
                 a[k] = in ? __ldcs(values + e) : 0.0;
-                c[k] = in ? __ldcs(col_idx + e) : 0;
+                c[k] = in ? __ldcs(col_idx + e) : -1;
             }
             for (; e0 < end; e0 += (int64_t)UNR * LPR) {
                 const int64_t n0 = e0 + (int64_t)UNR * LPR;
@@ -57,10 +58,11 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
                     const int64_t e = n0 + (int64_t)k * LPR;
                     const bool in = e < end;
                     a2[k] = in ? __ldcs(values + e) : 0.0;
-                    c2[k] = in ? __ldcs(col_idx + e) : 0;
+                    c2[k] = in ? __ldcs(col_idx + e) : -1;
                 }
 #pragma unroll
                 for (int k = 0; k < UNR; ++k) {
+                    if (c[k] < 0) continue;
 #pragma unroll
                     for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], __ldg(x + v * ldx + c[k]), acc[v]);
                 }
@@ -76,10 +78,11 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
                 const int64_t e = e0 + (int64_t)k * LPR;
                 const bool in = e < end;
                 a[k] = in ? values[e] : 0.0;
-                c[k] = in ? col_idx[e] : 0;
+                c[k] = in ? col_idx[e] : -1;
             }
 #pragma unroll
             for (int k = 0; k < UNR; ++k) {
+                if (c[k] < 0) continue;        // beyond the row end: no x is read (x[0] may be Inf or NaN)
 #pragma unroll
                 for (int v = 0; v < NV; ++v) acc[v] = fma(a[k], __ldg(x + v * ldx + c[k]), acc[v]);
             }
@@ -165,7 +168,7 @@ spmv_interleaved_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const
                 const int64_t e = e0 + (int64_t)k * LPR;
                 const bool in = e < end;
                 a[k] = in ? __ldcs(values + e) : 0.0;
-                c[k] = in ? __ldcs(col_idx + e) : 0;
+                c[k] = in ? __ldcs(col_idx + e) : -1;
             }
             for (; e0 < end; e0 += (int64_t)UNR * LPR) {
                 const int64_t n0 = e0 + (int64_t)UNR * LPR;
@@ -174,10 +177,11 @@ spmv_interleaved_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const
                     const int64_t e = n0 + (int64_t)k * LPR;
                     const bool in = e < end;
                     a2[k] = in ? __ldcs(values + e) : 0.0;
-                    c2[k] = in ? __ldcs(col_idx + e) : 0;
+                    c2[k] = in ? __ldcs(col_idx + e) : -1;
                 }
 #pragma unroll
                 for (int k = 0; k < UNR; ++k) {
+                    if (c[k] < 0) continue;        // beyond the row end: no x is read
 #pragma unroll
                     for (int h = 0; h < H; ++h) {
                         const double2 xv = __ldg(x + (int64_t)c[k] * H + h);

@@ -15,21 +15,22 @@ struct wpcd_grid {
     char* block_dev = nullptr;  // one device allocation holding p, q, ctrl, stage_off, stage_len
     double* p_dev = nullptr;    // [n_p+1]
     double* q_dev = nullptr;    // [n_q+1]
-    // Staged result of the last selection pass on this grid (scratch owned by the handle,
-    // written by wpcd_perm_count, consumed by wpcd_perm_build): one slot per box-test candidate.
-    int32_t* stage_col = nullptr;       // [stage_cap]  column index, or -1 for a rejected candidate
-    double4* stage_ext = nullptr;       // [stage_cap]  vertices of smallest / largest polar angle of Pi (survivors)
-    int32_t* stage_off = nullptr;       // [n_p*n_q]    first slot of a geometric row
-    int32_t* stage_len = nullptr;       // [n_p*n_q]    number of candidates of a geometric row
-    int32_t* ctrl = nullptr;            // [4] device: slot cursor, overflow flag, nnz_geo
-    int32_t* ctrl_pinned = nullptr;     // [4] pinned host copy
-    cudaEvent_t count_event = nullptr;  // behind the read-back of the selection result
-    cudaEvent_t rowptr_event = nullptr; // behind the row-pointer expansion of the last count
-    cudaStream_t count_stream = nullptr;
-    int64_t stage_cap = 0;
-    bool stage_valid = false;
-    bool select_ready = false;          // kernel attributes set
-    int64_t stage_nnz_geo = 0;
+    // Staged result of the last selection pass on this grid (scratch owned by the handle, written by wpcd_perm_count,
+    // consumed by wpcd_perm_build): one slot per box-test candidate.  Mutable: the calls take a const handle (the lattice
+    // does not change); include/wpcd.h says that count and build on one handle must not overlap in time.
+    mutable int32_t* stage_col = nullptr;       // [stage_cap]  column index, or -1 for a rejected candidate
+    mutable double4* stage_ext = nullptr;       // [stage_cap]  vertices of smallest / largest polar angle of Pi (survivors)
+    int32_t* stage_off = nullptr;               // [n_p*n_q]    first slot of a geometric row
+    int32_t* stage_len = nullptr;               // [n_p*n_q]    number of candidates of a geometric row
+    int32_t* ctrl = nullptr;                    // [4] device: slot cursor, overflow flag, nnz_geo
+    int32_t* ctrl_pinned = nullptr;             // [4] pinned host copy
+    mutable cudaEvent_t count_event = nullptr;  // behind the read-back of the selection result
+    mutable cudaEvent_t rowptr_event = nullptr; // behind the row-pointer expansion of the last count
+    mutable cudaStream_t count_stream = nullptr;
+    mutable int64_t stage_cap = 0;
+    mutable bool stage_valid = false;
+    mutable bool select_ready = false;          // kernel attributes set
+    mutable int64_t stage_nnz_geo = 0;
 };
 
 // ---- tables of the coupled-channel fill --------------------------
@@ -152,8 +153,8 @@ struct Workspace {
 Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base);
 
 // pattern.cu  (compiled with -fmad=false: the predicate is an IEEE contract)
-cudaError_t ensure_stage(wpcd_grid* g, int64_t want_cap);
-cudaError_t launch_geo_select(wpcd_grid* g, int32_t* geo_row_ptr_dev /* out: ptr */, cudaStream_t st);
+cudaError_t ensure_stage(const wpcd_grid* g, int64_t want_cap);
+cudaError_t launch_geo_select(const wpcd_grid* g, int32_t* geo_row_ptr_dev /* out: ptr */, cudaStream_t st);
 cudaError_t launch_rowptr(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr_dev, int64_t* row_ptr_dev,
                           cudaStream_t st);
 cudaError_t launch_geo_gather(const wpcd_grid* g, const int32_t* geo_row_ptr_dev, int32_t* geo_col, int32_t* geo_row,

@@ -15,8 +15,10 @@ import numpy as np
 from numpy.polynomial.legendre import leggauss, legval
 
 
-def element(a, b, c, d, L1, U1, L2, U2, l, lp, terms, m=240):
-    """terms: [(k, l1, l1', g)].  m x m midpoint cells in (q,q')."""
+def element(a, b, c, d, L1, U1, L2, U2, l, lp, terms, m=240, modulus=False):
+    """terms: [(k, l1, l1', g)].  m x m midpoint cells in (q,q').
+    modulus=True: every term's integrand is replaced by its modulus (|g| |P_k(x)|, everything else in (A7) is positive):
+    the absolute term sum that the oracle reports as `absval` (the scale A_e of DESIGN.md R9)."""
     hq, hqp = (b - a) / m, (d - c) / m
     q = a + (np.arange(m) + 0.5) * hq
     qp = c + (np.arange(m) + 0.5) * hqp
@@ -39,7 +41,8 @@ def element(a, b, c, d, L1, U1, L2, U2, l, lp, terms, m=240):
         for (k, l1, l1p, g) in terms:
             A = l1 + l1p
             B = (l - l1) + (lp - l1p)
-            G += g * Q ** (A + 1) * QP ** (B + 1) * legval(x, [0.0] * k + [1.0])
+            Pk = legval(x, [0.0] * k + [1.0])
+            G += (abs(g) * np.abs(Pk) if modulus else g * Pk) * Q ** (A + 1) * QP ** (B + 1)
         total += np.sum(w[r] * half * G / (pi1 ** (lp + 1) * pi2 ** (l + 1)))
     return total * hq * hqp / np.sqrt((U2 - L2) * (b - a) * (U1 - L1) * (d - c))
 

@@ -1,10 +1,18 @@
 """GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
 element.  Pattern (row_ptr, col_idx) bit-exact; values within
     1e-11 * max(|v|, A_e) + 1e-13 * V
-where A_e is the element's absolute-sum scale computed by the oracle and V = max|v| of the
+where A_e is the element's absolute-sum scale computed by the oracle (pinned by tests/test_oracle_perm.py:
+test_absval_against_cartesian_modulus, test_fp64_oracle_against_its_long_double_twin) and V = max|v| of the
 matrix: the floor covers the ill-conditioned sliver elements next to the pi1 = 0 / pi2 = 0
 corners, where rule R(n) itself is only ~1e-8 accurate in double precision (R9).
-SpMV within 1e-12 * sum_j |a_ij x_j|."""
+On top of it every WELL-CONDITIONED entry (A_e < 10 |v|: no cancellation between the terms) must agree to a plain
+relative 1e-11, and each comparison records its worst error / tolerance and the histogram of the plain relative errors
+(SURVEY 8(c)9); with WPCD_PARITY_REPORT=<file> the records are appended to that file (tests/parity_report.py turns them
+into profiles/r02_parity.md).  SpMV within 1e-12 * sum_j |a_ij x_j|."""
+import json
+import os
+import sys
+
 import numpy as np
 import pytest
 
@@ -16,6 +24,57 @@ pytestmark = pytest.mark.gpu
 
 VALUE_RTOL = 1e-11
 VALUE_FLOOR = 1e-13   # times max|v| of the matrix
+WELL_CONDITIONED = 10.0   # A_e / |v| below this: the plain relative error must be within VALUE_RTOL
+_HIST_EDGES = [0.0, 1e-15, 1e-14, 1e-13, 1e-12, 1e-11, 1e-10, 1e-9, 1e-6, 1e-3, np.inf]
+
+
+class _ValueCheck:
+    """Accumulates the element-by-element comparison of one test (possibly over several row samples)."""
+
+    def __init__(self, tag):
+        self.tag = tag
+        self.n = self.n_well = 0
+        self.worst = self.worst_well_rel = self.worst_rel = 0.0
+        self.hist = np.zeros(len(_HIST_EDGES) - 1, np.int64)
+        self.hist_well = np.zeros(len(_HIST_EDGES) - 1, np.int64)
+
+    def add(self, gv, v, av, vmax, where=""):
+        err = np.abs(gv - v)
+        tol = VALUE_RTOL * np.maximum(np.abs(v), av) + VALUE_FLOOR * vmax
+        ratio = err / np.maximum(tol, 1e-300)
+        assert np.all(np.isfinite(gv)), where
+        assert np.all(err <= tol), f"{self.tag} {where}: worst err/tol = {ratio.max()}"
+        nz = np.abs(v) > 0
+        rel = err[nz] / np.abs(v[nz])
+        well = av[nz] < WELL_CONDITIONED * np.abs(v[nz])
+        # an entry without cancellation between its terms: plain relative error (the floor only where |v| is far below V)
+        bad = well & (rel > VALUE_RTOL) & (err[nz] > VALUE_FLOOR * vmax)
+        assert not bad.any(), f"{self.tag} {where}: {bad.sum()} well-conditioned entries beyond {VALUE_RTOL} relative, worst {rel[bad].max()}"
+        self.n += int(err.size); self.n_well += int(well.sum())
+        self.worst = max(self.worst, float(ratio.max()) if err.size else 0.0)
+        if rel.size:
+            self.worst_rel = max(self.worst_rel, float(rel.max()))
+            self.hist += np.histogram(rel, bins=_HIST_EDGES)[0]
+        if well.any():
+            self.worst_well_rel = max(self.worst_well_rel, float(rel[well].max()))
+            self.hist_well += np.histogram(rel[well], bins=_HIST_EDGES)[0]
+
+    def close(self, **extra):
+        rec = {"test": self.tag, "entries": self.n, "well_conditioned": self.n_well, "worst_err_over_tol": self.worst,
+               "worst_rel_err_well_conditioned": self.worst_well_rel, "worst_rel_err": self.worst_rel,
+               "hist_edges": [e if np.isfinite(e) else "inf" for e in _HIST_EDGES],
+               "hist_rel_err": self.hist.tolist(), "hist_rel_err_well_conditioned": self.hist_well.tolist()}
+        rec.update(extra)
+        print("PARITY " + json.dumps(rec))
+        path = os.environ.get("WPCD_PARITY_REPORT")
+        if path:
+            with open(path, "a") as f:
+                f.write(json.dumps(rec) + "\n")
+        return self.worst
+
+
+def _caller():
+    return sys._getframe(2).f_code.co_name
 
 
 def _torch():
@@ -40,7 +99,7 @@ def _gpu_channels(wpcd, wl, two_J=None, parity=None):
     return wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=wl.j_pair_max)
 
 
-def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None, split=False):
+def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None, split=False, tag=None):
     grid = wpcd.wpcd_grid_create(p, q)
     flag = {0: 0, 1: wpcd.WPCD_RULE_KINK_SPLIT, 2: wpcd.WPCD_RULE_ANALYTIC_U}[int(split)]
     m = wpcd.build_perm(grid, gch, n_quad | flag)
@@ -54,10 +113,9 @@ def _compare_full(wpcd, p, q, n_quad, gch, tab, geo_rows=None, split=False):
     gv = m.values.cpu().numpy()
     sel = ~np.isnan(v)
     assert sel.any()
-    err = np.abs(gv[sel] - v[sel])
-    tol = VALUE_RTOL * np.maximum(np.abs(v[sel]), av[sel]) + VALUE_FLOOR * np.abs(v[sel]).max()
-    worst = np.max(err / np.maximum(tol, 1e-300)) if len(err) else 0.0
-    assert np.all(err <= tol), f"worst err/tol = {worst}"
+    chk = _ValueCheck(tag or _caller())
+    chk.add(gv[sel], v[sel], av[sel], np.abs(v[sel]).max())
+    chk.close(n_p=len(p) - 1, n_q=len(q) - 1, n_quad=n_quad, rule=int(split), nnz=int(m.nnz))
     assert np.all(np.isfinite(gv))
     return m, (rp, ci, v, av)
 
@@ -188,7 +246,7 @@ def test_fp64_peak_microbenchmark(wpcd):
 
 
 # ----------------------------------------------------------------------------- coupled channels
-def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows):
+def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows, tag=None):
     """Full row_ptr + geometric pattern, and col_idx / values on the sampled geometric rows
     (all channels), without materialising the oracle's full CSR (configs 3-5 sizes)."""
     torch = _torch()
@@ -212,7 +270,7 @@ def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows):
     pair_of[tab.gamma, tab.gammap] = np.arange(tab.n_pairs)
     vmax = np.abs(val).max()
     off = np.concatenate([[0], np.cumsum(cnt)])
-    worst = 0.0
+    chk = _ValueCheck(tag or _caller())
     # the products of the full-size matrix (general CSR kernel and the blocked one) on the sampled rows: the oracle's row
     # values times x, summed by the oracle side; the tolerance carries the value tolerance through the sum
     rows_all = m.rows
@@ -236,13 +294,12 @@ def _compare_sampled(wpcd, p, n_quad, gch, tab, geo_rows):
             ea = aval[off[ri]:off[ri + 1]][:, pair_of[g, coupled]].T.reshape(-1)
             gv = m.values[lo:hi].cpu().numpy()
             tol = VALUE_RTOL * np.maximum(np.abs(ev), ea) + VALUE_FLOOR * vmax
-            err = np.abs(gv - ev)
-            worst = max(worst, float(np.max(err / tol)))
-            assert np.all(err <= tol), f"channel {g} geo row {r}: worst err/tol {np.max(err / tol)}"
+            chk.add(gv, ev, ea, vmax, where=f"channel {g} geo row {r}")
             xs = xh[exp_cols]
             y_ref = float(np.dot(ev, xs))
             y_tol = float(np.dot(tol, np.abs(xs))) + 1e-12 * float(np.dot(np.abs(ev), np.abs(xs)))
             assert abs(y_csr[g * n_geo + r] - y_ref) <= y_tol and abs(y_blk[g * n_geo + r] - y_ref) <= y_tol, (g, r)
+    worst = chk.close(n_p=n, n_q=n, n_quad=n_quad, rule=0, nnz=int(m.nnz), sampled_geo_rows=int(len(geo_rows)), channels=int(tab.n_ch))
     return m, worst
 
 
@@ -266,34 +323,134 @@ def test_coupled_from_table_matches_builtin(wpcd):
     _compare_full(wpcd, p, p, 8, gch, tab)
 
 
-def test_cfg3_nd_half_plus_sampled(wpcd):
+def test_cfg3_nd_half_plus_full(wpcd):
+    """Config 3 (N = 100, J^pi = 1/2+, j <= 2: 18 channels, 7.9e7 nonzeros): pattern AND values of the whole matrix against
+    the oracle (values compared in full on configs 1-3), and the products of the CSR and the blocked kernel on
+    the whole matrix against the oracle's sequential product of the GPU values."""
+    torch = _torch()
     wl = wi.WORKLOADS["cfg3"]
     (two_J, parity), = wl.jpis
     p = wl.grid()
+    n = wl.n_bins
+    n_geo = n * n
     tab = _oracle_table(wl, two_J, parity)
     assert tab.n_ch == 18
-    m, worst = _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, two_J, parity), tab,
-                                np.arange(7, wl.n_bins ** 2, 61))
+    gch = _gpu_channels(wpcd, wl, two_J, parity)
+    grid = wpcd.wpcd_grid_create(p, p)
+    m = wpcd.build_perm(grid, gch, wl.n_quad)
+    torch.cuda.synchronize()
     assert m.rows == 18 * 100 * 100
+    geo_ptr, geo_col = operm.geo_pattern(p, p)
+    assert np.array_equal(m.geo_row_ptr.cpu().numpy().astype(np.int64), geo_ptr)
+    rp = operm.full_row_ptr(geo_ptr, tab, n, n)
+    assert np.array_equal(m.row_ptr.cpu().numpy(), rp) and m.nnz == rp[-1]
+    erow = np.repeat(np.arange(n_geo), np.diff(geo_ptr))
+    val, aval = operm.element_values(p, p, erow // n, erow % n, geo_col // n, geo_col % n, wl.n_quad, tab)     # [nnz_geo, pairs]
+    gv, gci = m.values.cpu().numpy(), m.col_idx.cpu().numpy()
+    pair_of = -np.ones((tab.n_ch, tab.n_ch), np.int64)
+    pair_of[tab.gamma, tab.gammap] = np.arange(tab.n_pairs)
+    cnt_e, pos_e = (geo_ptr[erow + 1] - geo_ptr[erow]), np.arange(len(erow)) - geo_ptr[erow]
+    vmax = np.abs(val).max()
+    chk = _ValueCheck("test_cfg3_nd_half_plus_full")
+    for g in range(tab.n_ch):
+        coupled = np.nonzero(tab.mask[g])[0]
+        for t, gp in enumerate(coupled):
+            dst = rp[g * n_geo + erow] + t * cnt_e + pos_e                 # where entry (g, r; gp, c) sits in the CSR
+            assert np.array_equal(gci[dst], gp * n_geo + geo_col)
+            chk.add(gv[dst], val[:, pair_of[g, gp]], aval[:, pair_of[g, gp]], vmax, where=f"pair ({g},{gp})")
+    chk.close(n_p=n, n_q=n, n_quad=wl.n_quad, rule=0, nnz=int(m.nnz), channels=18)
+    del val, aval
+    xh = wi.normal_vector(m.rows, k=333)
+    xd = torch.from_numpy(xh).cuda()
+    y_csr, y_blk = torch.empty_like(xd), torch.empty_like(xd)
+    wpcd.wpcd_perm_apply(m.rows, m.row_ptr, m.col_idx, m.values, xd, y_csr)
+    wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, xd, y_blk)
+    ref = operm.spmv(rp, gci, gv, xh)
+    scale = operm.spmv(rp, gci, np.abs(gv), np.abs(xh))
+    assert np.all(np.abs(y_csr.cpu().numpy() - ref) <= 1e-12 * scale + 1e-300)
+    assert np.all(np.abs(y_blk.cpu().numpy() - ref) <= 1e-12 * scale + 1e-300)
 
 
-def test_cfg4_sampled(wpcd):
+@pytest.mark.parametrize("two_J,parity,stride", [(1, 1, 397), (1, -1, 523), (3, 1, 1499), (3, -1, 1301)])
+def test_cfg4_sampled(wpcd, two_J, parity, stride):
+    """Config 4 (N = 150, j <= 3): all four J^pi matrices, full pattern, sampled geometric rows of every channel."""
     wl = wi.WORKLOADS["cfg4"]
     p = wl.grid()
-    for (two_J, parity), stride in [((1, 1), 397), ((3, -1), 1499)]:
-        tab = _oracle_table(wl, two_J, parity)
-        _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, two_J, parity), tab,
-                         np.arange(11, wl.n_bins ** 2, stride))
+    tab = _oracle_table(wl, two_J, parity)
+    _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, two_J, parity), tab, np.arange(11, wl.n_bins ** 2, stride),
+                     tag=f"test_cfg4_sampled[{two_J}/2,{'+' if parity > 0 else '-'}]")
 
 
-def test_cfg5_largest_sampled(wpcd):
-    # J = 7/2, parity -: the largest matrix of config 5 (62 channels, ~2.8e9 nonzeros, ~34 GB)
+@pytest.mark.parametrize("two_J,parity,stride", [(1, 1, 1201), (1, -1, 1103), (3, 1, 1801), (3, -1, 1709), (5, 1, 2399), (5, -1, 2203),
+                                                 (7, 1, 2609), (7, -1, 2503)])
+def test_cfg5_sampled(wpcd, two_J, parity, stride):
+    """Config 5 (N = 150, j <= 3): all eight J^pi matrices; 7/2- is the largest (62 channels, 3.2e9 nonzeros, 39 GB: offsets
+    beyond 2^31)."""
     wl = wi.WORKLOADS["cfg5"]
     p = wl.grid()
-    tab = _oracle_table(wl, 7, -1)
-    m, worst = _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, 7, -1), tab,
-                                np.arange(5, wl.n_bins ** 2, 2503))
-    assert m.nnz > 2_000_000_000
+    tab = _oracle_table(wl, two_J, parity)
+    m, worst = _compare_sampled(wpcd, p, wl.n_quad, _gpu_channels(wpcd, wl, two_J, parity), tab, np.arange(5, wl.n_bins ** 2, stride),
+                                tag=f"test_cfg5_sampled[{two_J}/2,{'+' if parity > 0 else '-'}]")
+    if (two_J, parity) == (7, -1):
+        assert m.nnz > 2_000_000_000
+
+
+@pytest.mark.parametrize("two_J,parity,jmax,nb,n", [(7, -1, 3, 8, 10), (1, 1, 2, 12, 8), (5, 1, 3, 6, 10)])
+def test_first_bin_cells_against_extended_precision(wpcd, two_J, parity, jmax, nb, n):
+    """on cells that touch p = 0 or p' = 0 the single (k,l1,l1') terms of pairs with l, l' >= 2 are huge and
+    only their sum is small.  The oracle sums the terms per node, the CUDA path integrates monomial moments first and
+    contracts with g afterwards (R8).  Against the SAME rule evaluated in long double (oracle built with
+    -DWPO_EXTENDED) the CUDA values must be no further off than FP64 rounding of the absolute term sum allows, and not
+    systematically worse than the FP64 oracle's own per-node sum: the moments-then-contract schedule loses no digits."""
+    torch = _torch()
+    chs = och.enumerate_channels(two_J, parity, jmax)
+    tab = operm.PairTable(chs, och.g_table(chs, two_J, 1))
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=two_J, parity=parity, two_T=1, j_pair_max=jmax)
+    p = wi.tan2_grid(nb)
+    grid = wpcd.wpcd_grid_create(p, p)
+    m = wpcd.build_perm(grid, gch, n)
+    torch.cuda.synchronize()
+    geo_ptr, geo_col = operm.geo_pattern(p, p)
+    n_geo = nb * nb
+    erow = np.repeat(np.arange(n_geo), np.diff(geo_ptr))
+    v64, a64 = operm.element_values(p, p, erow // nb, erow % nb, geo_col // nb, geo_col % nb, n, tab)
+    vex, _ = operm.element_values(p, p, erow // nb, erow % nb, geo_col // nb, geo_col % nb, n, tab, extended=True)
+    rp = operm.full_row_ptr(geo_ptr, tab, nb, nb)
+    gv = m.values.cpu().numpy()
+    cnt_e, pos_e = (geo_ptr[erow + 1] - geo_ptr[erow]), np.arange(len(erow)) - geo_ptr[erow]
+    vg = np.empty_like(v64)
+    for c in range(tab.n_pairs):
+        g, gp = tab.gamma[c], tab.gammap[c]
+        t = int(np.nonzero(np.nonzero(tab.mask[g])[0] == gp)[0][0])
+        vg[:, c] = gv[rp[g * n_geo + erow] + t * cnt_e + pos_e]
+    first_bin = ((erow // nb == 0) | (geo_col // nb == 0))[:, None] & ((tab.pair_l >= 2) & (tab.pair_lp >= 2))[None, :]
+    assert first_bin.sum() > 100
+    eps = 2.0 ** -53
+    e_gpu, e_64 = np.abs(vg - vex)[first_bin], np.abs(v64 - vex)[first_bin]
+    ae, vx = a64[first_bin], np.abs(vex)[first_bin]
+    cond = ae / np.maximum(vx, 1e-300)
+    assert np.median(cond) > 10 and cond.max() > 1e6                   # these ARE the ill-conditioned entries
+    # entry by entry: a few dozen roundings of the absolute sum, with the same constant for both FP64 evaluations
+    # (measured worst: 13 eps A_e on the device, 9.6 eps A_e for the oracle; the parity tolerance 1e-11 A_e is 9e4 eps A_e)
+    assert np.all(e_64 <= 64 * eps * ae) and np.all(e_gpu <= 64 * eps * ae), (np.max(e_64 / (eps * ae)), np.max(e_gpu / (eps * ae)))
+    # entry by entry against the oracle's own deviation: |v_gpu - v_ext| <= 1e-11 |v_ext| + c max(|v_64 - v_ext|, eps A_e)
+    bound = 1e-11 * vx + 64.0 * np.maximum(e_64, eps * ae)
+    assert np.all(e_gpu <= bound), np.max(e_gpu / bound)
+    # on the whole: the CUDA schedule is not worse than the per-node sum (rms of the errors in units of eps A_e)
+    rms_gpu, rms_64 = np.sqrt(np.mean((e_gpu / (eps * ae)) ** 2)), np.sqrt(np.mean((e_64 / (eps * ae)) ** 2))
+    print("PARITY " + json.dumps({"test": "test_first_bin_cells_against_extended_precision", "J2": two_J, "parity": parity, "n_bins": nb,
+                                  "entries": int(first_bin.sum()), "median_cond": float(np.median(cond)), "max_cond": float(cond.max()),
+                                  "rms_err_gpu_eps_Ae": float(rms_gpu), "rms_err_oracle64_eps_Ae": float(rms_64),
+                                  "max_err_gpu_eps_Ae": float(np.max(e_gpu / (eps * ae))), "max_err_oracle64_eps_Ae": float(np.max(e_64 / (eps * ae)))}))
+    path = os.environ.get("WPCD_PARITY_REPORT")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps({"test": "first_bin_extended", "J2": two_J, "parity": parity, "n_bins": nb, "entries": int(first_bin.sum()),
+                                "median_cond": float(np.median(cond)), "max_cond": float(cond.max()), "rms_err_gpu_eps_Ae": float(rms_gpu),
+                                "rms_err_oracle64_eps_Ae": float(rms_64), "max_err_gpu_eps_Ae": float(np.max(e_gpu / (eps * ae))),
+                                "max_err_oracle64_eps_Ae": float(np.max(e_64 / (eps * ae)))}) + "\n")
+    # measured: 1.0 - 1.2 eps A_e on the device (moments in FP64 MMA order, then the contraction), 0.3 - 0.5 for the per-node sum
+    assert rms_gpu <= 2.5 and rms_gpu <= 6.0 * rms_64
 
 
 def test_coupled_wide_classes_from_table(wpcd):
@@ -609,6 +766,72 @@ def test_count_and_build_on_different_streams(wpcd):
         s_build.synchronize()
         s_count.synchronize()
         assert torch.equal(row_ptr, ref.row_ptr) and torch.equal(col_idx, ref.col_idx) and torch.equal(values, ref.values)
+
+
+def test_concurrent_builds_of_different_orders(wpcd):
+    """Two builds with different quadrature orders (8 and 10: configs 1-3 and 4-5) in flight at the same time on two
+    streams and two grid handles: each launch carries its own rule, so neither disturbs the other (the rule
+    used to sit in one __constant__ bank per translation unit)."""
+    torch = _torch()
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=2)
+    sw = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    p = wi.tan2_grid(30, 1.0, 0.1, seed=77)
+    for ch in (gch, sw):
+        grids = [wpcd.wpcd_grid_create(p, p), wpcd.wpcd_grid_create(p, p)]
+        refs = [wpcd.build_perm(grids[0], ch, 8), wpcd.build_perm(grids[1], ch, 10)]
+        torch.cuda.synchronize()
+        assert not torch.equal(refs[0].values, refs[1].values)
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        for _ in range(4):
+            outs = []
+            for k, nq in enumerate((8, 10)):
+                rp, geo = torch.empty_like(refs[k].row_ptr), torch.empty_like(refs[k].geo_row_ptr)
+                nnz, nnz_geo = wpcd.wpcd_perm_count(grids[k], ch, nq, rp, geo, streams[k])
+                ws = torch.empty(max(wpcd.wpcd_perm_workspace_bytes(ch, nnz_geo), 256), dtype=torch.uint8, device="cuda")
+                outs.append((rp, geo, ws, torch.zeros(nnz, dtype=torch.int32, device="cuda"), torch.zeros(nnz, dtype=torch.float64, device="cuda")))
+            torch.cuda.synchronize()
+            for rep in range(3):                  # several builds back to back on both streams, interleaved from the host
+                for k, nq in enumerate((8, 10)):
+                    rp, geo, ws, ci, va = outs[k]
+                    wpcd.wpcd_perm_build(grids[k], ch, nq, rp, geo, ws, ci, va, streams[k])
+            torch.cuda.synchronize()
+            for k in range(2):
+                assert torch.equal(outs[k][3], refs[k].col_idx) and torch.equal(outs[k][4], refs[k].values), k
+
+
+def test_apply_ignores_columns_a_row_does_not_reference(wpcd):
+    """x[0] = inf / nan must not leak into rows that do not reference column 0 (padding slots of the batched loads used to
+    multiply 0 * x[0]); every product variant, short and long rows."""
+    torch = _torch()
+    rng = np.random.default_rng(5)
+    for rows, short, long_ in ((300, 3, 70), (400, 9, 300)):
+        lens = np.full(rows, short, dtype=np.int64)
+        lens[::5] = long_
+        rp = np.zeros(rows + 1, dtype=np.int64)
+        rp[1:] = np.cumsum(lens)
+        nnz = int(rp[-1])
+        ci = rng.integers(1, rows, nnz).astype(np.int32)          # no entry in column 0
+        v = rng.standard_normal(nnz)
+        rpd, cid, vd = torch.from_numpy(rp).cuda(), torch.from_numpy(ci).cuda(), torch.from_numpy(v).cuda()
+        for bad in (np.inf, np.nan):
+            xs = np.stack([wi.normal_vector(rows, k=40 + k) for k in range(4)])
+            xs[:, 0] = bad
+            x = torch.from_numpy(xs).cuda()
+            for n_vec in (1, 2, 4):
+                y = torch.empty(n_vec, rows, dtype=torch.float64, device="cuda")
+                wpcd.wpcd_perm_apply(rows, rpd, cid, vd, x[:n_vec].contiguous(), y, n_vec)
+                assert torch.isfinite(y).all()
+            xc = torch.from_numpy((xs[0] + 1j * xs[1])[None, :].copy()).cuda()
+            yc = torch.empty_like(xc)
+            wpcd.wpcd_perm_apply_complex(rows, rpd, cid, vd, xc, yc, 1)
+            assert torch.isfinite(torch.view_as_real(yc)).all()
+            xi = torch.from_numpy(np.ascontiguousarray(xs.T)).cuda()
+            yi = torch.empty_like(xi)
+            wpcd.wpcd_perm_apply_interleaved(rows, rpd, cid, vd, xi, yi)
+            assert torch.isfinite(yi).all()
+            ych = torch.empty(3, rows, dtype=torch.float64, device="cuda")
+            wpcd.wpcd_perm_apply_chain(rows, rpd, cid, vd, x[0].contiguous(), ych, 1)
+            assert torch.isfinite(ych[0]).all()
 
 
 def test_apply_interleaved(wpcd):

@@ -83,6 +83,64 @@ def test_elements_against_cartesian_A7_multichannel(nd_half_plus_j1):
             assert abs(v[n_e, c] - ref) < 1e-2 * max(av[n_e, c], 1e-3), (c, e)
 
 
+def test_absval_against_cartesian_modulus(nd_half_plus_j1):
+    """Pins A_e (`absval`), the scale of every coupled-channel value tolerance (R9): it must be the same integral
+    with each term's integrand replaced by its modulus -- evaluated here from the unreduced Cartesian form (A7) -- and for a
+    pair with a single k = 0 term it must equal |value| exactly.  Catches an inflated or deflated scale (a modulus taken
+    of the sum instead of the terms, a dropped factor, terms counted twice)."""
+    tab = nd_half_plus_j1
+    p = wi.tan2_grid(3, 1.0, 0.1, seed=5)
+    q = wi.tan2_grid(3, 0.8, 0.1, seed=6)
+    ptr, col = perm.geo_pattern(p, q)
+    n_q = len(q) - 1
+    rows = np.repeat(np.arange(len(ptr) - 1), np.diff(ptr))
+    sel = [e for e in range(len(col)) if min(rows[e] // n_q, col[e] // n_q) >= 1][:6]
+    v, av = perm.element_values(p, q, rows[sel] // n_q, rows[sel] % n_q, col[sel] // n_q, col[sel] % n_q, 48, tab)
+    assert np.all(av >= np.abs(v) * (1 - 1e-12))
+    n_terms = np.diff(tab.term_ptr)
+    # pairs whose terms cancel (several terms of both signs): there A_e differs from |v| and only the modulus integral fixes it
+    many = [c for c in range(tab.n_pairs) if n_terms[c] >= 3 and min(tab.pair_l[c], tab.pair_lp[c]) >= 1][:4]
+    many += [c for c in range(tab.n_pairs) if n_terms[c] >= 3 and tab.pair_l[c] == 2 and tab.pair_lp[c] == 0][:2]
+    assert len(many) >= 4
+    ratios = []
+    for c in many:
+        terms = [(tab.term_k[t], tab.term_l1[t], tab.term_l1p[t], tab.term_g[t]) for t in range(tab.term_ptr[c], tab.term_ptr[c + 1])]
+        for n_e, e in enumerate(sel):
+            i, j, ip, jp = rows[e] // n_q, rows[e] % n_q, col[e] // n_q, col[e] % n_q
+            ref = brute.element(q[j], q[j + 1], q[jp], q[jp + 1], p[ip], p[ip + 1], p[i], p[i + 1],
+                                int(tab.pair_l[c]), int(tab.pair_lp[c]), terms, m=120, modulus=True)
+            assert abs(av[n_e, c] - ref) < 1e-2 * max(ref, 1e-3), (c, e, av[n_e, c], ref)
+            ratios.append(av[n_e, c] / max(abs(v[n_e, c]), 1e-300))
+    assert max(ratios) > 1.5            # the sample does contain cancelling pairs (the pin is not vacuous)
+    # single-term pairs with k = 0 (P_0 = 1 > 0, every other factor positive): the modulus changes nothing
+    single = [c for c in range(tab.n_pairs) if n_terms[c] == 1 and tab.term_k[tab.term_ptr[c]] == 0]
+    assert single
+    assert np.array_equal(av[:, single], np.abs(v[:, single]))
+
+
+@pytest.mark.parametrize("two_J,parity,jmax,nb,n", [(1, 1, 2, 12, 8), (7, -1, 3, 8, 10)])
+def test_fp64_oracle_against_its_long_double_twin(two_J, parity, jmax, nb, n):
+    """The same source compiled with -DWPO_EXTENDED evaluates rule R(n) in long double.  The FP64 oracle must agree with
+    it to FP64 rounding of the ABSOLUTE term sum: |v64 - v80| <= 3e-12 A_e (measured worst 7e-13: sliver elements, whose
+    integration limits move with the rounding of the polygon angles) -- also on the first-bin cells where single
+    terms are huge and the value is small by cancellation, where the plain relative error is O(1).  Fixes the
+    meaning of A_e once more (an A_e too small by a factor would fail here) and bounds the oracle's own rounding, which the
+    GPU tolerance 1e-11 A_e has to cover with room to spare."""
+    chs = channels.enumerate_channels(two_J, parity, jmax)
+    tab = perm.PairTable(chs, channels.g_table(chs, two_J, 1))
+    p = wi.tan2_grid(nb)
+    ptr, col = perm.geo_pattern(p, p)
+    rows = np.repeat(np.arange(nb * nb), np.diff(ptr))
+    v, a = perm.element_values(p, p, rows // nb, rows % nb, col // nb, col % nb, n, tab)
+    ve, ae = perm.element_values(p, p, rows // nb, rows % nb, col // nb, col % nb, n, tab, extended=True)
+    assert np.all(np.abs(a - ae) <= 1e-11 * ae)
+    err = np.abs(v - ve)
+    assert np.all(err <= 3e-12 * a + 1e-300)
+    # the ill-conditioned entries are there: relative errors far above 1e-11 although err / A_e stays at rounding level
+    rel = err / np.maximum(np.abs(ve), 1e-300)
+    assert rel.max() > 1e-9 and np.median(rel) < 1e-13
+
+
 @pytest.fixture(scope="module")
 def swave_matrices(swave_table):
     out = {}

@@ -64,7 +64,7 @@ __host__ __device__ inline int moment_smem_doubles(const MomentShape& s)
 // b = B[lane%4][lane/4], (c0, c1) = C[lane/4][2 (lane%4) + {0,1}].
 __device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, double b)
 {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
 // I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] for one phi-node: (K1 x n) (n x n_ll) in 8x8x4 MMAs.
@@ -101,7 +101,7 @@ __device__ __forceinline__ double ipow_small(double b, int e)   // e < 64
 // Moment layout: element-major, moments[element - e_begin][mu] (coalesced stores here; the contraction stages the
 // contiguous range of one l-group per element).
 template <int MAXS, bool SPLIT>
-__global__ void __launch_bounds__(MOM_MAX_WARPS * 32)
+__global__ void __launch_bounds__(MOM_MAX_WARPS * 32, 16)
 moments_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape sh,
                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
@@ -313,6 +313,177 @@ moments_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__
         if (lane + 32 * s < n_mu) out[lane + 32 * s] = acc[s];
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// moments2_kernel -- the same moments for the plain rule R(n), 5 <= n <= 12, k_max <= 15: the production path.
+// One warp per geometric element.  Differences from moments_kernel (kept for the kink-split rule and the other orders):
+//   * the tables are stored TRANSPOSED, [quantity][node slot]: the lanes that set up the nodes write consecutive words,
+//     and with a row stride = 4 (mod 16) the MMA fragment loads are conflict-free as well;
+//   * T[l,l'] = wF zeta2^{-(l+1)} zeta1^{-(l'+1)} is never stored: two small power tables pa[l] = wF zeta2^{-(l+1)},
+//     pb[l'] = zeta1^{-(l'+1)} (2 (l_max+1) values per node instead of (l_max+1)^2) and one multiply when a B fragment
+//     is formed; node slots are padded to a multiple of 4 per phi-node with zeros, so no fragment needs a mask;
+//   * B fragments are formed once per (n-tile, k-step) and used for every m-tile; the MMAs are free to interleave.
+struct MomentShape2 {
+    int n;        // quadrature order
+    int G;        // phi-nodes whose x-nodes are set up together (G n <= 32 lanes)
+    int NP;       // node slots per phi-node: n rounded up to a multiple of 4 (KT = NP / 4 k-steps)
+    int RS;       // row stride of the transposed tables: >= G NP, = 4 (mod 16)
+    int K1;       // k_max + 1
+    int NT;       // n-tiles: ceil(n_ll / 8)
+    int IS;       // row stride of the I table: 8 NT + 2
+    int LM1;      // l_max + 1
+    int CP;       // 2 l_max + 3 powers of cos / sin
+    int n_ab, n_ll, n_mu;
+};
+
+__host__ __device__ inline int moment2_smem_doubles(const MomentShape2& s)
+{
+    // phi-node records | P_k [K1][RS] | pa [LM1][RS] | pb [LM1][RS] | I [K1][IS] | cos/sin powers [G][2][CP] | c^a s^b [n_ab]
+    return (s.n * NODE_F + s.K1 * s.RS + 2 * s.LM1 * s.RS + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;
+}
+
+template <int MAXS, int KT, int MT>
+__global__ void __launch_bounds__(32, 16)
+moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape2 sh,
+                int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
+                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
+                const int32_t* __restrict__ mu_pack, const int32_t* __restrict__ ab_pack, double* __restrict__ moments)
+{
+    extern __shared__ double sm[];
+    const int lane = threadIdx.x, quad = lane & 3, oct = lane >> 2;
+    const int n = sh.n, G = sh.G, NP = sh.NP, RS = sh.RS, K1 = sh.K1, NT = sh.NT, IS = sh.IS, LM1 = sh.LM1, CP = sh.CP, n_ab = sh.n_ab;
+    const int n_ll = sh.n_ll, n_mu = sh.n_mu;
+    const int64_t e = e_begin + blockIdx.x;
+    if (e >= e_end) return;
+    double* nodeS = sm;                       // [n][NODE_F]
+    double* Pt = nodeS + n * NODE_F;          // [K1][RS]   P_k(x) of node slot g NP + r
+    double* pa = Pt + K1 * RS;                // [LM1][RS]  wF zeta2^{-(l+1)}
+    double* pb = pa + LM1 * RS;               // [LM1][RS]  zeta1^{-(l'+1)}
+    double* Ib = pb + LM1 * RS;               // [K1][IS]   I[k][l,l'] of one phi-node
+    double* cs = Ib + K1 * IS;                // [G][2][CP] powers of cos, sin
+    double* csp = cs + G * 2 * CP;            // [n_ab]     c^a s^b of one phi-node
+    // the padding slots of the power tables must read as zero (they feed the MMAs); P_k only has to be finite there
+    for (int i = lane; i < (K1 + 2 * LM1) * RS; i += 32) Pt[i] = 0.0;
+    // per monomial: offset into Ib (low 16 bits) and into csp (high 16 bits)
+    int pk[MAXS];
+    double acc[MAXS];
+#pragma unroll
+    for (int s = 0; s < MAXS; ++s) {
+        const int m = lane + 32 * s;
+        acc[s] = 0.0;
+        pk[s] = -1;
+        if (m < n_mu) {
+            const int v = mu_pack[m], tp = trip_pack[v & 0xffff];
+            pk[s] = ((tp & 0xff) * IS + (tp >> 8)) | ((v >> 16) << 16);     // mu_pack: triple | ab index << 16
+        }
+    }
+    // this lane's (l, l') of every n-tile, as offsets of its power-table rows (-1: column beyond n_ll)
+    int la[4], lb[4];
+#pragma unroll
+    for (int nt = 0; nt < 4; ++nt) {
+        const int ll = nt * 8 + oct;
+        la[nt] = lb[nt] = -1;
+        if (nt < NT && ll < n_ll) { const int v = ll_pack[ll]; la[nt] = (v & 0xff) * RS; lb[nt] = (v >> 8) * RS; }
+    }
+    const int col = geo_col[e], row = geo_row[e];
+    const double2 ph = geo_phi[e];
+    const Cell z = load_cell(p, q, n_q, row, col);
+    const CellSq zs = square_cell(z);
+    const double norm = cell_norm(z);
+    const double half_phi = 0.5 * (ph.y - ph.x), mid_phi = 0.5 * (ph.x + ph.y);
+    __syncwarp();
+    if (ph.x < ph.y) {
+        // ---- step 1: everything that depends on phi only, one lane per phi-node (weight 0: the node contributes nothing)
+        for (int m = lane; m < n; m += 32) {
+            PhiNodeSq s;
+            const bool ok = phi_node_sq(z, zs, mid_phi + half_phi * rule.xi[m], s);
+            double* o = nodeS + m * NODE_F;
+            o[0] = ok ? half_phi * rule.w[m] : 0.0; o[1] = s.C; o[2] = s.S; o[3] = s.Lq2; o[4] = s.Uq2;
+            o[5] = s.b1; o[6] = s.b2; o[7] = s.beta; o[8] = s.u_lo; o[9] = s.u_hi;
+        }
+        __syncwarp();
+        for (int m0 = 0; m0 < n; m0 += G) {
+            const int cnt = min(G, n - m0);
+            // ---- step 2: node set-up, lane = (phi-node g, x-node r) -> slot g NP + r of the transposed tables
+            if (lane < cnt * n) {
+                const int g = lane / n, r = lane - g * n, slot = g * NP + r;
+                const double* o = nodeS + (m0 + g) * NODE_F;
+                if (o[0] != 0.0) {
+                    PhiNodeSq s;
+                    s.Lq2 = o[3]; s.Uq2 = o[4];
+                    const double b1 = o[5], b2 = o[6], beta = o[7], u_lo = o[8], u_hi = o[9];
+                    const double half_u = 0.5 * (u_hi - u_lo), mid_u = 0.5 * (u_lo + u_hi);
+                    const double u = mid_u + half_u * rule.xi[r];
+                    const double x = u - 1.0;
+                    const double iz1 = rsqrt(b1 + beta * u), iz2 = rsqrt(b2 + beta * u);
+                    const double wF = (o[0] * norm) * (half_u * rule.w[r]) * 0.5 * twoF_A14_sq(zs, s, iz1 * iz1, iz2 * iz2);
+                    double p0 = 1.0, p1 = x;
+                    Pt[slot] = 1.0;
+                    if (K1 > 1) Pt[RS + slot] = x;
+                    for (int k = 2; k < K1; ++k) {
+                        const double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) * rule.invk[k];
+                        Pt[k * RS + slot] = p2;
+                        p0 = p1; p1 = p2;
+                    }
+                    double za = wF * iz2, zb = iz1;                   // wF zeta2^{-(l+1)}, zeta1^{-(l'+1)}
+                    for (int l = 0; l < LM1; ++l) {
+                        pa[l * RS + slot] = za; pb[l * RS + slot] = zb;
+                        za *= iz2; zb *= iz1;
+                    }
+                }
+            }
+            // powers of cos, sin of the group's phi-nodes: lane = (phi-node, cos | sin), running product
+            if (lane < 2 * cnt) {
+                const double base = nodeS[(m0 + (lane >> 1)) * NODE_F + 1 + (lane & 1)];
+                double* d = cs + lane * CP;
+                double pw = 1.0;
+                for (int ex = 0; ex < CP; ++ex) { d[ex] = pw; pw *= base; }
+            }
+            __syncwarp();
+            for (int g = 0; g < cnt; ++g) {
+                if (nodeS[(m0 + g) * NODE_F] == 0.0) continue;           // warp-uniform
+                // c^a s^b table of this phi-node
+                for (int idx = lane; idx < n_ab; idx += 32) {
+                    const int ab = ab_pack[idx];
+                    csp[idx] = cs[(g * 2 + 0) * CP + (ab & 0xff)] * cs[(g * 2 + 1) * CP + (ab >> 8)];
+                }
+                // ---- step 3: I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] on the FP64 tensor cores
+                const int s0 = g * NP + quad;                          // this lane's node slot of k-step 0
+                double a[MT][KT];
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                    for (int kt = 0; kt < KT; ++kt) a[mt][kt] = mt * 8 + oct < K1 ? Pt[(mt * 8 + oct) * RS + s0 + 4 * kt] : 0.0;
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) {
+                    if (nt >= NT) break;
+                    double b[KT];
+#pragma unroll
+                    for (int kt = 0; kt < KT; ++kt) b[kt] = la[nt] >= 0 ? pa[la[nt] + s0 + 4 * kt] * pb[lb[nt] + s0 + 4 * kt] : 0.0;
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                        for (int kt = 0; kt < KT; ++kt) dmma_884(c0, c1, a[mt][kt], b[kt]);
+                        if (mt * 8 + oct < K1) *reinterpret_cast<double2*>(Ib + (mt * 8 + oct) * IS + nt * 8 + 2 * quad) = make_double2(c0, c1);
+                    }
+                }
+                __syncwarp();
+                // ---- step 4: M[mu] += c^{A+1} s^{B+1} I[k][l,l'], lane = monomial
+#pragma unroll
+                for (int s = 0; s < MAXS; ++s) {
+                    const int v = pk[s];
+                    if (v >= 0) acc[s] = fma(csp[v >> 16], Ib[v & 0xffff], acc[s]);
+                }
+                __syncwarp();
+            }
+        }
+    }
+    double* out = moments + (size_t)(e - e_begin) * n_mu;       // element-major: one contiguous row per element
+#pragma unroll
+    for (int s = 0; s < MAXS; ++s)
+        if (lane + 32 * s < n_mu) out[lane + 32 * s] = acc[s];
+}
+
 }  // namespace
 
 namespace {
@@ -505,6 +676,14 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     if ((int64_t)ch->ct_ncoup_max * nnz_geo + nnz_geo >= (int64_t)INT32_MAX) return cudaErrorInvalidValue;
     const int n_geo = g->n_p * g->n_q;
     const int maxs = (ch->n_mu + 31) / 32;
+    // the production path (plain rule, 5 <= n <= 12, k_max <= 15, l_max <= 4, <= 640 monomials): moments2_kernel
+    MomentShape2 s2;
+    s2.n = n_quad; s2.G = std::max(1, std::min(32 / std::max(n_quad, 1), 4)); s2.NP = 4 * ((n_quad + 3) / 4);
+    s2.RS = s2.G * s2.NP; while (s2.RS % 16 != 4) ++s2.RS;
+    s2.K1 = ch->k_max + 1; s2.NT = (ch->n_ll + 7) / 8; s2.IS = 8 * s2.NT + 2; s2.LM1 = ch->l_max + 1; s2.CP = 2 * ch->l_max + 3;
+    s2.n_ab = ch->n_ab; s2.n_ll = ch->n_ll; s2.n_mu = ch->n_mu;
+    const bool fast = !split && n_quad >= 5 && n_quad <= 12 && s2.K1 <= 16 && s2.NT <= 4 && maxs <= 20 && s2.K1 * s2.IS < 65536;
+    const size_t mom2_smem = sizeof(double) * (size_t)moment2_smem_doubles(s2);
 #define WPCD_MOM2(MS, SPL)                                                                                                        \
     do {                                                                                                                      \
         err = cudaFuncSetAttribute(moments_kernel<MS, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
@@ -514,6 +693,16 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
                                                                      ch->trip_pack_dev, ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);         \
     } while (0)
 #define WPCD_MOM(MS) do { if (split) WPCD_MOM2(MS, true); else WPCD_MOM2(MS, false); } while (0)
+#define WPCD_MOMF3(MS, KTV, MTV)                                                                                                    \
+    do {                                                                                                                          \
+        err = cudaFuncSetAttribute(moments2_kernel<MS, KTV, MTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom2_smem);      \
+        if (err != cudaSuccess) return err;                                                                                       \
+        moments2_kernel<MS, KTV, MTV><<<(unsigned)(e1 - e0), 32, mom2_smem, st>>>(qr, g->p_dev, g->q_dev, g->n_q, s2, e0, e1, ws.geo_col, \
+                                                                                  ws.geo_row, ws.geo_phi, ch->ll_pack_dev, ch->trip_pack_dev, \
+                                                                                  ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);   \
+    } while (0)
+#define WPCD_MOMF2(MS, KTV) do { if (s2.K1 <= 8) WPCD_MOMF3(MS, KTV, 1); else WPCD_MOMF3(MS, KTV, 2); } while (0)
+#define WPCD_MOMF(MS) do { if (s2.NP == 8) WPCD_MOMF2(MS, 2); else WPCD_MOMF2(MS, 3); } while (0)
     err = cudaFuncSetAttribute(contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem);
     if (err != cudaSuccess) return err;
     {
@@ -534,7 +723,12 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         {
             const unsigned blocks = (unsigned)((e1 - e0 + mom_warps - 1) / mom_warps);
             StageTimer timer(WPCD_STAGE_MOMENTS, st);
-            if (maxs <= 4) WPCD_MOM(4);
+            if (fast) {
+                if (maxs <= 8) WPCD_MOMF(8);
+                else if (maxs <= 16) WPCD_MOMF(16);
+                else WPCD_MOMF(20);
+            }
+            else if (maxs <= 4) WPCD_MOM(4);
             else if (maxs <= 8) WPCD_MOM(8);
             else if (maxs <= 12) WPCD_MOM(12);
             else if (maxs <= 16) WPCD_MOM(16);
@@ -553,6 +747,9 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
             if ((err = cudaGetLastError()) != cudaSuccess) return err;
         }
     }
+#undef WPCD_MOMF
+#undef WPCD_MOMF2
+#undef WPCD_MOMF3
 #undef WPCD_MOM
 #undef WPCD_MOM2
     return cudaSuccess;

@@ -337,8 +337,8 @@ struct MomentShape2 {
 
 __host__ __device__ inline int moment2_smem_doubles(const MomentShape2& s)
 {
-    // phi-node records | P_k [K1][RS] | pa [LM1][RS] | pb [LM1][RS] | I [K1][IS] | cos/sin powers [G][2][CP] | c^a s^b [n_ab]
-    return (s.n * NODE_F + s.K1 * s.RS + 2 * s.LM1 * s.RS + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;
+    // phi-node records | P_k [K1][RS] | pa [LM1 + 1][RS] (last row zero) | pb [LM1][RS] | I [K1][IS] | cos/sin powers [G][2][CP] | c^a s^b [n_ab]
+    return (s.n * NODE_F + s.K1 * s.RS + (2 * s.LM1 + 1) * s.RS + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;
 }
 
 template <int MAXS, int KT, int MT>
@@ -356,13 +356,13 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
     if (e >= e_end) return;
     double* nodeS = sm;                       // [n][NODE_F]
     double* Pt = nodeS + n * NODE_F;          // [K1][RS]   P_k(x) of node slot g NP + r
-    double* pa = Pt + K1 * RS;                // [LM1][RS]  wF zeta2^{-(l+1)}
-    double* pb = pa + LM1 * RS;               // [LM1][RS]  zeta1^{-(l'+1)}
+    double* pa = Pt + K1 * RS;                // [LM1 + 1][RS]  wF zeta2^{-(l+1)}; row LM1 stays zero (columns beyond n_ll)
+    double* pb = pa + (LM1 + 1) * RS;         // [LM1][RS]  zeta1^{-(l'+1)}
     double* Ib = pb + LM1 * RS;               // [K1][IS]   I[k][l,l'] of one phi-node
     double* cs = Ib + K1 * IS;                // [G][2][CP] powers of cos, sin
     double* csp = cs + G * 2 * CP;            // [n_ab]     c^a s^b of one phi-node
     // the padding slots of the power tables must read as zero (they feed the MMAs); P_k only has to be finite there
-    for (int i = lane; i < (K1 + 2 * LM1) * RS; i += 32) Pt[i] = 0.0;
+    for (int i = lane; i < (K1 + 2 * LM1 + 1) * RS; i += 32) Pt[i] = 0.0;
     // per monomial: offset into Ib (low 16 bits) and into csp (high 16 bits)
     int pk[MAXS];
     double acc[MAXS];
@@ -376,14 +376,18 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
             pk[s] = ((tp & 0xff) * IS + (tp >> 8)) | ((v >> 16) << 16);     // mu_pack: triple | ab index << 16
         }
     }
-    // this lane's (l, l') of every n-tile, as offsets of its power-table rows (-1: column beyond n_ll)
-    int la[4], lb[4];
+    // this lane's (l, l') of every n-tile: where its rows of the power tables start (a column beyond n_ll reads the zero row)
+    const double* qa[4];
+    const double* qb[4];
 #pragma unroll
     for (int nt = 0; nt < 4; ++nt) {
         const int ll = nt * 8 + oct;
-        la[nt] = lb[nt] = -1;
-        if (nt < NT && ll < n_ll) { const int v = ll_pack[ll]; la[nt] = (v & 0xff) * RS; lb[nt] = (v >> 8) * RS; }
+        qa[nt] = pa + LM1 * RS + quad; qb[nt] = pb + quad;
+        if (nt < NT && ll < n_ll) { const int v = ll_pack[ll]; qa[nt] = pa + (v & 0xff) * RS + quad; qb[nt] = pb + (v >> 8) * RS + quad; }
     }
+    const double* qp[MT];          // this lane's rows of the P table (a row beyond K1 reads the zero row of pa)
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) qp[mt] = mt * 8 + oct < K1 ? Pt + (mt * 8 + oct) * RS + quad : pa + LM1 * RS + quad;
     const int col = geo_col[e], row = geo_row[e];
     const double2 ph = geo_phi[e];
     const Cell z = load_cell(p, q, n_q, row, col);
@@ -447,18 +451,18 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
                     csp[idx] = cs[(g * 2 + 0) * CP + (ab & 0xff)] * cs[(g * 2 + 1) * CP + (ab >> 8)];
                 }
                 // ---- step 3: I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] on the FP64 tensor cores
-                const int s0 = g * NP + quad;                          // this lane's node slot of k-step 0
+                const int s0 = g * NP;                                 // first node slot of this phi-node
                 double a[MT][KT];
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
-                    for (int kt = 0; kt < KT; ++kt) a[mt][kt] = mt * 8 + oct < K1 ? Pt[(mt * 8 + oct) * RS + s0 + 4 * kt] : 0.0;
+                    for (int kt = 0; kt < KT; ++kt) a[mt][kt] = qp[mt][s0 + 4 * kt];
 #pragma unroll
                 for (int nt = 0; nt < 4; ++nt) {
                     if (nt >= NT) break;
                     double b[KT];
 #pragma unroll
-                    for (int kt = 0; kt < KT; ++kt) b[kt] = la[nt] >= 0 ? pa[la[nt] + s0 + 4 * kt] * pb[lb[nt] + s0 + 4 * kt] : 0.0;
+                    for (int kt = 0; kt < KT; ++kt) b[kt] = qa[nt][s0 + 4 * kt] * qb[nt][s0 + 4 * kt];
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) {
                         double c0 = 0.0, c1 = 0.0;

@@ -29,9 +29,16 @@ import wpcd_inputs as wi  # noqa: E402
 # DRAM bytes per launch of the dominant kernel from one `ncu --set full` capture (dram__bytes_read.sum +
 # dram__bytes_write.sum), profiles/r01h_ncu_full.md; null where no capture of that workload exists.
 NCU_TRAFFIC = {
-    ("cfg2", "spmv"): 3.84e6,            # spmv_kernel<32,4>, one pass of 4 right-hand sides over the 3.4 MB matrix (cold L2 under ncu)
+    ("cfg2", "spmv"): 3.84e6,            # spmv_kernel<32,4>, one pass of 4 right-hand sides over the 3.4 MB matrix (cold L2 under ncu; r01h)
     ("cfg2", "fill_swave"): 6.88e6,
-    ("cfg4", "spmv"): 6.19e9,            # J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
+    ("cfg4", "spmv"): 6.19e9,            # r01h: CSR product, J^pi = 1/2+ matrix (5.14e8 nnz): 6.17 GB algorithmic
+    # profiles/r02_ncu_full.md: one launch on the J^pi = 7/2- matrix (3.24e9 nonzeros, the largest of the eight)
+    ("cfg5", "spmv"): 26.29e9,           # spmv_georow_kernel<1,256>: 26.27 GB read + 0.02 GB written; algorithmic 26.40 GB for that matrix
+    ("cfg5", "fill_coupled"): 0.787e9,   # contract_kernel, one chunk of 16 000 elements: 0.680 GB written + 0.107 GB read; 0.703 GB algorithmic
+}
+NCU_TRAFFIC_NOTE = {
+    ("cfg5", "spmv"): "launch on the J^pi = 7/2- matrix (3.24e9 nnz; 26.40 GB algorithmic for that launch, the step's mean launch is smaller)",
+    ("cfg5", "fill_coupled"): "contract_kernel, one 16 000-element chunk of the J^pi = 7/2- matrix (0.703 GB algorithmic); the moments stay in L2",
 }
 
 METRIC = "P-matrix nonzeros/sec (FP64 build + the workload's P*vector SpMVs per step)"
@@ -604,6 +611,8 @@ def run_ours(args):
     key = kernels[dominant]
     for name, rf in roofs.items():
         rf["traffic"] = NCU_TRAFFIC.get((wl.name, name))
+        if (wl.name, name) in NCU_TRAFFIC_NOTE:
+            rf["traffic_launch"] = NCU_TRAFFIC_NOTE[(wl.name, name)]
     roofline = dict(roofs[key]) if key in roofs else {
         "bound": "alu", "achieved": None, "peak": fp64_peak / 1e12, "unit": "TFLOP/s", "frac": None, "traffic": None}
     roofline["kernel"] = dominant
@@ -635,7 +644,7 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps, "includes": "grid/channel handle creation (host g-table), count, build, the products with pinned-host x and y"
                             + (" (one wpcd_perm_apply_host call with n_vec = %d: the vectors are independent and known up front)" % n_spmv
-                               if jobs[0].x_all is not None and n_spmv else " (one wpcd_perm_apply_host call per product)")},
+                               if (not idle and jobs[0].x_all is not None and n_spmv) else " (one wpcd_perm_apply_blocked_host call per product)")},
         "gpu_launches": int(launches),
         "roofline": roofline,
         "rooflines": roofs,

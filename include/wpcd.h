@@ -133,7 +133,7 @@ wpcd_status wpcd_perm_count(const wpcd_grid* grid, const wpcd_channels* channels
 
 /* Scratch needed by wpcd_perm_build for a pattern with nnz_geo geometric entries
  * (geometric column / row / phi-range lists, and for coupled channels a block of monomial
- * moments of at most 256 MiB plus a small launch table).  0 on invalid arguments. */
+ * moments of at most 64 MiB, 16 bytes per geometric entry and a few counters).  0 on invalid arguments. */
 size_t wpcd_perm_workspace_bytes(const wpcd_channels* channels, int64_t nnz_geo);
 
 /* Steps 2b+3 (l.312): column indices and values.
@@ -153,8 +153,9 @@ size_t wpcd_perm_workspace_bytes(const wpcd_channels* channels, int64_t nnz_geo)
  * the accuracy and ten times the cost of R(n_quad)); n_quad | WPCD_RULE_ANALYTIC_U the rule RA(n_quad) of R15 (the
  * same cuts, the x-integral of every piece in closed form; only for the s-wave channel set, WPCD_ERR_UNSUPPORTED
  * otherwise).  The pattern (wpcd_perm_count) does not depend on the rule.
- * Coupled channels: a channel pair may use any number of (k, l1+l1') monomials (more than 32 are
- * handled in several passes); WPCD_ERR_CUDA "invalid argument" if the tables exceed shared memory.
+ * Coupled channels: a channel pair may use any number of (k, l1+l1') monomials; WPCD_ERR_CUDA "invalid argument" if the
+ * tables of one (l, l') exceed shared memory (more than ~2000 distinct monomials for one (l, l')) or if
+ * (largest number of coupled channels of a row + 1) * nnz_geo reaches 2^31.
  * Asynchronous on the stream. */
 wpcd_status wpcd_perm_build(const wpcd_grid* grid, const wpcd_channels* channels, int n_quad, void* cuda_stream,
                             const int64_t* row_ptr_dev, const int32_t* geo_row_ptr_dev,
@@ -162,9 +163,9 @@ wpcd_status wpcd_perm_build(const wpcd_grid* grid, const wpcd_channels* channels
                             int32_t* col_idx_dev, double* values_dev);
 
 /* y = P0 x for n_vec vectors (step 5, l.314; l.304).  x_dev[v*rows + c], y_dev[v*rows + r],
- * v = 0..n_vec-1 (vector-major), dev.  CSR arrays as produced above.  Asynchronous -- except that the first
- * product on a row_ptr_dev this process has not seen from wpcd_perm_count reads nnz back once (synchronises the
- * stream; do that call outside a CUDA-graph capture): the kernel variant is chosen from the mean row length. */
+ * v = 0..n_vec-1 (vector-major), dev.  Any CSR arrays with int64 row_ptr / int32 col_idx (as produced above, or the
+ * caller's own).  Asynchronous, capturable in a CUDA graph: the kernel variant (lanes per row) is chosen on the device
+ * from the mean row length row_ptr[rows] / rows; nothing is read back and nothing is remembered between calls. */
 wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
                             const double* values_dev, const double* x_dev, double* y_dev, int n_vec,
                             void* cuda_stream);
@@ -205,7 +206,8 @@ wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* grid, const wpcd_channels* 
  * 1.6e5 on a B200, measured: spmv_chain.cu) runs the whole chain in ONE cooperative launch -- row slices resident
  * in shared memory, a grid-wide barrier between products; any other matrix takes n_iter ordinary products on the
  * stream.  Either way a row is summed in a fixed lane order (deterministic), but the two orders differ, so results
- * agree to rounding, not bit for bit, across the two paths.  Asynchronous.  At most 64 fused chains in flight per
+ * agree to rounding, not bit for bit, across the two paths.  Reads the number of nonzeros back once per call (it
+ * sizes the shared-memory slices): synchronises the stream, then queues the work.  At most 64 fused chains in flight per
  * device (the barrier counters are a ring). */
 wpcd_status wpcd_perm_apply_chain(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev,
                                   const double* values_dev, const double* x_dev, double* y_dev, int n_iter,

@@ -158,9 +158,6 @@ Workspace carve_workspace(const wpcd_channels* ch, int64_t nnz_geo, void* base)
     return ws;
 }
 
-static std::mutex g_hint_mutex;
-static std::map<const void*, std::pair<int64_t, int64_t>> g_nnz_hint;   // row_ptr_dev -> (rows, nnz)
-
 static void free_channels_device(wpcd_channels* c)
 {
     if (c->ncoupled_dev) cudaDeviceSynchronize();   // the tables go back to the buffer cache: no kernel may still read them
@@ -602,11 +599,6 @@ wpcd_status wpcd_perm_count(const wpcd_grid* g, const wpcd_channels* c, int n_qu
     int64_t nnz_geo = g->stage_nnz_geo;
     *nnz_geo_out = nnz_geo;
     *nnz_out = nnz_geo * c->total_coupled;
-    {
-        std::lock_guard<std::mutex> lock(g_hint_mutex);
-        if (g_nnz_hint.size() > 4096) g_nnz_hint.clear();   // a heuristic cache only (kernel selection): keep it bounded
-        g_nnz_hint[row_ptr_dev] = {rows, *nnz_out};
-    }
     return WPCD_OK;
 }
 
@@ -674,22 +666,6 @@ wpcd_status wpcd_perm_build(const wpcd_grid* g, const wpcd_channels* c, int n_qu
     return WPCD_OK;
 }
 
-static double mean_row_hint(int64_t rows, const int64_t* row_ptr_dev, cudaStream_t st)
-{
-    {
-        std::lock_guard<std::mutex> lock(g_hint_mutex);
-        auto it = g_nnz_hint.find(row_ptr_dev);
-        if (it != g_nnz_hint.end() && it->second.first == rows) return (double)it->second.second / (double)std::max<int64_t>(rows, 1);
-    }
-    int64_t nnz = 0;
-    if (cudaMemcpyAsync(&nnz, row_ptr_dev + rows, sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess) return 32.0;
-    cudaStreamSynchronize(st);
-    std::lock_guard<std::mutex> lock(g_hint_mutex);
-    if (g_nnz_hint.size() > 4096) g_nnz_hint.clear();
-    g_nnz_hint[row_ptr_dev] = {rows, nnz};
-    return (double)nnz / (double)std::max<int64_t>(rows, 1);
-}
-
 wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
                             const double* x_dev, double* y_dev, int n_vec, void* cuda_stream)
 {
@@ -697,9 +673,7 @@ wpcd_status wpcd_perm_apply(int64_t rows, const int64_t* row_ptr_dev, const int3
     if (rows == 0 || n_vec == 0) return WPCD_OK;
     if (!row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply: null pointer");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
-    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply: null matrix arrays");
-    cudaError_t err = launch_spmv(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, mean_row, st);
+    cudaError_t err = launch_spmv(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply");
     return WPCD_OK;
 }
@@ -713,9 +687,7 @@ wpcd_status wpcd_perm_apply_complex(int64_t rows, const int64_t* row_ptr_dev, co
     if ((reinterpret_cast<uintptr_t>(x_dev) & 15) || (reinterpret_cast<uintptr_t>(y_dev) & 15))
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_complex: x and y must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
-    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_complex: null matrix arrays");
-    cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, 2, mean_row, st);
+    cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, 2, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_complex");
     return WPCD_OK;
 }
@@ -730,9 +702,7 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
     if ((reinterpret_cast<uintptr_t>(x_dev) & 15) || (reinterpret_cast<uintptr_t>(y_dev) & 15))
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: x and y must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
-    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_interleaved: null matrix arrays");
-    cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, 1, n_inter, mean_row, st);
+    cudaError_t err = launch_spmv_interleaved(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, 1, n_inter, st);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_interleaved");
     return WPCD_OK;
 }
@@ -763,16 +733,20 @@ wpcd_status wpcd_perm_apply_chain(int64_t rows, const int64_t* row_ptr_dev, cons
     if (x_dev + rows > y_dev && y_dev + (int64_t)n_iter * rows > x_dev)
         return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: x overlaps y");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    double mean_row = mean_row_hint(rows, row_ptr_dev, st);
-    if (mean_row > 0.0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: null matrix arrays");
+    // the fused launch sizes its shared-memory slices from the number of nonzeros: one small read-back per call
+    int64_t nnz = 0;
+    cudaError_t nerr = cudaMemcpyAsync(&nnz, row_ptr_dev + rows, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    if (nerr == cudaSuccess) nerr = cudaStreamSynchronize(st);
+    if (nerr != cudaSuccess) return cuda_fail(nerr, "wpcd_perm_apply_chain");
+    if (nnz > 0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_chain: null matrix arrays");
     int fused = 0;
-    cudaError_t err = launch_spmv_chain(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_iter, mean_row, st, &fused);
+    cudaError_t err = launch_spmv_chain(rows, row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_iter, nnz, st, &fused);
     if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_chain");
     if (!fused) {
         const double* xin = x_dev;
         for (int k = 0; k < n_iter; ++k) {
             double* yk = y_dev + (int64_t)k * rows;
-            err = launch_spmv(rows, row_ptr_dev, col_idx_dev, values_dev, xin, yk, 1, mean_row, st);
+            err = launch_spmv(rows, row_ptr_dev, col_idx_dev, values_dev, xin, yk, 1, st);
             if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_chain");
             xin = yk;
         }

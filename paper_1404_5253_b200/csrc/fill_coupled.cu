@@ -4,22 +4,19 @@
 // B = l+l'-A).  The geometry (F, zeta, limits) is shared by ALL channel pairs of a geometric
 // element, so the work is split in two kernels:
 //
-//   moments_kernel   one warp per geometric element.  With the x-sum factored out,
+//   moments kernels  one warp per geometric element.  With the x-sum factored out,
 //                      M[k,A,l,l'] = sum_m  W_m c_m^{A+1} s_m^{B+1}  I_m[k,l,l'],
 //                      I_m[k,l,l'] = sum_r  P_k(x_r) T_r[l,l'],   T_r[l,l'] = w_r F_r zeta1^{-(l'+1)} zeta2^{-(l+1)}.
-//                    lanes = phi-nodes for the phi set-up, = (phi-node, x-node) pairs for the node set-up
-//                    that writes P_k and T to shared memory; I_m = P^T T, a small dense contraction
-//                    (K1 x n)(n x n_ll), runs on the FP64 tensor cores (mma.sync m8n8k4, SASS DMMA);
-//                    lanes = monomials for the final multiply-add with the c^a s^b table.
-//                    Moments are written as [tile of 32 elements][mu][32] (256-byte lines per monomial).
-//   contract_kernel  value[pair][element] = sum_m G[pair][m] M[m][element] class by class
-//                    (wpcd_internal.h): lane = element, the class block of the moment row lives in
-//                    REGISTERS, the dense coefficient rows G stream from shared memory as broadcast
-//                    128-bit loads.  A CTA owns one slab of classes (copied to shared memory once,
-//                    by a TMA bulk copy) and walks over many 32-element tiles, so that the table is
-//                    read from L2 a few hundred times in all and every moment exactly once; the next
-//                    class block is staged by cp.async while the current one is contracted.  Each
-//                    pair writes 32 consecutive CSR values + column indices per warp (coalesced).
+//                    lanes = phi-nodes for the phi set-up, = (phi-node, x-node) pairs for the node set-up;
+//                    I_m = P^T T, a small dense contraction (K1 x n)(n x n_ll), runs on the FP64 tensor cores
+//                    (mma.sync m8n8k4, SASS DMMA); lanes = monomials for the final multiply-add with the c^a s^b
+//                    table.  moments2_kernel: the production path (plain rule, 5 <= n <= 12; transposed conflict-free
+//                    tables, power tables instead of T); moments_kernel: kink-split rule and every other order.
+//                    Moments are written element-major, moments[element][mu].
+//   contract_kernel  value[element][pair] = sum_m M[element][m] G[pair][m] on the FP64 tensor cores, pairs grouped by
+//                    (l, l') and by monomial set (wpcd_internal.h); persistent CTAs pull (group, tile block) units,
+//                    keep the group's tables and the block's moments in shared memory and write, per pair, coalesced
+//                    runs of CSR values and column indices.
 #include <math.h>
 
 #include <mutex>

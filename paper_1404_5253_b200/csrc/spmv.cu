@@ -18,14 +18,9 @@ namespace wpcd_detail { bool use_pdl(); }
 namespace {
 
 template <int LPR, int NV, bool PIPE>
-__global__ void __launch_bounds__(256)
-spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
-            const double* __restrict__ values, const double* __restrict__ x, double* __restrict__ y, int64_t ldx)
+__device__ __forceinline__ void spmv_rows(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+                                          const double* __restrict__ values, const double* __restrict__ x, double* __restrict__ y, int64_t ldx)
 {
-    // Programmatic dependent launch: this grid may be scheduled while the previous kernel of the
-    // stream drains; nothing is read or written before the wait, so the usual stream order holds.
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = t / LPR;
     const int sub = (int)(t - row * LPR);
@@ -100,14 +95,43 @@ spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __
     }
 }
 
-template <int LPR, int NV, bool PIPE = false>
-cudaError_t launch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
-                   double* y, cudaStream_t st)
+// Which variant a matrix takes is decided ON THE DEVICE from its mean row length (row_ptr[rows] / rows): no host copy of nnz,
+// no synchronisation, nothing remembered between calls.  Row lengths of P0 are very skewed (median 11, max ~400 per
+// coupled channel at N = 100) and a small matrix is latency-bound by its longest row, so wide rows are preferred early:
+// 4 / 8 / 16 lanes per row up to a mean of 3 / 6 / 12 entries, 32 beyond, software-pipelined from 128.  The grid is sized
+// for 32 lanes per row; with fewer lanes the surplus CTAs return at once (such matrices are tiny).
+__device__ __forceinline__ int pick_lanes(int64_t rows, int64_t nnz, int forced, bool no_pipe, bool& pipe)
 {
-    int64_t threads = rows * LPR;
-    int64_t blocks = (threads + 255) / 256;
+    int lpr = forced;
+    if (lpr != 4 && lpr != 8 && lpr != 16 && lpr != 32) lpr = nnz <= 3 * rows ? 4 : nnz <= 6 * rows ? 8 : nnz <= 12 * rows ? 16 : 32;
+    pipe = forced == 0 && !no_pipe && nnz >= 128 * rows;
+    return lpr;
+}
+
+template <int NV>
+__global__ void __launch_bounds__(256)
+spmv_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+            const double* __restrict__ values, const double* __restrict__ x, double* __restrict__ y, int64_t ldx, int forced, int no_pipe)
+{
+    // Programmatic dependent launch: this grid may be scheduled while the previous kernel of the
+    // stream drains; nothing is read or written before the wait, so the usual stream order holds.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    bool pipe;
+    const int lpr = pick_lanes(rows, row_ptr[rows], forced, no_pipe != 0, pipe);
+    if ((int64_t)blockIdx.x * blockDim.x >= rows * lpr) return;
+    if (pipe) spmv_rows<32, NV, true>(rows, row_ptr, col_idx, values, x, y, ldx);
+    else if (lpr == 32) spmv_rows<32, NV, false>(rows, row_ptr, col_idx, values, x, y, ldx);
+    else if (lpr == 16) spmv_rows<16, NV, false>(rows, row_ptr, col_idx, values, x, y, ldx);
+    else if (lpr == 8) spmv_rows<8, NV, false>(rows, row_ptr, col_idx, values, x, y, ldx);
+    else spmv_rows<4, NV, false>(rows, row_ptr, col_idx, values, x, y, ldx);
+}
+
+template <class K, class... A>
+cudaError_t launch_pdl(K kernel, int64_t rows, cudaStream_t st, A... args)
+{
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.gridDim = dim3((unsigned)((rows * 32 + 255) / 256));
     cfg.blockDim = dim3(256);
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
@@ -116,25 +140,15 @@ cudaError_t launch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx,
     cfg.attrs = attr;
     cfg.numAttrs = wpcd_detail::use_pdl() ? 1 : 0;
     ++wpcd_detail::g_launches;
-    return cudaLaunchKernelEx(&cfg, spmv_kernel<LPR, NV, PIPE>, rows, row_ptr, col_idx, values, x, y, rows);
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
 }
 
 template <int NV>
 cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values, const double* x,
-                     double* y, double mean_row, cudaStream_t st)
+                     double* y, cudaStream_t st)
 {
-    const int forced = wpcd_detail::g_debug.spmv_lanes_per_row.load();
-    if (forced == 4) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (forced == 8) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (forced == 16) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (forced == 32) return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    // Row lengths of P0 are very skewed (median 11, max ~400 per coupled channel at N = 100), and a small
-    // matrix is latency-bound by its longest row: prefer wide rows early.
-    if (mean_row <= 3.0) return launch<4, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (mean_row <= 6.0) return launch<8, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (mean_row <= 12.0) return launch<16, NV>(rows, row_ptr, col_idx, values, x, y, st);
-    if (!wpcd_detail::g_debug.spmv_no_pipeline.load() && mean_row >= 128.0) return launch<32, NV, true>(rows, row_ptr, col_idx, values, x, y, st);
-    return launch<32, NV>(rows, row_ptr, col_idx, values, x, y, st);
+    return launch_pdl(spmv_kernel<NV>, rows, st, rows, row_ptr, col_idx, values, x, y, rows,
+                      wpcd_detail::g_debug.spmv_lanes_per_row.load(), wpcd_detail::g_debug.spmv_no_pipeline.load());
 }
 
 // ---------------------------------------------------------------- interleaved right-hand sides
@@ -142,12 +156,9 @@ cudaError_t dispatch(int64_t rows, const int64_t* row_ptr, const int32_t* col_id
 // the transition operator of eq. 12 is complex -- NI = 4 two complex or four real vectors.
 // An entry costs ONE gather of NI*8 bytes and NI multiply-adds.
 template <int LPR, bool PIPE, int NI>
-__global__ void __launch_bounds__(256)
-spmv_interleaved_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
-                        const double* __restrict__ values, const double2* __restrict__ x, double2* __restrict__ y)
+__device__ __forceinline__ void spmv_interleaved_rows(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+                                                      const double* __restrict__ values, const double2* __restrict__ x, double2* __restrict__ y)
 {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
     constexpr int H = NI / 2;                 // 16-byte pieces per column
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = t / LPR;
@@ -231,32 +242,28 @@ spmv_interleaved_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const
     }
 }
 
-template <int LPR, bool PIPE, int NI>
-cudaError_t launch_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                               const double2* x, double2* y, cudaStream_t st)
+template <int NI>
+__global__ void __launch_bounds__(256)
+spmv_interleaved_kernel(int64_t rows, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
+                        const double* __restrict__ values, const double2* __restrict__ x, double2* __restrict__ y, int no_pipe)
 {
-    int64_t blocks = (rows * LPR + 255) / 256;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)blocks);
-    cfg.blockDim = dim3(256);
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = wpcd_detail::use_pdl() ? 1 : 0;
-    ++wpcd_detail::g_launches;
-    return cudaLaunchKernelEx(&cfg, spmv_interleaved_kernel<LPR, PIPE, NI>, rows, row_ptr, col_idx, values, x, y);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    bool pipe;
+    int lpr = pick_lanes(rows, row_ptr[rows], 0, no_pipe != 0, pipe);
+    if (lpr < 8) lpr = 8;
+    if ((int64_t)blockIdx.x * blockDim.x >= rows * lpr) return;
+    if (pipe) spmv_interleaved_rows<32, true, NI>(rows, row_ptr, col_idx, values, x, y);
+    else if (lpr == 32) spmv_interleaved_rows<32, false, NI>(rows, row_ptr, col_idx, values, x, y);
+    else if (lpr == 16) spmv_interleaved_rows<16, false, NI>(rows, row_ptr, col_idx, values, x, y);
+    else spmv_interleaved_rows<8, false, NI>(rows, row_ptr, col_idx, values, x, y);
 }
 
 template <int NI>
 cudaError_t dispatch_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                                 const double2* x, double2* y, double mean_row, cudaStream_t st)
+                                 const double2* x, double2* y, cudaStream_t st)
 {
-    if (mean_row <= 6.0) return launch_interleaved<8, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
-    if (mean_row <= 12.0) return launch_interleaved<16, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
-    if (mean_row >= 128.0) return launch_interleaved<32, true, NI>(rows, row_ptr, col_idx, values, x, y, st);
-    return launch_interleaved<32, false, NI>(rows, row_ptr, col_idx, values, x, y, st);
+    return launch_pdl(spmv_interleaved_kernel<NI>, rows, st, rows, row_ptr, col_idx, values, x, y, wpcd_detail::g_debug.spmv_no_pipeline.load());
 }
 
 // ---------------------------------------------------------------- FP64 FMA peak
@@ -282,16 +289,16 @@ bool use_pdl()
 }
 
 cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                        const double* x, double* y, int n_vec, double mean_row, cudaStream_t st)
+                        const double* x, double* y, int n_vec, cudaStream_t st)
 {
     int v = 0;
     while (v < n_vec) {
         const double* xv = x + (int64_t)v * rows;
         double* yv = y + (int64_t)v * rows;
         cudaError_t err;
-        if (n_vec - v >= 4) { err = dispatch<4>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 4; }
-        else if (n_vec - v >= 2) { err = dispatch<2>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 2; }
-        else { err = dispatch<1>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st); v += 1; }
+        if (n_vec - v >= 4) { err = dispatch<4>(rows, row_ptr, col_idx, values, xv, yv, st); v += 4; }
+        else if (n_vec - v >= 2) { err = dispatch<2>(rows, row_ptr, col_idx, values, xv, yv, st); v += 2; }
+        else { err = dispatch<1>(rows, row_ptr, col_idx, values, xv, yv, st); v += 1; }
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;
@@ -299,13 +306,13 @@ cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col
 
 // n_vec groups of n_inter interleaved components each (group-major: x[(g*rows + c)*n_inter + v])
 cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                                    const double* x, double* y, int n_vec, int n_inter, double mean_row, cudaStream_t st)
+                                    const double* x, double* y, int n_vec, int n_inter, cudaStream_t st)
 {
     for (int v = 0; v < n_vec; ++v) {
         const double2* xv = reinterpret_cast<const double2*>(x) + (int64_t)v * rows * (n_inter / 2);
         double2* yv = reinterpret_cast<double2*>(y) + (int64_t)v * rows * (n_inter / 2);
-        cudaError_t err = n_inter == 4 ? dispatch_interleaved<4>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st)
-                                       : dispatch_interleaved<2>(rows, row_ptr, col_idx, values, xv, yv, mean_row, st);
+        cudaError_t err = n_inter == 4 ? dispatch_interleaved<4>(rows, row_ptr, col_idx, values, xv, yv, st)
+                                       : dispatch_interleaved<2>(rows, row_ptr, col_idx, values, xv, yv, st);
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;

@@ -257,7 +257,7 @@ namespace wpcd_detail {
 // *fused = 1 if the chain ran as one cooperative launch, 0 if the matrix does not qualify (the caller then issues
 // n_iter ordinary products).
 cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                              const double* x, double* y, int n_iter, double mean_row, cudaStream_t st, int* fused)
+                              const double* x, double* y, int n_iter, int64_t nnz, cudaStream_t st, int* fused)
 {
     *fused = 0;
     const int mode = g_debug.chain_mode.load();
@@ -273,7 +273,6 @@ cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_
         cudaDeviceGetAttribute(&d.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     }
     if (!d.coop || d.sms <= 0) return cudaSuccess;
-    const int64_t nnz = (int64_t)(mean_row * (double)rows + 0.5);
     const int64_t smem_budget = (int64_t)d.smem_optin - 2048;
     // per-CTA slice: nnz / G entries (+ one long row of slack) and about rows / G rows; the whole matrix must fit on chip
     const int64_t want_entries = nnz / d.sms + nnz / d.sms / 4 + 2048;

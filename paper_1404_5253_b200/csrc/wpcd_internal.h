@@ -169,14 +169,14 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
 
 // spmv.cu
 cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                        const double* x, double* y, int n_vec, double mean_row, cudaStream_t st);
+                        const double* x, double* y, int n_vec, cudaStream_t st);
 cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                                    const double* x, double* y, int n_vec, int n_inter, double mean_row, cudaStream_t st);
+                                    const double* x, double* y, int n_vec, int n_inter, cudaStream_t st);
 // spmv_blocked.cu
 cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
                                 const double* values, const double* x, double* y, int n_vec, cudaStream_t st);
 cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
-                              const double* x, double* y, int n_iter, double mean_row, cudaStream_t st, int* fused);
+                              const double* x, double* y, int n_iter, int64_t nnz, cudaStream_t st, int* fused);
 cudaError_t run_fp64_peak(cudaStream_t st, double* flops_out);
 
 // kernel_apply.cu

@@ -9,6 +9,9 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
+#include <algorithm>
+#include <array>
+#include <map>
 #include <vector>
 
 namespace wpcd_host {
@@ -117,6 +120,39 @@ struct Pair { int gamma, gammap; std::vector<Term> terms; };
 inline std::vector<Pair> g_table(const std::vector<Channel>& ch, int two_J, int two_T) {
     std::vector<Pair> pairs;
     auto hat = [](int x) { return (long double)(2 * x + 1); };
+    // The orbital part depends on (l, lambda, l', lambda'; L, l1, l1', k) only -- not on the spins, j, I of the channels -- so
+    // it is tabulated once per distinct (l, lambda, l', lambda') and reused by every channel pair that carries these labels
+    // (62 channels share ~20 distinct (l, lambda) for the nd tables of j <= 3: a tenth of the evaluations).
+    struct OrbitalBlock { int Llo, Lhi, K; std::vector<long double> v; };      // v[((L - Llo) (l+1) + l1) (l'+1) + l1'] K + k]
+    std::map<std::array<int, 4>, OrbitalBlock> blocks;
+    auto block_of = [&](int l, int lam, int lp, int lamp) -> const OrbitalBlock& {
+        const std::array<int, 4> key = {l, lam, lp, lamp};
+        auto it = blocks.find(key);
+        if (it != blocks.end()) return it->second;
+        OrbitalBlock blk;
+        blk.Llo = std::max(std::abs(l - lam), std::abs(lp - lamp));
+        blk.Lhi = std::min(l + lam, lp + lamp);
+        blk.K = l + lam + lp + lamp + 1;                               // k <= min(l1 + lambda + l1', l2' + lambda' + l2) < K
+        const int nL = blk.Lhi >= blk.Llo ? blk.Lhi - blk.Llo + 1 : 0;
+        blk.v.assign((size_t)nL * (l + 1) * (lp + 1) * blk.K, 0.0L);
+        for (int L = blk.Llo; L <= blk.Lhi; ++L)
+            for (int l1 = 0; l1 <= l; ++l1)
+                for (int l1p = 0; l1p <= lp; ++l1p) {
+                    const int l2 = l - l1, l2p = lp - l1p;
+                    const int kmax = std::min(l1 + lam + l1p, l2p + lamp + l2);
+                    for (int k = 0; k <= kmax; ++k)
+                        blk.v[((size_t)((L - blk.Llo) * (l + 1) + l1) * (lp + 1) + l1p) * blk.K + k] = orbital(l, lam, lp, lamp, L, l1, l1p, k);
+                }
+        return blocks.emplace(key, std::move(blk)).first->second;
+    };
+    // the 9j symbol of a channel for every (L, S) it can take part in: {l s j; lambda 1/2 I; L S J}
+    int Lmax = 0;
+    for (const Channel& c : ch) Lmax = std::max(Lmax, c.l + c.lam);
+    std::vector<long double> nj(ch.size() * (size_t)(Lmax + 1) * 2, 0.0L);
+    for (size_t a = 0; a < ch.size(); ++a)
+        for (int L = std::abs(ch[a].l - ch[a].lam); L <= ch[a].l + ch[a].lam; ++L)
+            for (int si = 0; si < 2; ++si)
+                nj[(a * (Lmax + 1) + L) * 2 + si] = nine_j(2 * ch[a].l, 2 * ch[a].s, 2 * ch[a].j, 2 * ch[a].lam, 1, ch[a].two_I, 2 * L, 1 + 2 * si, two_J);
     for (size_t a = 0; a < ch.size(); ++a)
         for (size_t b = 0; b < ch.size(); ++b) {
             const Channel &c = ch[a], &d = ch[b];
@@ -133,14 +169,15 @@ inline std::vector<Pair> g_table(const std::vector<Channel>& ch, int two_J, int 
                 for (int two_S = 1; two_S <= 3; two_S += 2) {
                     long double spin = six_j(1, 1, 2 * c.s, 1, two_S, 2 * d.s);
                     if (spin == 0.0L) continue;
-                    long double n1 = nine_j(2 * c.l, 2 * c.s, 2 * c.j, 2 * c.lam, 1, c.two_I, 2 * L, two_S, two_J);
+                    long double n1 = nj[(a * (Lmax + 1) + L) * 2 + (two_S >> 1)];
                     if (n1 == 0.0L) continue;
-                    long double n2 = nine_j(2 * d.l, 2 * d.s, 2 * d.j, 2 * d.lam, 1, d.two_I, 2 * L, two_S, two_J);
+                    long double n2 = nj[(b * (Lmax + 1) + L) * 2 + (two_S >> 1)];
                     wL[L - Llo] += (long double)(2 * L + 1) * (two_S + 1) * spin * n1 * n2;
                     any = any || (n2 != 0.0L);
                 }
             if (!any) continue;
             Pair pr{(int)a, (int)b, {}};
+            const OrbitalBlock& blk = block_of(c.l, c.lam, d.l, d.lam);
             for (int l1 = 0; l1 <= c.l; ++l1)
                 for (int l1p = 0; l1p <= d.l; ++l1p) {
                     int l2 = c.l - l1, l2p = d.l - l1p;
@@ -148,7 +185,8 @@ inline std::vector<Pair> g_table(const std::vector<Channel>& ch, int two_J, int 
                     for (int k = 0; k <= kmax; ++k) {
                         long double tot = 0.0L;
                         for (int L = Llo; L <= Lhi; ++L)
-                            if (wL[L - Llo] != 0.0L) tot += wL[L - Llo] * orbital(c.l, c.lam, d.l, d.lam, L, l1, l1p, k);
+                            if (wL[L - Llo] != 0.0L)
+                                tot += wL[L - Llo] * blk.v[((size_t)((L - blk.Llo) * (c.l + 1) + l1) * (d.l + 1) + l1p) * blk.K + k];
                         double g = (double)(pref * iso * tot);
                         if (std::fabs(g) > 1e-14) pr.terms.push_back({k, l1, l1p, g});
                     }

@@ -566,13 +566,15 @@ contract_kernel(int64_t e0, int64_t e1, int64_t nnz_geo, int n_geo, const int4* 
         // ---- stage the moments of this (l, l') for the block's elements: warp = element row, lanes along the monomials
         {
             const double* src = moments + (size_t)(es - e0) * n_mu + g.mu_lo;
-            // asynchronous copies (8 bytes each: a row starts on an 8-byte boundary only), all in flight together
-            for (int ei = warp; ei < rows; ei += CT_WARPS) {
-                const double* s = src + (size_t)ei * n_mu;
-                const uint32_t d = (uint32_t)__cvta_generic_to_shared(Ms + ei * ms_stride);
+            // asynchronous copies (8 bytes each: a row starts on an 8-byte boundary only), all in flight together; the
+            // addresses advance by constant strides (an element row is n_mu doubles away from the next)
+            const double* s = src + (size_t)warp * n_mu + lane;
+            uint32_t d = (uint32_t)__cvta_generic_to_shared(Ms + warp * ms_stride + lane);
+            const size_t s_step = (size_t)CT_WARPS * n_mu;
+            const uint32_t d_step = (uint32_t)(CT_WARPS * ms_stride * sizeof(double));
+            for (int ei = warp; ei < rows; ei += CT_WARPS, s += s_step, d += d_step)
                 for (int mi = lane; mi < g.n_mono; mi += 32)
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + 8 * mi), "l"(s + mi) : "memory");
-            }
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + 8 * (mi - lane)), "l"(s + (mi - lane)) : "memory");
             for (int i = tid; i < rows; i += CT_THREADS) rec_s[i] = __ldg(elem_rec + es + i);       // grp, cnt, gcol, row
             asm volatile("cp.async.commit_group;" ::: "memory");
             asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -724,9 +726,13 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         {
             const unsigned blocks = (unsigned)((e1 - e0 + mom_warps - 1) / mom_warps);
             StageTimer timer(WPCD_STAGE_MOMENTS, st);
-            if (fast) {
+            if (fast) {            // accumulator slots per lane: ceil(n_mu / 32), in steps of two above 8 (an unused slot still issues)
                 if (maxs <= 8) WPCD_MOMF(8);
+                else if (maxs <= 10) WPCD_MOMF(10);
+                else if (maxs <= 12) WPCD_MOMF(12);
+                else if (maxs <= 14) WPCD_MOMF(14);
                 else if (maxs <= 16) WPCD_MOMF(16);
+                else if (maxs <= 18) WPCD_MOMF(18);
                 else WPCD_MOMF(20);
             }
             else if (maxs <= 4) WPCD_MOM(4);

@@ -944,7 +944,8 @@ def test_apply_blocked(wpcd):
 
 def test_apply_blocked_chunked_paths(wpcd):
     """The same product with a tiny x tile (wpcd_debug_set): geometric rows cut into column chunks, channels into channel
-    chunks, runs of coupled channels split at chunk boundaries; 1, 2, 3 and 5 vectors per call."""
+    chunks, runs of coupled channels split at chunk boundaries; 1 .. 15 vectors per call (scalar passes of 1, 2 and 4 vectors,
+    tensor-core passes of 5 .. 8)."""
     torch = _torch()
     gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=1, two_T=1, j_pair_max=2)
     p, q = wi.tan2_grid(9, 1.0, 0.1, seed=41), wi.tan2_grid(11, 0.8, 0.1, seed=42)
@@ -954,12 +955,13 @@ def test_apply_blocked_chunked_paths(wpcd):
     try:
         for tile in (0, 7, 40, 256):
             wpcd.wpcd_debug_set("blocked_tile_doubles", tile)
-            for n_vec in (1, 2, 3, 5, 9, 15):
+            for n_vec in (1, 2, 3, 5, 6, 9, 12, 15):
                 xs = np.stack([wi.normal_vector(m.rows, k=820 + k) for k in range(n_vec)])
                 x = torch.from_numpy(xs).cuda()
-                y = torch.full_like(x, np.nan)
+                y = torch.full((n_vec + 1, m.rows), np.nan, dtype=torch.float64, device="cuda")    # one guard vector behind
                 wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y, n_vec=n_vec)
                 yh = y.cpu().numpy()
+                assert np.all(np.isnan(yh[n_vec])), (tile, n_vec)      # a pass padded to 8 vectors writes only those asked for
                 for k in range(n_vec):
                     ref = operm.spmv(rp, ci, v, xs[k])
                     scale = operm.spmv(rp, ci, np.abs(v), np.abs(xs[k]))

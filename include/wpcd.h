@@ -191,7 +191,11 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
  * shifted by gamma' * n_p * n_q.  One CTA per geometric row (i,j) gathers the values of x at those columns for all
  * channels into shared memory once, and the n_channels rows of that (i,j) then stream only their VALUES: 8 bytes per
  * nonzero from HBM instead of the 12 of the general CSR product, and one gather per (channel, geometric entry) instead of
- * one per nonzero (the SpMV is HBM-bound).  Up to 4 vectors share one pass over the matrix.
+ * one per nonzero (the SpMV is HBM-bound).  Several vectors share one pass over the matrix: 5 - 8 go
+ * through the FP64 tensor cores (values as A fragments, the planes of the x tile as B; n_channels <= 64, else scalar
+ * passes), fewer through scalar passes of 4, 2, 1; n_vec is cut into such passes.  A tensor-core pass works on an
+ * interleaved copy of its x vectors held in stream-ordered scratch (cudaMallocAsync / cudaFreeAsync on cuda_stream,
+ * 64 rows bytes, released behind the product; allowed during stream capture).
  * geo_row_ptr_dev as written by wpcd_perm_count, col_idx_dev / values_dev by wpcd_perm_build, for THESE handles (not
  * checked; row_ptr_dev is not read); x_dev, y_dev [n_vec][rows], dev, x_dev must not alias y_dev.  Each row is summed in a
  * fixed order (deterministic; agrees with wpcd_perm_apply to rounding).  Asynchronous.  At most 64 such products in

@@ -243,7 +243,7 @@ spmv_georow_mma8_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row
         if (ticket >= (unsigned int)n_geo) break;
         const int r = n_geo - 1 - (int)ticket;                 // the long rows sit at the high cell indices: they go first
         const int grp = geo_row_ptr[r], cnt = geo_row_ptr[r + 1] - grp;
-        double c0 = 0.0, c1 = 0.0;                             // D[row oct][vectors 2 quad, 2 quad + 1]
+        double c[4][2] = {};                                   // D[row oct][vectors 2 quad, 2 quad + 1]: four independent chains of MMAs
         if (cnt > 0 && first_gamma >= 0) {
             const int32_t* cfirst = col_idx + (chan_off[first_gamma] * nnz_geo + (int64_t)ncoupled[first_gamma] * grp);
             const double* vrow = values + (my_off + (int64_t)my_nc * grp);          // this lane's CSR row (gamma, r)
@@ -289,8 +289,8 @@ spmv_georow_mma8_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row
                             for (int k = 0; k < GM_UNR; ++k) {
                                 if (s + 4 * k >= cs) break;                               // warp-uniform
                                 const bool in = s + 4 * k + quad < cs;
-                                dmma_884g(c0, c1, a[k], in ? xb[s + 4 * k] : 0.0);
-                                if (has_q) dmma_884g(c0, c1, aq[k], in ? xq[s + 4 * k] : 0.0);
+                                dmma_884g(c[k & 1][0], c[k & 1][1], a[k], in ? xb[s + 4 * k] : 0.0);
+                                if (has_q) dmma_884g(c[2 + (k & 1)][0], c[2 + (k & 1)][1], aq[k], in ? xq[s + 4 * k] : 0.0);
                             }
                         }
                     }
@@ -298,7 +298,8 @@ spmv_georow_mma8_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row
             }
         }
         // ---- the partial sums of the wpg warps of a row group, added in a fixed order
-        *reinterpret_cast<double2*>(ypart + (size_t)warp * 64 + oct * 8 + 2 * quad) = make_double2(c0, c1);
+        *reinterpret_cast<double2*>(ypart + (size_t)warp * 64 + oct * 8 + 2 * quad) =
+            make_double2((c[0][0] + c[1][0]) + (c[2][0] + c[3][0]), (c[0][1] + c[1][1]) + (c[2][1] + c[3][1]));
         __syncthreads();
         for (int i = tid; i < n_ch * 8; i += GM_THREADS) {
             const int ga = i >> 3, v = i & 7;

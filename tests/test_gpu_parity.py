@@ -1128,3 +1128,69 @@ def test_coupled_limits_of_the_table(wpcd):
     p = np.array([0.2, 0.5, 1.1, 2.0])          # away from p = 0: the single terms of l = 7 are not integrable there
     q = np.array([0.1, 0.6, 1.4])
     _compare_full(wpcd, p, q, 5, gch, tab)
+
+
+class _Guarded:
+    """A device buffer with sentinel bands in front of it and behind it (compute-sanitizer is closed on the GPU pool: this is
+    the bounds check the tests can make themselves)."""
+    BAND = 4096         # bytes
+
+    def __init__(self, torch, n, dtype):
+        self.item = torch.empty(0, dtype=dtype).element_size()
+        self.g = self.BAND // self.item
+        self.full = torch.empty(n + 2 * self.g, dtype=dtype, device="cuda")
+        self.full.view(torch.uint8).fill_(0xA5)
+        self.view = self.full[self.g:self.g + n]
+        self.torch = torch
+
+    def intact(self):
+        b = self.full.view(self.torch.uint8)
+        n = self.BAND
+        return bool((b[:n] == 0xA5).all().item()) and bool((b[b.numel() - n:] == 0xA5).all().item())
+
+
+@pytest.mark.parametrize("model", ["swave", "nd"])
+def test_no_write_outside_the_buffers(wpcd, model):
+    """Every output buffer of count / build / the products sits between sentinel bands that must come back untouched, and
+    the matrix built into them is the one of the ordinary path.  Sizes are ragged on purpose (7 x 9 cells, n = 10; the
+    coupled set has 18 channels: partial element tiles, a partial moment chunk, partial row groups of the tensor-core product)."""
+    torch = _torch()
+    p, q = wi.tan2_grid(7, 1.0, 0.1, seed=51), wi.tan2_grid(9, 0.9, 0.1, seed=52)
+    grid = wpcd.wpcd_grid_create(p, q)
+    if model == "swave":
+        gch = wpcd.wpcd_channels_create(wpcd.WPCD_SPINLESS_SWAVE, g0=0.5)
+    else:
+        gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=2)
+    ref = wpcd.build_perm(grid, gch, 10)
+    rows, n_geo = ref.rows, (len(p) - 1) * (len(q) - 1)
+    row_ptr, geo_row_ptr = _Guarded(torch, rows + 1, torch.int64), _Guarded(torch, n_geo + 1, torch.int32)
+    nnz, nnz_geo = wpcd.wpcd_perm_count(grid, gch, 10, row_ptr.view, geo_row_ptr.view)
+    assert (nnz, nnz_geo) == (ref.nnz, ref.nnz_geo)
+    col_idx, values = _Guarded(torch, nnz, torch.int32), _Guarded(torch, nnz, torch.float64)
+    ws = _Guarded(torch, max(wpcd.wpcd_perm_workspace_bytes(gch, nnz_geo), 256), torch.uint8)
+    wpcd.wpcd_perm_build(grid, gch, 10, row_ptr.view, geo_row_ptr.view, ws.view, col_idx.view, values.view)
+    torch.cuda.synchronize()
+    for name, b in (("row_ptr", row_ptr), ("geo_row_ptr", geo_row_ptr), ("col_idx", col_idx), ("values", values), ("workspace", ws)):
+        assert b.intact(), name
+    assert torch.equal(row_ptr.view, ref.row_ptr) and torch.equal(geo_row_ptr.view, ref.geo_row_ptr)
+    assert torch.equal(col_idx.view, ref.col_idx) and torch.equal(values.view, ref.values)
+    # the products: y between bands, every pass width of both products
+    for n_vec in (1, 2, 3, 4, 5, 8, 11):
+        x = torch.from_numpy(np.stack([wi.normal_vector(rows, k=1300 + k) for k in range(n_vec)])).cuda()
+        y = _Guarded(torch, n_vec * rows, torch.float64)
+        wpcd.wpcd_perm_apply(rows, row_ptr.view, col_idx.view, values.view, x, y.view, n_vec=n_vec)
+        torch.cuda.synchronize()
+        assert y.intact(), ("apply", n_vec)
+        y_csr = y.view.clone()
+        assert bool(torch.isfinite(y_csr).all().item())
+        if model == "nd":
+            y = _Guarded(torch, n_vec * rows, torch.float64)
+            wpcd.wpcd_perm_apply_blocked(grid, gch, row_ptr.view, geo_row_ptr.view, col_idx.view, values.view, x, y.view, n_vec=n_vec)
+            torch.cuda.synchronize()
+            assert y.intact(), ("apply_blocked", n_vec)
+            scale = float(torch.abs(y_csr).max().item())
+            assert float(torch.abs(y.view - y_csr).max().item()) <= 1e-12 * max(scale, 1.0) * 50
+    y = _Guarded(torch, 6 * rows, torch.float64)
+    wpcd.wpcd_perm_apply_chain(rows, row_ptr.view, col_idx.view, values.view, x[0].contiguous(), y.view, 6)
+    torch.cuda.synchronize()
+    assert y.intact(), "apply_chain"

@@ -204,6 +204,22 @@ wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* grid, const wpcd_channels* 
                                     const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
                                     const double* x_dev, double* y_dev, int n_vec, void* cuda_stream);
 
+/* The same product for callers that must not allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): 1 <= n_vec <= 8 vectors in ONE tensor-core pass, whose scratch -- the interleaved copy of the x vectors,
+ * 64 bytes per row -- lives in a fixed device array of the library (WPCD_NOALLOC_MAX_ROWS rows = 16 MiB, held by every GPU
+ * that loads the library until the process exits) instead of a stream-ordered allocation.  The call makes no cudaMalloc,
+ * cudaMallocAsync, cudaFree or other allocating call.  Arguments, layout and result as wpcd_perm_apply_blocked (same
+ * kernel, same summation order: identical output for 5 <= n_vec <= 8).
+ * WPCD_ERR_UNSUPPORTED if rows = n_channels * n_p * n_q > WPCD_NOALLOC_MAX_ROWS, n_channels > 64 or n_vec > 8 -- nothing is
+ * launched then; use wpcd_perm_apply_blocked.
+ * All calls on a device share the array: each call overwrites every word it later reads (nothing has to be cleared
+ * between calls), but two calls that overlap on the GPU -- different streams without an ordering between them -- race on
+ * it and give wrong results.  Calls on one stream are ordered and safe.  Asynchronous. */
+#define WPCD_NOALLOC_MAX_ROWS 262144
+wpcd_status wpcd_perm_apply_blocked_noalloc(const wpcd_grid* grid, const wpcd_channels* channels, const int64_t* row_ptr_dev,
+                                            const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                            const double* x_dev, double* y_dev, int n_vec, void* cuda_stream);
+
 /* The dependent products of the simple iteration (paper step 5; Neumann terms):
  * y_k = P0 y_{k-1}, k = 1 .. n_iter, y_0 = x.  y_dev holds all iterates, y_dev[(k-1)*rows + r] = (P0^k x)[r], dev;
  * x_dev [rows], dev, must not overlap y_dev.  A matrix in the size window where it pays (about 1.6e4 <= nnz <=

@@ -26,13 +26,14 @@ WPCD_ND = 1
 WPCD_RULE_KINK_SPLIT = 0x100   # OR into n_quad: kink-split rule RS(n) (R14)
 WPCD_RULE_ANALYTIC_U = 0x200   # OR into n_quad: rule RA(n), exact x-integral, s-wave only (R15)
 WPCD_MAX_QUAD = 64
+WPCD_NOALLOC_MAX_ROWS = 262144   # rows wpcd_perm_apply_blocked_noalloc accepts (its fixed 16 MiB scratch array)
 
 EXPORTS = [
     "wpcd_last_error", "wpcd_grid_create", "wpcd_grid_destroy", "wpcd_channels_create",
     "wpcd_channels_create_from_table", "wpcd_channels_destroy", "wpcd_channels_count", "wpcd_channels_pairs",
     "wpcd_channels_terms", "wpcd_channels_monomials", "wpcd_channels_coefficients", "wpcd_channels_get_quantum_numbers", "wpcd_channels_get_table", "wpcd_rows",
     "wpcd_geo_rows", "wpcd_perm_count", "wpcd_perm_workspace_bytes", "wpcd_perm_build", "wpcd_perm_apply",
-    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_perm_apply_blocked_host", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
+    "wpcd_perm_apply_host", "wpcd_perm_apply_complex", "wpcd_perm_apply_interleaved", "wpcd_perm_apply_chain", "wpcd_perm_apply_blocked", "wpcd_perm_apply_blocked_noalloc", "wpcd_perm_apply_blocked_host", "wpcd_block_apply", "wpcd_kernel_apply", "wpcd_neumann_terms",
     "wpcd_pade_sum", "wpcd_fp64_peak", "wpcd_launch_count", "wpcd_trace_enable", "wpcd_trace_read", "wpcd_debug_set",
 ]
 TRACE_STAGES = ["geo_count", "scan", "geo_index", "fill_swave", "moments", "contract"]
@@ -85,6 +86,7 @@ def load():
     L.wpcd_perm_apply_complex.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_interleaved.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_blocked.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    L.wpcd_perm_apply_blocked_noalloc.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_perm_apply_blocked_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
     L.wpcd_perm_apply_chain.argtypes = [i64, vp, vp, vp, vp, vp, i32, vp]
     L.wpcd_block_apply.argtypes = [i32, i32, i32, vp, i32, vp, vp, i32, vp]
@@ -293,6 +295,16 @@ def wpcd_perm_apply_blocked(grid, channels, row_ptr, geo_row_ptr, col_idx, value
     _check(load().wpcd_perm_apply_blocked(grid.handle, channels.handle, _dev_ptr(row_ptr, torch.int64), _dev_ptr(geo_row_ptr, torch.int32),
                                           _dev_ptr(col_idx, torch.int32), _dev_ptr(values, torch.float64), _dev_ptr(x, torch.float64),
                                           _dev_ptr(y, torch.float64), n_vec, _stream_ptr(stream)))
+
+
+def wpcd_perm_apply_blocked_noalloc(grid, channels, row_ptr, geo_row_ptr, col_idx, values, x, y, n_vec=1, stream=None):
+    """wpcd_perm_apply_blocked for callers that must not allocate: n_vec <= 8, rows <= WPCD_NOALLOC_MAX_ROWS, scratch in a
+    fixed device array of the library (calls that overlap on the GPU race on it)."""
+    import torch
+
+    _check(load().wpcd_perm_apply_blocked_noalloc(grid.handle, channels.handle, _dev_ptr(row_ptr, torch.int64), _dev_ptr(geo_row_ptr, torch.int32),
+                                                  _dev_ptr(col_idx, torch.int32), _dev_ptr(values, torch.float64), _dev_ptr(x, torch.float64),
+                                                  _dev_ptr(y, torch.float64), n_vec, _stream_ptr(stream)))
 
 
 def wpcd_perm_apply_blocked_host(grid, channels, row_ptr, geo_row_ptr, col_idx, values, x_host, y_host, x_dev, y_dev, n_vec=1, stream=None):

@@ -724,6 +724,27 @@ wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* g, const wpcd_channels* c, 
     return WPCD_OK;
 }
 
+wpcd_status wpcd_perm_apply_blocked_noalloc(const wpcd_grid* g, const wpcd_channels* c, const int64_t* row_ptr_dev,
+                                            const int32_t* geo_row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
+                                            const double* x_dev, double* y_dev, int n_vec, void* cuda_stream)
+{
+    if (!g || !c) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_noalloc: null handle");
+    if (n_vec < 0) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_noalloc: negative size");
+    const int64_t rows = wpcd_rows(g, c);
+    if (rows == 0 || n_vec == 0) return WPCD_OK;
+    if (n_vec > 8) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_apply_blocked_noalloc: at most 8 vectors per call");
+    if (rows > WPCD_NOALLOC_MAX_ROWS)
+        return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_apply_blocked_noalloc: " + std::to_string(rows) + " rows exceed WPCD_NOALLOC_MAX_ROWS = " +
+                                              std::to_string(WPCD_NOALLOC_MAX_ROWS) + " (the fixed scratch array); use wpcd_perm_apply_blocked");
+    if (c->n_ch > 64) return fail(WPCD_ERR_UNSUPPORTED, "wpcd_perm_apply_blocked_noalloc: more than 64 channels");
+    if (!row_ptr_dev || !geo_row_ptr_dev || !x_dev || !y_dev) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_noalloc: null pointer");
+    if (!c->ncoupled_dev) return fail(WPCD_ERR_CUDA, "wpcd_perm_apply_blocked_noalloc: channel tables are not on a device (no CUDA device?)");
+    if (c->total_coupled > 0 && (!col_idx_dev || !values_dev)) return fail(WPCD_ERR_INVALID_ARG, "wpcd_perm_apply_blocked_noalloc: null matrix arrays");
+    cudaError_t err = launch_spmv_blocked_noalloc(g, c, geo_row_ptr_dev, col_idx_dev, values_dev, x_dev, y_dev, n_vec, static_cast<cudaStream_t>(cuda_stream));
+    if (err != cudaSuccess) return cuda_fail(err, "wpcd_perm_apply_blocked_noalloc");
+    return WPCD_OK;
+}
+
 wpcd_status wpcd_perm_apply_chain(int64_t rows, const int64_t* row_ptr_dev, const int32_t* col_idx_dev, const double* values_dev,
                                   const double* x_dev, double* y_dev, int n_iter, void* cuda_stream)
 {

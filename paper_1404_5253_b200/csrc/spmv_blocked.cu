@@ -12,6 +12,7 @@
 // through a work queue (row lengths are very skewed and grow with the cell indices).
 #include <algorithm>
 #include <atomic>
+#include <mutex>
 
 #include "wpcd_internal.h"
 
@@ -323,6 +324,11 @@ spmv_georow_mma8_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row
 
 }  // namespace
 
+// Scratch of wpcd_perm_apply_blocked_noalloc: the interleaved copy of up to 8 x vectors of a matrix with at most
+// WPCD_NOALLOC_MAX_ROWS rows (16 MiB), held by every device that loads the library until the process exits.  In host code this
+// name is a host-side stand-in, not a device address: the launcher below asks cudaGetSymbolAddress for the address.
+static __device__ __align__(256) double g_noalloc_xi[(size_t)WPCD_NOALLOC_MAX_ROWS * 8];
+
 namespace wpcd_detail {
 
 bool use_pdl();
@@ -414,6 +420,51 @@ cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, con
         if (err != cudaSuccess) return err;
     }
     return cudaSuccess;
+}
+
+// The tensor-core pass with its scratch in g_noalloc_xi: no cudaMalloc / cudaFree of any kind.  nv = 1 .. 8 vectors, n_ch <= 64,
+// rows <= WPCD_NOALLOC_MAX_ROWS (checked by the caller).  Every call uses the same array: the interleave kernel rewrites all
+// 8 rows words the product reads (zeros for the vectors nv .. 7), so nothing of an earlier call is seen; two calls that
+// overlap on the GPU (different streams) race on it.
+cudaError_t launch_spmv_blocked_noalloc(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
+                                        const double* values, const double* x, double* y, int nv, cudaStream_t st)
+{
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static double* xi_of_device[MAX_DEV] = {};             // device address of g_noalloc_xi, per device
+    static std::atomic<unsigned int> next_slot{1u << 21};
+    int dev = 0, sms = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return err;
+    if (dev < 0 || dev >= MAX_DEV) return cudaErrorInvalidDevice;
+    double* xi = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (!xi_of_device[dev]) {                          // once per device, with that device current
+            void* ptr = nullptr;
+            err = cudaGetSymbolAddress(&ptr, g_noalloc_xi);
+            if (err != cudaSuccess) return err;
+            xi_of_device[dev] = static_cast<double*>(ptr);
+        }
+        xi = xi_of_device[dev];
+    }
+    err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (err != cudaSuccess) return err;
+    const int n_geo = g->n_p * g->n_q;
+    const int64_t rows = (int64_t)ch->n_ch * n_geo;
+    if (rows > WPCD_NOALLOC_MAX_ROWS || ch->n_ch > 8 * GM_GROUPS || nv < 1 || nv > 8) return cudaErrorInvalidValue;
+    const int cap = 2560;
+    const size_t smem = sizeof(double) * ((size_t)(cap + 4) * 8 + (size_t)GM_WARPS * 64) + sizeof(int32_t) * ((size_t)cap + (size_t)ch->n_ch * ch->n_ch);
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    err = cudaFuncSetAttribute(spmv_georow_mma8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    const int blocks = std::max(1, std::min(n_geo, sms));
+    const int slot = (int)(next_slot.fetch_add(1) % GB_RING);
+    g_launches += 2;
+    interleave8_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(rows, nv, x, rows, xi);
+    spmv_georow_mma8_kernel<<<blocks, GM_THREADS, smem, st>>>(n_geo, ch->n_ch, geo_row_ptr, col_idx, values, ch->chan_off_dev, ch->ncoupled_dev,
+                                                             ch->run_ptr_dev, ch->runs_dev, ch->first_gamma, ch->first_gp, xi, y, rows, nv, cap, slot);
+    return cudaGetLastError();
 }
 
 }  // namespace wpcd_detail

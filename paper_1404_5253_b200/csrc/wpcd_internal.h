@@ -175,6 +175,8 @@ cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const 
 // spmv_blocked.cu
 cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
                                 const double* values, const double* x, double* y, int n_vec, cudaStream_t st);
+cudaError_t launch_spmv_blocked_noalloc(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
+                                        const double* values, const double* x, double* y, int nv, cudaStream_t st);
 cudaError_t launch_spmv_chain(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                               const double* x, double* y, int n_iter, int64_t nnz, cudaStream_t st, int* fused);
 cudaError_t run_fp64_peak(cudaStream_t st, double* flops_out);

@@ -21,6 +21,24 @@ DebugSwitches g_debug;
 
 void set_error(const std::string& msg) { t_error = msg; }
 
+cudaError_t raise_dyn_smem(const void* kernel, size_t bytes)
+{
+    static std::mutex mu;
+    static std::map<std::pair<const void*, int>, size_t> have;      // (kernel, device) -> limit in force
+    if (bytes <= 48 * 1024) return cudaSuccess;                       // the default limit covers it
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return err;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t& h = have[{kernel, dev}];
+    if (bytes > h) {
+        err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (err != cudaSuccess) return err;
+        h = bytes;
+    }
+    return cudaSuccess;
+}
+
 static wpcd_status fail(wpcd_status code, const std::string& msg)
 {
     set_error(msg);

@@ -689,7 +689,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     const size_t mom2_smem = sizeof(double) * (size_t)moment2_smem_doubles(s2);
 #define WPCD_MOM2(MS, SPL)                                                                                                        \
     do {                                                                                                                      \
-        err = cudaFuncSetAttribute(moments_kernel<MS, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom_smem);           \
+        err = raise_dyn_smem(moments_kernel<MS, SPL>, mom_smem);           \
         if (err != cudaSuccess) return err;                                                                                   \
         moments_kernel<MS, SPL><<<blocks, mom_warps * 32, mom_smem, st>>>(qr, g->p_dev, g->q_dev, g->n_q, sh, e0, e1, ws.geo_col,      \
                                                                      ws.geo_row, ws.geo_phi, ch->ll_pack_dev,                 \
@@ -698,7 +698,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
 #define WPCD_MOM(MS) do { if (split) WPCD_MOM2(MS, true); else WPCD_MOM2(MS, false); } while (0)
 #define WPCD_MOMF3(MS, KTV, MTV)                                                                                                    \
     do {                                                                                                                          \
-        err = cudaFuncSetAttribute(moments2_kernel<MS, KTV, MTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mom2_smem);      \
+        err = raise_dyn_smem(moments2_kernel<MS, KTV, MTV>, mom2_smem);      \
         if (err != cudaSuccess) return err;                                                                                       \
         moments2_kernel<MS, KTV, MTV><<<(unsigned)(e1 - e0), 32, mom2_smem, st>>>(qr, g->p_dev, g->q_dev, g->n_q, s2, e0, e1, ws.geo_col, \
                                                                                   ws.geo_row, ws.geo_phi, ch->ll_pack_dev, ch->trip_pack_dev, \
@@ -706,7 +706,7 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     } while (0)
 #define WPCD_MOMF2(MS, KTV) do { if (s2.K1 <= 8) WPCD_MOMF3(MS, KTV, 1); else WPCD_MOMF3(MS, KTV, 2); } while (0)
 #define WPCD_MOMF(MS) do { if (s2.NP == 8) WPCD_MOMF2(MS, 2); else WPCD_MOMF2(MS, 3); } while (0)
-    err = cudaFuncSetAttribute(contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem);
+    err = raise_dyn_smem(contract_kernel, ct_smem);
     if (err != cudaSuccess) return err;
     {
         StageTimer timer(WPCD_STAGE_GEO_INDEX, st);

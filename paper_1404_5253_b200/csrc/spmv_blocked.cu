@@ -351,7 +351,7 @@ static cudaError_t launch_georow(const wpcd_grid* g, const wpcd_channels* ch, co
     const int cap = forced > 0 ? forced : (NV == 1 ? 1536 : 3072);        // doubles per vector
     const size_t smem = sizeof(double) * ((size_t)cap * NV + (size_t)ch->n_ch * NV) + sizeof(int32_t) * (size_t)cap;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    cudaError_t err = cudaFuncSetAttribute(spmv_georow_kernel<NV, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t err = raise_dyn_smem(spmv_georow_kernel<NV, THREADS>, smem);
     if (err != cudaSuccess) return err;
     int per_sm = 0;
     err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spmv_georow_kernel<NV, THREADS>, THREADS, smem);
@@ -379,7 +379,7 @@ static cudaError_t launch_georow_mma8(const wpcd_grid* g, const wpcd_channels* c
     const int cap = forced > 0 ? forced : 2560;
     const size_t smem = sizeof(double) * ((size_t)(cap + 4) * 8 + (size_t)GM_WARPS * 64) + sizeof(int32_t) * ((size_t)cap + (size_t)ch->n_ch * ch->n_ch);
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    cudaError_t err = cudaFuncSetAttribute(spmv_georow_mma8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t err = raise_dyn_smem(spmv_georow_mma8_kernel, smem);
     if (err != cudaSuccess) return err;
     const int blocks = std::max(1, std::min(n_geo, sms));
     const int slot = (int)(next_slot.fetch_add(1) % GB_RING);
@@ -456,7 +456,7 @@ cudaError_t launch_spmv_blocked_noalloc(const wpcd_grid* g, const wpcd_channels*
     const int cap = 2560;
     const size_t smem = sizeof(double) * ((size_t)(cap + 4) * 8 + (size_t)GM_WARPS * 64) + sizeof(int32_t) * ((size_t)cap + (size_t)ch->n_ch * ch->n_ch);
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    err = cudaFuncSetAttribute(spmv_georow_mma8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    err = raise_dyn_smem(spmv_georow_mma8_kernel, smem);
     if (err != cudaSuccess) return err;
     const int blocks = std::max(1, std::min(n_geo, sms));
     const int slot = (int)(next_slot.fetch_add(1) % GB_RING);

@@ -172,6 +172,11 @@ cudaError_t launch_spmv(int64_t rows, const int64_t* row_ptr, const int32_t* col
                         const double* x, double* y, int n_vec, cudaStream_t st);
 cudaError_t launch_spmv_interleaved(int64_t rows, const int64_t* row_ptr, const int32_t* col_idx, const double* values,
                                     const double* x, double* y, int n_vec, int n_inter, cudaStream_t st);
+// api.cu: the dynamic shared-memory limit of a kernel belongs to the function (per device) and setting it REPLACES the value.
+// This keeps the largest size ever asked for, under a lock: launches from several host threads with different sizes
+// (two builds with different channel sets) cannot undercut each other between the attribute call and the launch.
+cudaError_t raise_dyn_smem(const void* kernel, size_t bytes);
+template <class K> inline cudaError_t raise_dyn_smem(K* kernel, size_t bytes) { return raise_dyn_smem(reinterpret_cast<const void*>(kernel), bytes); }
 // spmv_blocked.cu
 cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, const int32_t* geo_row_ptr, const int32_t* col_idx,
                                 const double* values, const double* x, double* y, int n_vec, cudaStream_t st);

@@ -799,6 +799,50 @@ def test_concurrent_builds_of_different_orders(wpcd):
                 assert torch.equal(outs[k][3], refs[k].col_idx) and torch.equal(outs[k][4], refs[k].values), k
 
 
+def test_builds_and_products_from_two_host_threads(wpcd):
+    """Two host threads, each with its own stream, grid handle and channel set (different table sizes, so different
+    shared-memory sizes of the same kernels), build and multiply at the same time: the results are those of the serial calls
+    (the dynamic shared-memory limit of a kernel is only ever raised, under a lock)."""
+    import threading
+
+    torch = _torch()
+    sets = [dict(two_J=1, parity=1, j_pair_max=1), dict(two_J=5, parity=-1, j_pair_max=3)]
+    p = wi.tan2_grid(12, 1.0, 0.1, seed=91)
+    work = []
+    for kw in sets:
+        grid = wpcd.wpcd_grid_create(p, p)
+        gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_T=1, **kw)
+        ref = wpcd.build_perm(grid, gch, 8)
+        x = torch.from_numpy(np.stack([wi.normal_vector(ref.rows, k=1500 + k) for k in range(8)])).cuda()
+        y_ref = torch.empty_like(x)
+        wpcd.wpcd_perm_apply_blocked(grid, gch, ref.row_ptr, ref.geo_row_ptr, ref.col_idx, ref.values, x, y_ref, n_vec=8)
+        work.append((grid, gch, ref, x, y_ref))
+    torch.cuda.synchronize()
+    errors = []
+
+    def run(k):
+        try:
+            grid, gch, ref, x, y_ref = work[k]
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for _ in range(6):
+                    m = wpcd.build_perm(grid, gch, 8, stream=st)
+                    y = torch.empty_like(x)
+                    wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y, n_vec=8, stream=st)
+                    st.synchronize()
+                    assert torch.equal(m.col_idx, ref.col_idx) and torch.equal(m.values, ref.values), k
+                    assert torch.equal(y, y_ref), k
+        except BaseException as e:   # noqa: BLE001 -- reported in the main thread
+            errors.append((k, repr(e)))
+
+    threads = [threading.Thread(target=run, args=(k,)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
 def test_apply_ignores_columns_a_row_does_not_reference(wpcd):
     """x[0] = inf / nan must not leak into rows that do not reference column 0 (padding slots of the batched loads used to
     multiply 0 * x[0]); every product variant, short and long rows."""

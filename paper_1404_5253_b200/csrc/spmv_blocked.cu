@@ -174,6 +174,15 @@ spmv_georow_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row_ptr,
     }
 }
 
+// 8-byte load of a matrix value that asks L2 to bring the whole 256-byte neighbourhood from DRAM: the A-fragment loads below
+// touch 32 bytes per row at a time (7.40 -> 7.15 ms on the 3.2e9-nonzero matrix)
+__device__ __forceinline__ double ld_value_l2_256(const double* p)
+{
+    double v;
+    asm volatile("ld.global.nc.L2::256B.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+
 __device__ __forceinline__ void dmma_884g(double& c0, double& c1, double a, double b)
 {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
@@ -283,8 +292,8 @@ spmv_georow_mma8_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row
 #pragma unroll
                             for (int k = 0; k < GM_UNR; ++k) {
                                 const bool in = s + 4 * k + quad < cs;
-                                a[k] = (in && rk >= 0) ? __ldg(vp + s + 4 * k) : 0.0;
-                                aq[k] = (in && rq >= 0) ? __ldg(vq + s + 4 * k) : 0.0;
+                                a[k] = (in && rk >= 0) ? ld_value_l2_256(vp + s + 4 * k) : 0.0;
+                                aq[k] = (in && rq >= 0) ? ld_value_l2_256(vq + s + 4 * k) : 0.0;
                             }
 #pragma unroll
                             for (int k = 0; k < GM_UNR; ++k) {

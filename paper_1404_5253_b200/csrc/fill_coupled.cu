@@ -338,6 +338,9 @@ __host__ __device__ inline int moment2_smem_doubles(const MomentShape2& s)
     return (s.n * NODE_F + s.K1 * s.RS + (2 * s.LM1 + 1) * s.RS + s.K1 * s.IS + s.G * 2 * s.CP + s.n_ab + 1) & ~1;
 }
 
+#ifndef MOM_HOIST_MAX
+#define MOM_HOIST_MAX 14
+#endif
 template <int MAXS, int KT, int MT>
 __global__ void __launch_bounds__(32, 16)
 moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape2 sh,
@@ -360,18 +363,31 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
     double* csp = cs + G * 2 * CP;            // [n_ab]     c^a s^b of one phi-node
     // the padding slots of the power tables must read as zero (they feed the MMAs); P_k only has to be finite there
     for (int i = lane; i < (K1 + 2 * LM1 + 1) * RS; i += 32) Pt[i] = 0.0;
-    // per monomial: offset into Ib (low 16 bits) and into csp (high 16 bits)
-    int pk[MAXS];
+    // per monomial: BYTE offsets from sm of its I entry (low 16 bits) and of its c^a s^b entry (high 16 bits): the multiply-add
+    // of step 4 then needs no address arithmetic beyond one mask / shift, and no predicate -- a slot beyond n_mu points both
+    // at a word of the zero row of pa (the whole block of a warp is < 64 KB, checked by the host)
+    const unsigned off_zero = (unsigned)((pa + LM1 * RS - sm) * sizeof(double));
+    const unsigned off_ib = (unsigned)((Ib - sm) * sizeof(double)), off_csp = (unsigned)((csp - sm) * sizeof(double));
+    unsigned pk[MAXS];
     double acc[MAXS];
 #pragma unroll
     for (int s = 0; s < MAXS; ++s) {
         const int m = lane + 32 * s;
         acc[s] = 0.0;
-        pk[s] = -1;
+        pk[s] = (off_zero << 16) | off_zero;
         if (m < n_mu) {
-            const int v = mu_pack[m], tp = trip_pack[v & 0xffff];
-            pk[s] = ((tp & 0xff) * IS + (tp >> 8)) | ((v >> 16) << 16);     // mu_pack: triple | ab index << 16
+            const int v = mu_pack[m], tp = trip_pack[v & 0xffff];            // mu_pack: triple | ab index << 16
+            pk[s] = ((off_csp + 8u * (unsigned)(v >> 16)) << 16) | (off_ib + 8u * (unsigned)((tp & 0xff) * IS + (tp >> 8)));
         }
+    }
+    const char* smb = reinterpret_cast<const char*>(sm);
+    // this lane's (up to two) entries of the c^a s^b table: byte offsets of c^a and s^b inside a phi-node's power block
+    unsigned abo[2];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const int idx = lane + 32 * j;
+        const int ab = idx < n_ab ? ab_pack[idx] : 0;
+        abo[j] = (8u * (unsigned)(ab & 0xff) << 16) | 8u * (unsigned)(CP + (ab >> 8));
     }
     // this lane's (l, l') of every n-tile: where its rows of the power tables start (a column beyond n_ll reads the zero row)
     const double* qa[4];
@@ -443,9 +459,16 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
             for (int g = 0; g < cnt; ++g) {
                 if (nodeS[(m0 + g) * NODE_F] == 0.0) continue;           // warp-uniform
                 // c^a s^b table of this phi-node
-                for (int idx = lane; idx < n_ab; idx += 32) {
-                    const int ab = ab_pack[idx];
-                    csp[idx] = cs[(g * 2 + 0) * CP + (ab & 0xff)] * cs[(g * 2 + 1) * CP + (ab >> 8)];
+                {
+                    const char* csg = reinterpret_cast<const char*>(cs + g * 2 * CP);
+#pragma unroll
+                    for (int j = 0; j < 2; ++j)
+                        if (lane + 32 * j < n_ab)
+                            csp[lane + 32 * j] = *reinterpret_cast<const double*>(csg + (abo[j] >> 16)) * *reinterpret_cast<const double*>(csg + (abo[j] & 0xffffu));
+                    for (int idx = lane + 64; idx < n_ab; idx += 32) {      // more than 64 exponent pairs: not for l <= 4
+                        const int ab = ab_pack[idx];
+                        csp[idx] = cs[(g * 2 + 0) * CP + (ab & 0xff)] * cs[(g * 2 + 1) * CP + (ab >> 8)];
+                    }
                 }
                 // ---- step 3: I[k][l,l'] = sum_r P_k(x_r) T_r[l,l'] on the FP64 tensor cores
                 const int s0 = g * NP;                                 // first node slot of this phi-node
@@ -472,8 +495,9 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
                 // ---- step 4: M[mu] += c^{A+1} s^{B+1} I[k][l,l'], lane = monomial
 #pragma unroll
                 for (int s = 0; s < MAXS; ++s) {
-                    const int v = pk[s];
-                    if (v >= 0) acc[s] = fma(csp[v >> 16], Ib[v & 0xffff], acc[s]);
+                    unsigned v = pk[s];
+                    if (MAXS > MOM_HOIST_MAX) asm volatile("" : "+r"(v));      // many slots: the two addresses are formed here, not kept in registers
+                    acc[s] = fma(*reinterpret_cast<const double*>(smb + (v >> 16)), *reinterpret_cast<const double*>(smb + (v & 0xffffu)), acc[s]);
                 }
                 __syncwarp();
             }
@@ -685,7 +709,8 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
     s2.RS = s2.G * s2.NP; while (s2.RS % 16 != 4) ++s2.RS;
     s2.K1 = ch->k_max + 1; s2.NT = (ch->n_ll + 7) / 8; s2.IS = 8 * s2.NT + 2; s2.LM1 = ch->l_max + 1; s2.CP = 2 * ch->l_max + 3;
     s2.n_ab = ch->n_ab; s2.n_ll = ch->n_ll; s2.n_mu = ch->n_mu;
-    const bool fast = !split && n_quad >= 5 && n_quad <= 12 && s2.K1 <= 16 && s2.NT <= 4 && maxs <= 20 && s2.K1 * s2.IS < 65536;
+    const bool fast = !split && n_quad >= 5 && n_quad <= 12 && s2.K1 <= 16 && s2.NT <= 4 && maxs <= 20 &&
+                      sizeof(double) * (size_t)moment2_smem_doubles(s2) < 65536;     // 16-bit byte offsets inside a warp's block
     const size_t mom2_smem = sizeof(double) * (size_t)moment2_smem_doubles(s2);
 #define WPCD_MOM2(MS, SPL)                                                                                                        \
     do {                                                                                                                      \

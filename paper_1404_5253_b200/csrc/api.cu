@@ -276,6 +276,17 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->n_ab = (int)c->ab_pack.size();
     if (c->n_ab >= 32768) return fail(WPCD_ERR_UNSUPPORTED, "too many cos/sin exponent pairs");
     c->n_mu = (int)c->mu_pack.size();
+    // the same per monomial with the triple resolved: offset k IS + (l,l') into the I table of moments2_kernel (row stride
+    // IS = 8 ceil(n_ll / 8) + 2) | exponent-pair index << 16 -- one table look-up per monomial instead of two dependent ones
+    {
+        const int IS = 8 * (((int)c->ll_pack.size() + 7) / 8) + 2;
+        c->mu_ib_pack.resize(c->mu_pack.size());
+        for (size_t m = 0; m < c->mu_pack.size(); ++m) {
+            const int v = c->mu_pack[m], tp = c->trip_pack[v & 0xffff];
+            const int o = (tp & 0xff) * IS + (tp >> 8);
+            c->mu_ib_pack[m] = (o < 65536 ? o : 65535) | (v & ~0xffff);       // beyond 16 bits: moments2_kernel is not taken (K1 IS < 65536)
+        }
+    }
     // ---- contraction tables: (l, l') groups -> items (at most 8 pairs of the group with exactly the same monomials: for the nd
     // tables a class separates the (lambda, lambda') values, whose k-ranges differ);
     // every group's tables are one blob [items | pairs | idx | g] that the kernel copies to shared memory verbatim
@@ -359,14 +370,14 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return WPCD_OK; }
     // all device tables in ONE allocation and ONE copy (eight separate synchronous copies cost ~55 us per handle)
     auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
-    constexpr int NT = 11;
+    constexpr int NT = 12;
     const size_t sz[NT] = {sizeof(int32_t) * c->ncoupled.size(), sizeof(int64_t) * chan_off.size(), sizeof(int32_t) * c->coupled_gp.size(),
                            sizeof(int32_t) * c->ll_pack.size(),  sizeof(int32_t) * c->trip_pack.size(), sizeof(int32_t) * c->mu_pack.size(),
                            sizeof(int32_t) * c->ab_pack.size(),  sizeof(wpcd_ct_group) * c->ct_groups.size(), c->ct_blob.size(),
-                           sizeof(int32_t) * c->run_ptr.size(),  sizeof(int4) * c->runs.size()};
+                           sizeof(int32_t) * c->run_ptr.size(),  sizeof(int4) * c->runs.size(), sizeof(int32_t) * c->mu_ib_pack.size()};
     const void* src[NT] = {c->ncoupled.data(), chan_off.data(), c->coupled_gp.data(), c->ll_pack.data(), c->trip_pack.data(),
                            c->mu_pack.data(), c->ab_pack.data(), c->ct_groups.data(), c->ct_blob.data(), c->run_ptr.data(),
-                           c->runs.data()};
+                           c->runs.data(), c->mu_ib_pack.data()};
     size_t off[NT + 1];
     off[0] = 0;
     for (int k = 0; k < NT; ++k) off[k + 1] = off[k] + pad(std::max<size_t>(sz[k], 1));
@@ -388,6 +399,7 @@ static wpcd_status finalize_channels(wpcd_channels* c)
     c->ct_blob_dev = c->tables_dev + off[8];
     c->run_ptr_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[9]);
     c->runs_dev = reinterpret_cast<int4*>(c->tables_dev + off[10]);
+    c->mu_ib_pack_dev = reinterpret_cast<int32_t*>(c->tables_dev + off[11]);
     return WPCD_OK;
 }
 

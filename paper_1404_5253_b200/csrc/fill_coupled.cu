@@ -345,8 +345,8 @@ template <int MAXS, int KT, int MT>
 __global__ void __launch_bounds__(32, 16)
 moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict__ p, const double* __restrict__ q, int n_q, MomentShape2 sh,
                 int64_t e_begin, int64_t e_end, const int32_t* __restrict__ geo_col, const int32_t* __restrict__ geo_row,
-                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ trip_pack,
-                const int32_t* __restrict__ mu_pack, const int32_t* __restrict__ ab_pack, double* __restrict__ moments)
+                const double2* __restrict__ geo_phi, const int32_t* __restrict__ ll_pack, const int32_t* __restrict__ mu_ib_pack,
+                const int32_t* __restrict__ ab_pack, double* __restrict__ moments)
 {
     extern __shared__ double sm[];
     const int lane = threadIdx.x, quad = lane & 3, oct = lane >> 2;
@@ -376,8 +376,8 @@ moments2_kernel(const __grid_constant__ QuadRule rule, const double* __restrict_
         acc[s] = 0.0;
         pk[s] = (off_zero << 16) | off_zero;
         if (m < n_mu) {
-            const int v = mu_pack[m], tp = trip_pack[v & 0xffff];            // mu_pack: triple | ab index << 16
-            pk[s] = ((off_csp + 8u * (unsigned)(v >> 16)) << 16) | (off_ib + 8u * (unsigned)((tp & 0xff) * IS + (tp >> 8)));
+            const unsigned v = (unsigned)mu_ib_pack[m];                       // (k IS + ll) | ab index << 16
+            pk[s] = ((off_csp + 8u * (v >> 16)) << 16) | (off_ib + 8u * (v & 0xffffu));
         }
     }
     const char* smb = reinterpret_cast<const char*>(sm);
@@ -726,8 +726,8 @@ cudaError_t launch_fill_coupled(const wpcd_grid* g, const wpcd_channels* ch, int
         err = raise_dyn_smem(moments2_kernel<MS, KTV, MTV>, mom2_smem);      \
         if (err != cudaSuccess) return err;                                                                                       \
         moments2_kernel<MS, KTV, MTV><<<(unsigned)(e1 - e0), 32, mom2_smem, st>>>(qr, g->p_dev, g->q_dev, g->n_q, s2, e0, e1, ws.geo_col, \
-                                                                                  ws.geo_row, ws.geo_phi, ch->ll_pack_dev, ch->trip_pack_dev, \
-                                                                                  ch->mu_pack_dev, ch->ab_pack_dev, ws.moments);   \
+                                                                                  ws.geo_row, ws.geo_phi, ch->ll_pack_dev, ch->mu_ib_pack_dev, \
+                                                                                  ch->ab_pack_dev, ws.moments);   \
     } while (0)
 #define WPCD_MOMF2(MS, KTV) do { if (s2.K1 <= 8) WPCD_MOMF3(MS, KTV, 1); else WPCD_MOMF3(MS, KTV, 2); } while (0)
 #define WPCD_MOMF(MS) do { if (s2.NP == 8) WPCD_MOMF2(MS, 2); else WPCD_MOMF2(MS, 3); } while (0)

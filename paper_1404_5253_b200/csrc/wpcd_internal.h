@@ -74,6 +74,7 @@ struct wpcd_channels {
     std::vector<int32_t> ll_pack;     // [n_ll]   l | l' << 8            distinct (l, l')
     std::vector<int32_t> trip_pack;   // [n_trip] k | ll << 8            distinct (k, l, l'), sorted by (ll, k)
     std::vector<int32_t> mu_pack;     // [n_mu]   trip | ab << 16
+    std::vector<int32_t> mu_ib_pack;  // [n_mu]   (k IS + ll) | ab << 16: the triple resolved for moments2_kernel
     std::vector<int32_t> ab_pack;     // [n_ab]   (A+1) | (B+1) << 8       distinct exponent pairs of cos, sin
     int n_ab = 0;
     // contraction tables (host copies; the device copies sit in tables_dev)
@@ -90,6 +91,7 @@ struct wpcd_channels {
     int32_t* ll_pack_dev = nullptr;
     int32_t* trip_pack_dev = nullptr;
     int32_t* mu_pack_dev = nullptr;
+    int32_t* mu_ib_pack_dev = nullptr;
     int32_t* ab_pack_dev = nullptr;
     wpcd_ct_group* ct_groups_dev = nullptr;
     unsigned char* ct_blob_dev = nullptr;

@@ -415,7 +415,7 @@ cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, con
         const double* xv = x + (int64_t)v * rows;
         double* yv = y + (int64_t)v * rows;
         cudaError_t err;
-        // 5 .. 8 vectors: one tensor-core pass (7.4 ms on the 3.2e9-nonzero matrix whatever their number; the scalar kernels
+        // 5 .. 8 vectors: one tensor-core pass (7.1 ms on the 3.2e9-nonzero matrix whatever their number; the scalar kernels
         // take 7.0 ms for 4 vectors, 4.6 for 2, 4.0 for 1)
         if (n_vec - v >= 5 && ch->n_ch <= 8 * GM_GROUPS) {
             const int nv = std::min(8, n_vec - v);

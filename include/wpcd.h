@@ -191,9 +191,9 @@ wpcd_status wpcd_perm_apply_interleaved(int64_t rows, const int64_t* row_ptr_dev
  * shifted by gamma' * n_p * n_q.  One CTA per geometric row (i,j) gathers the values of x at those columns for all
  * channels into shared memory once, and the n_channels rows of that (i,j) then stream only their VALUES: 8 bytes per
  * nonzero from HBM instead of the 12 of the general CSR product, and one gather per (channel, geometric entry) instead of
- * one per nonzero (the SpMV is HBM-bound).  Several vectors share one pass over the matrix: 5 - 8 go
+ * one per nonzero (the SpMV is HBM-bound).  Several vectors share one pass over the matrix: 3 - 8 go
  * through the FP64 tensor cores (values as A fragments, the planes of the x tile as B; n_channels <= 64, else scalar
- * passes), fewer through scalar passes of 4, 2, 1; n_vec is cut into such passes.  A tensor-core pass works on an
+ * passes of 8, 4), fewer through scalar passes of 2, 1; n_vec is cut into such passes.  A tensor-core pass works on an
  * interleaved copy of its x vectors held in stream-ordered scratch (cudaMallocAsync / cudaFreeAsync on cuda_stream,
  * 64 rows bytes, released behind the product; allowed during stream capture).
  * geo_row_ptr_dev as written by wpcd_perm_count, col_idx_dev / values_dev by wpcd_perm_build, for THESE handles (not
@@ -209,7 +209,7 @@ wpcd_status wpcd_perm_apply_blocked(const wpcd_grid* grid, const wpcd_channels* 
  * 64 bytes per row -- lives in a fixed device array of the library (WPCD_NOALLOC_MAX_ROWS rows = 16 MiB, held by every GPU
  * that loads the library until the process exits) instead of a stream-ordered allocation.  The call makes no cudaMalloc,
  * cudaMallocAsync, cudaFree or other allocating call.  Arguments, layout and result as wpcd_perm_apply_blocked (same
- * kernel, same summation order: identical output for 5 <= n_vec <= 8).
+ * kernel, same summation order: identical output for 3 <= n_vec <= 8).
  * WPCD_ERR_UNSUPPORTED if rows = n_channels * n_p * n_q > WPCD_NOALLOC_MAX_ROWS, n_channels > 64 or n_vec > 8 -- nothing is
  * launched then; use wpcd_perm_apply_blocked.
  * All calls on a device share the array: each call overwrites every word it later reads (nothing has to be cleared
@@ -313,6 +313,7 @@ int64_t wpcd_launch_count(void);
  *   "no_pdl"                1: launch the products without programmatic dependent launch
  *   "chain_mode"            1: wpcd_perm_apply_chain fuses whenever the matrix fits on chip, 2: never fuses
  *   "blocked_tile_doubles"  > 0: size of the x tile of wpcd_perm_apply_blocked (small values exercise its chunked paths)
+ *   "blocked_no_mma"        1: wpcd_perm_apply_blocked never takes the tensor-core pass (scalar passes of 8, 4, 2, 1 vectors)
  * WPCD_ERR_INVALID_ARG for an unknown key. */
 wpcd_status wpcd_debug_set(const char* key, int64_t value);
 

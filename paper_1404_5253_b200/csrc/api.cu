@@ -1037,6 +1037,7 @@ wpcd_status wpcd_debug_set(const char* key, int64_t value)
     else if (k == "no_pdl") g_debug.no_pdl = (int)value;
     else if (k == "chain_mode") g_debug.chain_mode = (int)value;
     else if (k == "blocked_tile_doubles") g_debug.blocked_tile_doubles = (int)value;
+    else if (k == "blocked_no_mma") g_debug.blocked_no_mma = (int)value;
     else return fail(WPCD_ERR_INVALID_ARG, "wpcd_debug_set: unknown key " + k);
     return WPCD_OK;
 }

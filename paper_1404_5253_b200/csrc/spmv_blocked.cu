@@ -114,11 +114,18 @@ spmv_georow_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row_ptr,
                 for (int glo = 0; glo < n_ch; glo += gpc) {
                     const int ghi = min(n_ch, glo + gpc);
                     __syncthreads();                           // gcol is there; the previous X tile is no longer read
-                    for (int i = tid; i < (ghi - glo) * cs; i += GB_THREADS) {
-                        const int gg = i / cs, s = i - gg * cs;
-                        const double* xp = x + (int64_t)(glo + gg) * n_geo + gcol[s];
+                    {
+                        // tile entry i = (channel gg, geometric entry s), advanced without divisions
+                        const int n_tile = (ghi - glo) * cs;
+                        const int dq = GB_THREADS / cs, dr = GB_THREADS - dq * cs;
+                        int gg = tid / cs, s = tid - gg * cs;
+                        for (int i = tid; i < n_tile; i += GB_THREADS) {
+                            const double* xp = x + (int64_t)(glo + gg) * n_geo + gcol[s];
 #pragma unroll
-                        for (int v = 0; v < NV; ++v) X[v * cap + i] = __ldg(xp + v * ldx);
+                            for (int v = 0; v < NV; ++v) X[v * cap + i] = __ldg(xp + v * ldx);
+                            gg += dq; s += dr;
+                            if (s >= cs) { s -= cs; ++gg; }
+                        }
                     }
                     __syncthreads();
                     for (int ga = warp; ga < n_ch; ga += GB_WARPS) {
@@ -266,15 +273,22 @@ spmv_georow_mma8_kernel(int n_geo, int n_ch, const int32_t* __restrict__ geo_row
                 for (int glo = 0; glo < n_ch; glo += gpc) {
                     const int ghi = min(n_ch, glo + gpc);
                     __syncthreads();                           // gcol is there; the previous X tile is no longer read
-                    // x comes interleaved (xi[column][8]): 16 bytes per load, the four quarters of a 64-byte piece one after
-                    // the other (consecutive lanes write consecutive words of a plane)
-                    for (int qv = 0; qv < 4; ++qv)
-                        for (int i = tid; i < (ghi - glo) * cs; i += GM_THREADS) {
-                            const int gg = i / cs, s = i - gg * cs;
-                            const double2 xv = __ldg(reinterpret_cast<const double2*>(xi + ((int64_t)(glo + gg) * n_geo + gcol[s]) * 8) + qv);
-                            X[(2 * qv) * ps + i] = xv.x;
-                            X[(2 * qv + 1) * ps + i] = xv.y;
+                    // x comes interleaved (xi[column][8]): a thread takes tile entries i = tid, tid + GM_THREADS, ... and moves the
+                    // 64 bytes of each as four 16-byte loads; (channel gg, geometric entry s) of i advance without divisions
+                    {
+                        const int n_tile = (ghi - glo) * cs;
+                        const int dq = GM_THREADS / cs, dr = GM_THREADS - dq * cs;
+                        int gg = tid / cs, s = tid - gg * cs;
+                        for (int i = tid; i < n_tile; i += GM_THREADS) {
+                            const double2* xp = reinterpret_cast<const double2*>(xi + ((int64_t)(glo + gg) * n_geo + gcol[s]) * 8);
+                            const double2 x0 = __ldg(xp), x1 = __ldg(xp + 1), x2 = __ldg(xp + 2), x3 = __ldg(xp + 3);
+                            double* d = X + i;
+                            d[0] = x0.x; d[ps] = x0.y; d[2 * ps] = x1.x; d[3 * ps] = x1.y;
+                            d[4 * ps] = x2.x; d[5 * ps] = x2.y; d[6 * ps] = x3.x; d[7 * ps] = x3.y;
+                            gg += dq; s += dr;
+                            if (s >= cs) { s -= cs; ++gg; }
                         }
+                    }
                     __syncthreads();
                     // this warp's share of the chunk's channels gamma', two at a time (their value loads are independent);
                     // per gamma' the cs tile entries in steps of 4 (one MMA each), GM_UNR steps of loads in flight together
@@ -415,9 +429,9 @@ cudaError_t launch_spmv_blocked(const wpcd_grid* g, const wpcd_channels* ch, con
         const double* xv = x + (int64_t)v * rows;
         double* yv = y + (int64_t)v * rows;
         cudaError_t err;
-        // 5 .. 8 vectors: one tensor-core pass (7.1 ms on the 3.2e9-nonzero matrix whatever their number; the scalar kernels
-        // take 7.0 ms for 4 vectors, 4.6 for 2, 4.0 for 1)
-        if (n_vec - v >= 5 && ch->n_ch <= 8 * GM_GROUPS) {
+        // 3 .. 8 vectors: one tensor-core pass (6.7 ms on the 3.2e9-nonzero matrix whatever their number; the scalar kernels
+        // take 6.8 ms for 4 vectors, 4.4 for 2, 3.9 for 1)
+        if (n_vec - v >= 3 && ch->n_ch <= 8 * GM_GROUPS && g_debug.blocked_no_mma.load() == 0) {
             const int nv = std::min(8, n_vec - v);
             err = launch_georow_mma8(g, ch, geo_row_ptr, col_idx, values, xv, yv, rows, nv, st);
             v += nv;

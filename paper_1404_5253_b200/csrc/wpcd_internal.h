@@ -124,6 +124,7 @@ struct DebugSwitches {
     std::atomic<int> spmv_no_pipeline{0};        // 1: never take the software-pipelined long-row variant
     std::atomic<int> no_pdl{0};                  // 1: launch the products without programmatic dependent launch
     std::atomic<int> chain_mode{0};              // 1: fused chain whenever the matrix fits on chip, 2: never
+    std::atomic<int> blocked_no_mma{0};          // 1: the blocked product never takes the tensor-core pass (scalar passes of 8, 4, 2, 1 vectors)
     std::atomic<int> blocked_tile_doubles{0};    // > 0: size of the blocked product's x tile (small values exercise the chunked paths)
 };
 extern DebugSwitches g_debug;

@@ -988,8 +988,8 @@ def test_apply_blocked(wpcd):
 
 def test_apply_blocked_chunked_paths(wpcd):
     """The same product with a tiny x tile (wpcd_debug_set): geometric rows cut into column chunks, channels into channel
-    chunks, runs of coupled channels split at chunk boundaries; 1 .. 15 vectors per call (scalar passes of 1, 2 and 4 vectors,
-    tensor-core passes of 5 .. 8)."""
+    chunks, runs of coupled channels split at chunk boundaries; 1 .. 15 vectors per call (scalar passes of 1 and 2 vectors,
+    tensor-core passes of 3 .. 8; with "blocked_no_mma" the scalar passes of 4 and 8 vectors)."""
     torch = _torch()
     gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=3, parity=1, two_T=1, j_pair_max=2)
     p, q = wi.tan2_grid(9, 1.0, 0.1, seed=41), wi.tan2_grid(11, 0.8, 0.1, seed=42)
@@ -997,8 +997,9 @@ def test_apply_blocked_chunked_paths(wpcd):
     m = wpcd.build_perm(grid, gch, 4)
     rp, ci, v = m.row_ptr.cpu().numpy(), m.col_idx.cpu().numpy(), m.values.cpu().numpy()
     try:
-        for tile in (0, 7, 40, 256):
+        for tile, no_mma in ((0, 0), (7, 0), (40, 0), (256, 0), (0, 1), (40, 1)):
             wpcd.wpcd_debug_set("blocked_tile_doubles", tile)
+            wpcd.wpcd_debug_set("blocked_no_mma", no_mma)          # 1: the scalar passes of 4 and 8 vectors as well
             for n_vec in (1, 2, 3, 5, 6, 9, 12, 15):
                 xs = np.stack([wi.normal_vector(m.rows, k=820 + k) for k in range(n_vec)])
                 x = torch.from_numpy(xs).cuda()
@@ -1012,6 +1013,7 @@ def test_apply_blocked_chunked_paths(wpcd):
                     assert np.all(np.abs(yh[k] - ref) <= 1e-12 * scale + 1e-300), (tile, n_vec, k)
     finally:
         wpcd.wpcd_debug_set("blocked_tile_doubles", 0)
+        wpcd.wpcd_debug_set("blocked_no_mma", 0)
 
 
 def _chain_check(wpcd, torch, rows, rp, ci, v, rpd, cid, vd, n_iter, tag):

@@ -48,7 +48,7 @@ def test_noalloc_product_matches_the_existing_path_twice_in_a_row(wpcd):
                     scale = operm.spmv(rp, ci_, np.abs(v), np.abs(xs[k]))
                     assert np.all(np.abs(ys[0][k] - yr[k]) <= SPMV_RTOL * scale + 1e-300), (rep, ci, n_vec, k)
                     assert np.all(np.abs(ys[0][k] - ref) <= SPMV_RTOL * scale + 1e-300), (rep, ci, n_vec, k)
-                if n_vec >= 5:                                             # the existing path takes the same kernel: same bits
+                if n_vec >= 3:                                             # the existing path takes the same kernel: same bits
                     assert np.array_equal(ys[0][:n_vec], yr)
 
 

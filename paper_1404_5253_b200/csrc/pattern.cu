@@ -383,7 +383,7 @@ cudaError_t ensure_stage(const wpcd_grid* g, int64_t want_cap)
         cudaGetDevice(&dev);
         std::lock_guard<std::mutex> lock(attr_mutex);
         size_t& have = attr_max[dev];
-        if (need > 48 * 1024 && need > have) {
+        if (need > 32 * 1024 && need > have) {      // the default 48 KB limit counts the static shared memory too
             if ((err = cudaFuncSetAttribute(geo_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need)) != cudaSuccess) return err;
             have = need;
         }

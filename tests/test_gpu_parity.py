@@ -1016,6 +1016,29 @@ def test_apply_blocked_chunked_paths(wpcd):
         wpcd.wpcd_debug_set("blocked_no_mma", 0)
 
 
+def test_dynamic_shared_memory_just_under_the_default_limit(wpcd):
+    """A launch whose DYNAMIC shared memory is within a few bytes below 48 KB while static + dynamic is above it: the
+    opt-in limit has to be raised although the dynamic part alone would fit the default (10 channels, one vector, x tile of
+    4089 doubles: 12 * 4089 + 8 * 10 = 49 148 bytes + 16 static)."""
+    torch = _torch()
+    gch = wpcd.wpcd_channels_create(wpcd.WPCD_ND, two_J=1, parity=1, two_T=1, j_pair_max=1)
+    assert gch.count == 10
+    p = wi.tan2_grid(8, 1.0, 0.1, seed=95)
+    grid = wpcd.wpcd_grid_create(p, p)
+    m = wpcd.build_perm(grid, gch, 4)
+    xs = wi.normal_vector(m.rows, k=1700)
+    x = torch.from_numpy(xs[None, :].copy()).cuda()
+    y0, y1 = torch.empty_like(x), torch.full_like(x, np.nan)
+    wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y0)
+    try:
+        wpcd.wpcd_debug_set("blocked_tile_doubles", 4089)
+        wpcd.wpcd_perm_apply_blocked(grid, gch, m.row_ptr, m.geo_row_ptr, m.col_idx, m.values, x, y1)
+    finally:
+        wpcd.wpcd_debug_set("blocked_tile_doubles", 0)
+    torch.cuda.synchronize()
+    assert torch.equal(y0, y1)
+
+
 def _chain_check(wpcd, torch, rows, rp, ci, v, rpd, cid, vd, n_iter, tag):
     xh = wi.normal_vector(rows, k=900)
     x = torch.from_numpy(xh).cuda()
